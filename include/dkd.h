@@ -1,0 +1,155 @@
+/*
+ * dkd.h — C-ABI boundary of libdkd: B200-native (sm_100a) keypoint post-processing for learned
+ * visual front-ends: ALIKED-style Differentiable Keypoint Detection (DKD) + descriptor sampling.
+ *
+ * Reference: /root/reference/PAPER.md ("DL-VINS-Factory", arxiv/paper_2607_01757)
+ *   PAPER.md:84-86   (Sec. III-A)  score map -> DKD -> sub-pixel keypoints
+ *   PAPER.md:97-101  (Eq. 1)       Phi(I) = {(p_i, d_i, s_i)}: pixel coordinates p_i in R^2,
+ *                                  l2-normalised descriptors d_i in R^D, D in {64,128,256}, s_i in [0,1]
+ *   PAPER.md:118                   LK pathway needs keypoints only (desc == NULL here)
+ *   PAPER.md:120-122 (Sec. III-A)  custom CUDA DKD: NMS, sorting, patch extraction; dynamic count
+ *   PAPER.md:128,132               stereo pair processed as one batch (B = 2)
+ *   PAPER.md:139                   sets zero-padded to the keypoint cap (static shapes downstream)
+ * The paper prints no formula for these steps; the exact arithmetic is fixed by BASELINE.json
+ * `north_star` steps (1)-(4) and the readings G1..G21 in DESIGN.md.
+ *
+ * C99, no C++ types, no exceptions cross the boundary.  All `device` pointers are CUDA device
+ * memory on the context's device; `host` pointers are ordinary (preferably pinned) host memory.
+ * The caller owns every input/output buffer and the stream; a dkd_ctx owns only its workspace.
+ */
+#ifndef DKD_H_
+#define DKD_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dkd_ctx dkd_ctx;   /* opaque */
+
+/* return codes: 0 = OK, negative = error; on INVALID_ARG / UNSUPPORTED / CAPACITY nothing was
+ * launched and no output was written. */
+enum {
+    DKD_OK = 0,
+    DKD_ERR_INVALID_ARG = -1,   /* NULL required pointer, size < 1, r < 1, T <= 0 or non-finite, ... */
+    DKD_ERR_UNSUPPORTED = -2,   /* r > DKD_MAX_RADIUS; D*elemsize not a multiple of 16 B or > DKD_MAX_ROW_BYTES;
+                                   desc/out_desc not 16-byte aligned; score not 4-byte aligned; unknown dtype */
+    DKD_ERR_CAPACITY = -3,      /* B, H, W, top_k or D above the dkd_create maxima */
+    DKD_ERR_CUDA = -4           /* CUDA runtime/driver failure; text in dkd_last_error() */
+};
+
+enum { DKD_F32 = 0, DKD_F16 = 1 };          /* descriptor-map element type */
+
+#define DKD_MAX_RADIUS    4                 /* (2r+1)^2 window, r in [1,4] (paper's extractors use 2..4) */
+#define DKD_MAX_TOP_K     8192              /* per-image cap (paper: 160..384) */
+#define DKD_MAX_ROW_BYTES 2048              /* D * elemsize of one descriptor row */
+
+/* options for dkd_set_option (defaults in brackets) */
+enum {
+    DKD_OPT_USE_GRAPH = 0,   /* [1] run each dkd_extract as ONE cached CUDA-graph launch (north_star:
+                                "the whole stereo pair in one CUDA-graph launch"); 0 = plain launches.
+                                Ignored (plain launches) while `stream` is being captured by the caller. */
+    DKD_OPT_USE_TMA   = 1    /* [1] NMS tiles staged by TMA (cp.async.bulk.tensor) when W % 4 == 0 and
+                                score is 16-byte aligned; 0 = always the plain-load tile loader. */
+};
+
+typedef struct {
+    int device;                 /* CUDA ordinal */
+    int max_batch, max_h, max_w;
+    int max_top_k;              /* <= DKD_MAX_TOP_K */
+    int max_dim;                /* max D (0 = keypoints only) */
+} dkd_create_params;
+
+/* Allocates the workspace once on p->device (candidate keys sized for the worst case — every
+ * interior pixel a candidate — so selection is exact on any input).
+ * Returns DKD_OK and *out, or an error (and *out = NULL). */
+int dkd_create(const dkd_create_params* p, dkd_ctx** out);
+
+/* Frees the workspace.  NULL is a no-op -> DKD_OK.  The caller must have synchronised any stream
+ * that still runs work enqueued through this context. */
+int dkd_destroy(dkd_ctx* ctx);
+
+/* Text of the last error on this context (ctx-owned, valid until the next call on ctx);
+ * with ctx == NULL, the text of the last dkd_create failure (static storage). */
+const char* dkd_last_error(const dkd_ctx* ctx);
+
+/* Device bytes owned by the context. */
+size_t dkd_workspace_bytes(const dkd_ctx* ctx);
+
+int dkd_set_option(dkd_ctx* ctx, int option, int value);
+
+/*
+ * dkd_extract — the whole hot path for a batch of B independent images (north_star steps 1-4;
+ * PAPER.md:120-122 stages; Eq. 1 outputs):
+ *   (1) mask = r-pixel border exclusion AND S > thresh (strict) AND S >= every S in the (2r+1)^2
+ *       window (ties are all maxima);
+ *   (2) per image keep K_b = min(top_k, #candidates) ordered by (score desc, linear index y*W+x asc)
+ *       — selection on the float bits, bit-exact;
+ *   (3) soft-argmax over the same window: w = exp((S - S_centre)/T), (dx,dy) = sum w*(i,j) / sum w,
+ *       p = (x+dx, y+dy) in score-map pixel units, (x,y) order;
+ *   (4) if desc != NULL: bilinear sample of the channel-last map at u = (px+0.5)/stride - 0.5
+ *       (likewise v), clamped to the map, fp32 accumulation, divided by max(||d||_2, 1e-12);
+ *   (5) slots i >= K_b are zero-filled.
+ *
+ *   score      device [B,H,W] f32, contiguous.                                   (read only)
+ *   desc       device [B,Hd,Wd,D] channel-last, DKD_F16 or DKD_F32, contiguous, 16-byte aligned,
+ *              or NULL to skip step (4) (then out_desc must be NULL).  Hd*stride, Wd*stride need
+ *              not equal H, W: sampling positions are clamped to the map.           (read only)
+ *   out_kpts   device [B,top_k,2] f32 (x,y)
+ *   out_scores device [B,top_k]   f32, raw S at the integer peak (bit-identical to the input)
+ *   out_desc   device [B,top_k,D] same element type as desc, 16-byte aligned
+ *   out_count  device [B] i32 = K_b
+ *   stream     cudaStream_t (NULL = legacy default stream)
+ *
+ * Asynchronous and stream-ordered: no host synchronisation, no allocation, no host read of the
+ * counts; outputs are valid once `stream` reaches the end of the enqueued work.  One context must
+ * not be used from two streams concurrently (the workspace is shared).  Outputs are a pure
+ * function of the inputs (deterministic).  Non-finite scores are outside the contract.
+ */
+int dkd_extract(dkd_ctx* ctx,
+                const float* score, int B, int H, int W,
+                const void* desc, int desc_dtype, int Hd, int Wd, int D, int stride,
+                int r, float thresh, int top_k, float T,
+                float* out_kpts, float* out_scores, void* out_desc, int32_t* out_count,
+                void* stream);
+
+/* dkd_extract plus two optional outputs (either may be NULL):
+ *   out_index  device [B,top_k] i32: linear index y*W+x of the integer peak, -1 in padding
+ *              (integer positions cannot be recovered from the refined coordinates);
+ *   out_offset device [B,top_k,2] f32: the sub-pixel offset (dx,dy) before it is added to (x,y)
+ *              (the 1e-5 px parity bound applies to this; G11). */
+int dkd_extract_ex(dkd_ctx* ctx,
+                   const float* score, int B, int H, int W,
+                   const void* desc, int desc_dtype, int Hd, int Wd, int D, int stride,
+                   int r, float thresh, int top_k, float T,
+                   float* out_kpts, float* out_scores, void* out_desc, int32_t* out_count,
+                   int32_t* out_index, float* out_offset,
+                   void* stream);
+
+/*
+ * dkd_extract_host — the same call with HOST buffers (the end-to-end path): copies score (and desc)
+ * host->device into context-owned staging buffers, runs dkd_extract_ex, copies every non-NULL
+ * output device->host, and synchronises `stream` before returning.  Staging is (re)allocated on
+ * first use / growth.  Pointers have the shapes above; pinned memory makes the copies asynchronous.
+ * desc_resident != 0 reuses the descriptor map uploaded by the previous call with the same
+ * desc pointer and shape (a dense network would leave it on the device).
+ */
+int dkd_extract_host(dkd_ctx* ctx,
+                     const float* score, int B, int H, int W,
+                     const void* desc, int desc_dtype, int Hd, int Wd, int D, int stride,
+                     int r, float thresh, int top_k, float T,
+                     float* out_kpts, float* out_scores, void* out_desc, int32_t* out_count,
+                     int32_t* out_index, float* out_offset,
+                     int desc_resident, void* stream);
+
+/* Number of kernels one dkd_extract launches for these arguments (for launch accounting). */
+int dkd_launches_per_extract(const dkd_ctx* ctx, int with_desc);
+
+const char* dkd_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DKD_H_ */

@@ -1,0 +1,213 @@
+"""ctypes binding of include/dkd.h — same names, argument marshalling only."""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+from typing import Optional
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+F32, F16 = 0, 1
+OPT_USE_GRAPH, OPT_USE_TMA = 0, 1
+MAX_RADIUS, MAX_TOP_K, MAX_ROW_BYTES = 4, 8192, 2048
+
+EXPORTED_SYMBOLS = (
+    "dkd_create", "dkd_destroy", "dkd_last_error", "dkd_workspace_bytes", "dkd_set_option",
+    "dkd_extract", "dkd_extract_ex", "dkd_extract_host", "dkd_launches_per_extract", "dkd_version",
+)
+
+
+class DKDError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"dkd error {code}: {msg}")
+        self.code = code
+
+
+class _CreateParams(ctypes.Structure):
+    _fields_ = [("device", ctypes.c_int), ("max_batch", ctypes.c_int), ("max_h", ctypes.c_int),
+                ("max_w", ctypes.c_int), ("max_top_k", ctypes.c_int), ("max_dim", ctypes.c_int)]
+
+
+def lib_path() -> str:
+    return os.path.join(_HERE, "libdkd.so")
+
+
+_lib = None
+
+
+def load_library():
+    """Loads libdkd.so (in-tree).  Fails loudly if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = lib_path()
+    if not os.path.exists(path):
+        raise DKDError(-4, f"{path} not built — run `python -m paper_2607_01757_b200.build` "
+                           "(or __graft_entry__.build()); there is no CPU fallback")
+    L = ctypes.CDLL(path)
+    vp, i, f = ctypes.c_void_p, ctypes.c_int, ctypes.c_float
+    L.dkd_create.restype = i
+    L.dkd_create.argtypes = [ctypes.POINTER(_CreateParams), ctypes.POINTER(vp)]
+    L.dkd_destroy.restype = i
+    L.dkd_destroy.argtypes = [vp]
+    L.dkd_last_error.restype = ctypes.c_char_p
+    L.dkd_last_error.argtypes = [vp]
+    L.dkd_workspace_bytes.restype = ctypes.c_size_t
+    L.dkd_workspace_bytes.argtypes = [vp]
+    L.dkd_set_option.restype = i
+    L.dkd_set_option.argtypes = [vp, i, i]
+    L.dkd_launches_per_extract.restype = i
+    L.dkd_launches_per_extract.argtypes = [vp, i]
+    L.dkd_version.restype = ctypes.c_char_p
+    common = [vp, vp, i, i, i, vp, i, i, i, i, i, i, f, i, f, vp, vp, vp, vp]
+    L.dkd_extract.restype = i
+    L.dkd_extract.argtypes = common + [vp]
+    L.dkd_extract_ex.restype = i
+    L.dkd_extract_ex.argtypes = common + [vp, vp, vp]
+    L.dkd_extract_host.restype = i
+    L.dkd_extract_host.argtypes = common + [vp, vp, i, vp]
+    _lib = L
+    return L
+
+
+@dataclass
+class DKDResult:
+    kpts: torch.Tensor                 # [B,k,2] f32 (x,y)
+    scores: torch.Tensor               # [B,k]   f32
+    desc: Optional[torch.Tensor]       # [B,k,D] f16|f32
+    count: torch.Tensor                # [B]     i32
+    index: Optional[torch.Tensor]      # [B,k]   i32 (-1 padding)
+    offsets: Optional[torch.Tensor]    # [B,k,2] f32 (dx,dy)
+
+
+def _dt(t: Optional[torch.Tensor]) -> int:
+    if t is None or t.dtype == torch.float32:
+        return F32
+    if t.dtype == torch.float16:
+        return F16
+    raise DKDError(-2, "descriptor map must be float16 or float32")
+
+
+def _ptr(t: Optional[torch.Tensor]):
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+class DKD:
+    """One context = one device workspace.  `extract` mirrors dkd_extract_ex, `extract_host`
+    mirrors dkd_extract_host."""
+
+    def __init__(self, max_batch: int, max_h: int, max_w: int, max_top_k: int, max_dim: int = 0,
+                 device: int = 0):
+        self._h = None
+        L = load_library()
+        if not torch.cuda.is_available():
+            raise DKDError(-4, "no CUDA device: libdkd has no CPU fallback")
+        self._L = L
+        self.device = torch.device("cuda", device)
+        p = _CreateParams(device, max_batch, max_h, max_w, max_top_k, max_dim)
+        h = ctypes.c_void_p()
+        rc = L.dkd_create(ctypes.byref(p), ctypes.byref(h))
+        if rc != 0:
+            raise DKDError(rc, L.dkd_last_error(None).decode())
+        self._h = h
+
+    def close(self):
+        if self._h is not None:
+            self._L.dkd_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc: int):
+        if rc != 0:
+            raise DKDError(rc, self._L.dkd_last_error(self._h).decode())
+
+    def set_option(self, option: int, value: int):
+        self._check(self._L.dkd_set_option(self._h, option, value))
+
+    @property
+    def workspace_bytes(self) -> int:
+        return int(self._L.dkd_workspace_bytes(self._h))
+
+    def launches_per_extract(self, with_desc: bool = True) -> int:
+        return int(self._L.dkd_launches_per_extract(self._h, int(with_desc)))
+
+    # -- device buffers ---------------------------------------------------------------------
+    def alloc_outputs(self, B: int, top_k: int, desc: Optional[torch.Tensor], D: int = 0,
+                      want_index=True, want_offsets=True, device=None, pin=False) -> DKDResult:
+        dev = self.device if device is None else device
+        kw = dict(device=dev, pin_memory=pin) if pin else dict(device=dev)
+        return DKDResult(
+            kpts=torch.empty((B, top_k, 2), dtype=torch.float32, **kw),
+            scores=torch.empty((B, top_k), dtype=torch.float32, **kw),
+            desc=None if desc is None else torch.empty((B, top_k, D), dtype=desc.dtype, **kw),
+            count=torch.empty((B,), dtype=torch.int32, **kw),
+            index=torch.empty((B, top_k), dtype=torch.int32, **kw) if want_index else None,
+            offsets=torch.empty((B, top_k, 2), dtype=torch.float32, **kw) if want_offsets else None,
+        )
+
+    def extract(self, score: torch.Tensor, desc: Optional[torch.Tensor], stride: int, r: int,
+                thresh: float, top_k: int, T: float, out: Optional[DKDResult] = None,
+                stream: Optional[torch.cuda.Stream] = None, want_index=True, want_offsets=True) -> DKDResult:
+        """score [B,H,W] f32 cuda contiguous; desc [B,Hd,Wd,D] f16|f32 cuda contiguous or None.
+        Asynchronous on `stream` (default: the current torch stream)."""
+        if not (score.is_cuda and score.is_contiguous() and score.dtype == torch.float32 and score.dim() == 3):
+            raise DKDError(-1, "score must be a contiguous CUDA float32 [B,H,W] tensor")
+        B, H, W = score.shape
+        Hd = Wd = D = 0
+        if desc is not None:
+            if not (desc.is_cuda and desc.is_contiguous() and desc.dim() == 4 and desc.shape[0] == B):
+                raise DKDError(-1, "desc must be a contiguous CUDA [B,Hd,Wd,D] tensor")
+            _, Hd, Wd, D = desc.shape
+        if out is None:
+            out = self.alloc_outputs(B, top_k, desc, D, want_index, want_offsets)
+        st = torch.cuda.current_stream(self.device) if stream is None else stream
+        rc = self._L.dkd_extract_ex(self._h, _ptr(score), B, H, W, _ptr(desc), _dt(desc), Hd, Wd, D,
+                                    int(stride), int(r), float(thresh), int(top_k), float(T),
+                                    _ptr(out.kpts), _ptr(out.scores), _ptr(out.desc), _ptr(out.count),
+                                    _ptr(out.index), _ptr(out.offsets), ctypes.c_void_p(st.cuda_stream))
+        self._check(rc)
+        return out
+
+    def extract_literal(self, score, desc, stride, r, thresh, top_k, T, out: DKDResult, stream=None):
+        """dkd_extract (the literal north_star signature: no index / offset outputs)."""
+        B, H, W = score.shape
+        Hd = Wd = D = 0
+        if desc is not None:
+            _, Hd, Wd, D = desc.shape
+        st = torch.cuda.current_stream(self.device) if stream is None else stream
+        rc = self._L.dkd_extract(self._h, _ptr(score), B, H, W, _ptr(desc), _dt(desc), Hd, Wd, D,
+                                 int(stride), int(r), float(thresh), int(top_k), float(T),
+                                 _ptr(out.kpts), _ptr(out.scores), _ptr(out.desc), _ptr(out.count),
+                                 ctypes.c_void_p(st.cuda_stream))
+        self._check(rc)
+        return out
+
+    def extract_host(self, score: torch.Tensor, desc: Optional[torch.Tensor], stride: int, r: int,
+                     thresh: float, top_k: int, T: float, out: Optional[DKDResult] = None,
+                     desc_resident: bool = False, stream: Optional[torch.cuda.Stream] = None) -> DKDResult:
+        """HOST tensors in, HOST tensors out (copies inside the call, synchronous on return)."""
+        if score.is_cuda or not score.is_contiguous() or score.dtype != torch.float32 or score.dim() != 3:
+            raise DKDError(-1, "score must be a contiguous CPU float32 [B,H,W] tensor")
+        B, H, W = score.shape
+        Hd = Wd = D = 0
+        if desc is not None:
+            if desc.is_cuda or not desc.is_contiguous() or desc.dim() != 4 or desc.shape[0] != B:
+                raise DKDError(-1, "desc must be a contiguous CPU [B,Hd,Wd,D] tensor")
+            _, Hd, Wd, D = desc.shape
+        if out is None:
+            out = self.alloc_outputs(B, top_k, desc, D, device="cpu", pin=True)
+        st = torch.cuda.current_stream(self.device) if stream is None else stream
+        rc = self._L.dkd_extract_host(self._h, _ptr(score), B, H, W, _ptr(desc), _dt(desc), Hd, Wd, D,
+                                      int(stride), int(r), float(thresh), int(top_k), float(T),
+                                      _ptr(out.kpts), _ptr(out.scores), _ptr(out.desc), _ptr(out.count),
+                                      _ptr(out.index), _ptr(out.offsets), int(desc_resident),
+                                      ctypes.c_void_p(st.cuda_stream))
+        self._check(rc)
+        return out

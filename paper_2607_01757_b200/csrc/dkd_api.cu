@@ -1,0 +1,427 @@
+// dkd_api.cu — host side of libdkd: the C-ABI of include/dkd.h (argument validation, workspace,
+// TMA descriptor, launches, CUDA-graph cache, host-buffer path).  See DESIGN.md.
+#include "dkd.h"
+
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <vector>
+
+#include "dkd_kernels.cuh"
+
+using namespace dkd;
+
+namespace {
+
+typedef CUresult (*PFN_tensorMapEncodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                             const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
+                                             CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                             CUtensorMapFloatOOBfill);
+
+char g_create_error[512] = "";
+
+struct ExtractArgs {                       // everything that determines the enqueued work
+    const float* score;
+    int B, H, W;
+    const void* desc;
+    int desc_dtype, Hd, Wd, D, stride, r;
+    float thresh;
+    int top_k;
+    float T;
+    float* out_kpts;
+    float* out_scores;
+    void* out_desc;
+    int32_t* out_count;
+    int32_t* out_index;
+    float* out_offset;
+    int use_tma;
+};
+
+struct GraphEntry {
+    ExtractArgs key;
+    cudaGraphExec_t exec;
+    unsigned long long last_use;
+};
+
+constexpr size_t GRAPH_CACHE_CAP = 256;
+
+}  // namespace
+
+struct dkd_ctx {
+    dkd_create_params p;
+    int num_sms;
+    int nms_ctas_per_sm[MAX_R + 1];
+    PFN_tensorMapEncodeTiled encode;
+    // workspace (device)
+    uint64_t* cand;          // [max_tiles * TILE_PX] candidate keys, one private segment per tile
+    int* tile_cnt;           // [max_tiles]
+    int32_t* sel_idx;        // [max_batch * max_top_k]
+    size_t max_tiles;
+    size_t ws_bytes;
+    // host-path staging (device), grown on demand
+    void* st_score; size_t st_score_bytes;
+    void* st_desc;  size_t st_desc_bytes;
+    void* st_out;   size_t st_out_bytes;
+    const void* st_desc_src; size_t st_desc_src_bytes;      // what st_desc currently holds
+    // options
+    int use_graph, use_tma;
+    std::vector<GraphEntry> graphs;
+    unsigned long long tick;
+    char err[512];
+};
+
+namespace {
+
+int fail(dkd_ctx* ctx, int code, const char* fmt, const char* a = "", const char* b = "") {
+    if (ctx) snprintf(ctx->err, sizeof(ctx->err), fmt, a, b);
+    return code;
+}
+int fail_cuda(dkd_ctx* ctx, const char* what, cudaError_t e) {
+    return fail(ctx, DKD_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+#define CK(ctx, call)                                                  \
+    do {                                                               \
+        cudaError_t e_ = (call);                                       \
+        if (e_ != cudaSuccess) return fail_cuda((ctx), #call, e_);     \
+    } while (0)
+
+template <int R>
+cudaError_t setup_nms(dkd_ctx* ctx) {
+    cudaError_t e = cudaFuncSetAttribute(k_nms_tma<R>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         NMS_STAGES * stage_bytes(R));
+    if (e != cudaSuccess) return e;
+    int n = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_nms_tma<R>, NMS_THREADS, NMS_STAGES * stage_bytes(R));
+    ctx->nms_ctas_per_sm[R] = n > 0 ? n : 1;
+    return e;
+}
+
+template <int R>
+cudaError_t launch_nms(dkd_ctx* ctx, const ExtractArgs& a, int tiles_x, int tiles_y, int total, cudaStream_t st) {
+    if (a.use_tma) {
+        CUtensorMap tmap;
+        const cuuint64_t dims[3] = {(cuuint64_t)a.W, (cuuint64_t)a.H, (cuuint64_t)a.B};
+        const cuuint64_t strides[2] = {(cuuint64_t)a.W * 4, (cuuint64_t)a.W * a.H * 4};
+        const cuuint32_t box[3] = {(cuuint32_t)PITCH, (cuuint32_t)tile_rows(R), 1};
+        const cuuint32_t estr[3] = {1, 1, 1};
+        CUresult r = ctx->encode(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(a.score), dims, strides,
+                                 box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                 CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+        int grid = ctx->num_sms * ctx->nms_ctas_per_sm[R];
+        if (grid > total) grid = total;
+        k_nms_tma<R><<<grid, NMS_THREADS, NMS_STAGES * stage_bytes(R), st>>>(tmap, a.H, a.W, tiles_x, tiles_y, total,
+                                                                             a.thresh, ctx->cand, ctx->tile_cnt);
+    } else {
+        k_nms_plain<R><<<total, NMS_THREADS, 0, st>>>(a.score, a.H, a.W, tiles_x, tiles_y, a.thresh, ctx->cand,
+                                                      ctx->tile_cnt);
+    }
+    return cudaGetLastError();
+}
+
+template <int R>
+cudaError_t launch_rg(const ExtractArgs& a, const int32_t* sel, cudaStream_t st) {
+    const int nslots = a.B * a.top_k;
+    const int grid = (nslots + RG_THREADS / 32 - 1) / (RG_THREADS / 32);
+    const unsigned char* d = static_cast<const unsigned char*>(a.desc);
+    unsigned char* od = static_cast<unsigned char*>(a.out_desc);
+#define RG_ARGS a.score, a.H, a.W, sel, nslots, a.top_k, a.T, d, a.Hd, a.Wd, a.D, a.stride, a.out_kpts, a.out_scores, a.out_offset, od
+    if (a.desc == nullptr)
+        k_refine_gather<R, -1><<<grid, RG_THREADS, 0, st>>>(RG_ARGS);
+    else if (a.desc_dtype == DKD_F16)
+        k_refine_gather<R, DKD_F16><<<grid, RG_THREADS, 0, st>>>(RG_ARGS);
+    else
+        k_refine_gather<R, DKD_F32><<<grid, RG_THREADS, 0, st>>>(RG_ARGS);
+#undef RG_ARGS
+    return cudaGetLastError();
+}
+
+// Enqueue the three kernels of one extract on `st`.  No sync, no allocation: capture-safe.
+cudaError_t enqueue(dkd_ctx* ctx, const ExtractArgs& a, cudaStream_t st) {
+    const int tiles_x = (a.W + TW - 1) / TW, tiles_y = (a.H + TH - 1) / TH;
+    const int tpi = tiles_x * tiles_y, total = tpi * a.B;
+    cudaError_t e;
+    switch (a.r) {
+        case 1: e = launch_nms<1>(ctx, a, tiles_x, tiles_y, total, st); break;
+        case 2: e = launch_nms<2>(ctx, a, tiles_x, tiles_y, total, st); break;
+        case 3: e = launch_nms<3>(ctx, a, tiles_x, tiles_y, total, st); break;
+        default: e = launch_nms<4>(ctx, a, tiles_x, tiles_y, total, st); break;
+    }
+    if (e != cudaSuccess) return e;
+    int32_t* sel = a.out_index ? a.out_index : ctx->sel_idx;
+    k_select<<<a.B, SEL_THREADS, SORT_CAP * sizeof(uint64_t), st>>>(ctx->cand, ctx->tile_cnt, tpi, a.top_k, sel,
+                                                                    a.out_count);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    switch (a.r) {
+        case 1: return launch_rg<1>(a, sel, st);
+        case 2: return launch_rg<2>(a, sel, st);
+        case 3: return launch_rg<3>(a, sel, st);
+        default: return launch_rg<4>(a, sel, st);
+    }
+}
+
+int validate(dkd_ctx* ctx, const ExtractArgs& a) {
+    if (!ctx) return DKD_ERR_INVALID_ARG;
+    if (!a.score || !a.out_kpts || !a.out_scores || !a.out_count)
+        return fail(ctx, DKD_ERR_INVALID_ARG, "NULL required pointer (score/out_kpts/out_scores/out_count)");
+    if (a.B < 1 || a.H < 1 || a.W < 1 || a.top_k < 1) return fail(ctx, DKD_ERR_INVALID_ARG, "B, H, W, top_k must be >= 1");
+    if (a.r < 1) return fail(ctx, DKD_ERR_INVALID_ARG, "r must be >= 1");
+    if (!(a.T > 0.0f) || !isfinite(a.T)) return fail(ctx, DKD_ERR_INVALID_ARG, "T must be finite and > 0");
+    if (isnan(a.thresh)) return fail(ctx, DKD_ERR_INVALID_ARG, "thresh is NaN");
+    if ((a.desc == nullptr) != (a.out_desc == nullptr))
+        return fail(ctx, DKD_ERR_INVALID_ARG, "desc and out_desc must both be NULL or both be set");
+    if (a.desc) {
+        if (a.Hd < 1 || a.Wd < 1 || a.D < 1 || a.stride < 1)
+            return fail(ctx, DKD_ERR_INVALID_ARG, "Hd, Wd, D, stride must be >= 1");
+        if (a.desc_dtype != DKD_F32 && a.desc_dtype != DKD_F16)
+            return fail(ctx, DKD_ERR_UNSUPPORTED, "desc_dtype must be DKD_F32 or DKD_F16");
+    }
+    if (a.r > DKD_MAX_RADIUS) return fail(ctx, DKD_ERR_UNSUPPORTED, "r > DKD_MAX_RADIUS");
+    if (reinterpret_cast<uintptr_t>(a.score) & 3) return fail(ctx, DKD_ERR_UNSUPPORTED, "score not 4-byte aligned");
+    if (a.desc) {
+        const size_t rowb = static_cast<size_t>(a.D) * (a.desc_dtype == DKD_F16 ? 2 : 4);
+        if (rowb % 16 != 0 || rowb > DKD_MAX_ROW_BYTES)
+            return fail(ctx, DKD_ERR_UNSUPPORTED, "D * elemsize must be a multiple of 16 and <= DKD_MAX_ROW_BYTES");
+        if ((reinterpret_cast<uintptr_t>(a.desc) & 15) || (reinterpret_cast<uintptr_t>(a.out_desc) & 15))
+            return fail(ctx, DKD_ERR_UNSUPPORTED, "desc / out_desc not 16-byte aligned");
+        if (a.D > ctx->p.max_dim) return fail(ctx, DKD_ERR_CAPACITY, "D > max_dim");
+        if (static_cast<long long>(a.stride) * 2 > 0x3fffffff) return fail(ctx, DKD_ERR_UNSUPPORTED, "stride too large");
+    }
+    if (a.B > ctx->p.max_batch || a.H > ctx->p.max_h || a.W > ctx->p.max_w || a.top_k > ctx->p.max_top_k)
+        return fail(ctx, DKD_ERR_CAPACITY, "B, H, W or top_k above the dkd_create maxima");
+    return DKD_OK;
+}
+
+bool same_key(const ExtractArgs& x, const ExtractArgs& y) { return memcmp(&x, &y, sizeof(ExtractArgs)) == 0; }
+
+int run(dkd_ctx* ctx, ExtractArgs a, cudaStream_t st) {
+    int rc = validate(ctx, a);
+    if (rc != DKD_OK) return rc;
+    a.use_tma = ctx->use_tma && ctx->encode && (a.W % 4 == 0) && ((reinterpret_cast<uintptr_t>(a.score) & 15) == 0);
+
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    CK(ctx, cudaStreamIsCapturing(st, &cap));
+    if (!ctx->use_graph || cap != cudaStreamCaptureStatusNone) {
+        CK(ctx, enqueue(ctx, a, st));
+        return DKD_OK;
+    }
+    ++ctx->tick;
+    for (auto& g : ctx->graphs)
+        if (same_key(g.key, a)) {
+            g.last_use = ctx->tick;
+            CK(ctx, cudaGraphLaunch(g.exec, st));
+            return DKD_OK;
+        }
+    // first call with these arguments: capture the launches once, then replay as one graph launch
+    cudaGraph_t graph = nullptr;
+    CK(ctx, cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
+    cudaError_t e = enqueue(ctx, a, st);
+    cudaError_t e2 = cudaStreamEndCapture(st, &graph);
+    if (e != cudaSuccess || e2 != cudaSuccess) {
+        if (graph) cudaGraphDestroy(graph);
+        return fail_cuda(ctx, "graph capture", e != cudaSuccess ? e : e2);
+    }
+    cudaGraphExec_t exec = nullptr;
+    e = cudaGraphInstantiate(&exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) return fail_cuda(ctx, "cudaGraphInstantiate", e);
+    if (ctx->graphs.size() >= GRAPH_CACHE_CAP) {            // evict the least recently used entry
+        size_t v = 0;
+        for (size_t i = 1; i < ctx->graphs.size(); ++i)
+            if (ctx->graphs[i].last_use < ctx->graphs[v].last_use) v = i;
+        cudaGraphExecDestroy(ctx->graphs[v].exec);
+        ctx->graphs[v] = ctx->graphs.back();
+        ctx->graphs.pop_back();
+    }
+    GraphEntry ge;
+    ge.key = a;
+    ge.exec = exec;
+    ge.last_use = ctx->tick;
+    ctx->graphs.push_back(ge);
+    CK(ctx, cudaGraphLaunch(exec, st));
+    return DKD_OK;
+}
+
+int grow(dkd_ctx* ctx, void** buf, size_t* have, size_t need) {
+    if (need <= *have) return DKD_OK;
+    if (*buf) CK(ctx, cudaFree(*buf));
+    *buf = nullptr;
+    *have = 0;
+    CK(ctx, cudaMalloc(buf, need));
+    *have = need;
+    return DKD_OK;
+}
+
+size_t align256(size_t x) { return (x + 255) & ~static_cast<size_t>(255); }
+
+}  // namespace
+
+extern "C" {
+
+const char* dkd_version(void) { return "dkd-b200 0.1 (sm_100a)"; }
+
+int dkd_create(const dkd_create_params* p, dkd_ctx** out) {
+    if (out) *out = nullptr;
+    if (!p || !out) { snprintf(g_create_error, sizeof(g_create_error), "NULL argument"); return DKD_ERR_INVALID_ARG; }
+    if (p->max_batch < 1 || p->max_h < 1 || p->max_w < 1 || p->max_top_k < 1 || p->max_dim < 0 ||
+        static_cast<long long>(p->max_h) * p->max_w > 0x7fffffffLL) {
+        snprintf(g_create_error, sizeof(g_create_error), "invalid maxima");
+        return DKD_ERR_INVALID_ARG;
+    }
+    if (p->max_top_k > DKD_MAX_TOP_K) {
+        snprintf(g_create_error, sizeof(g_create_error), "max_top_k > DKD_MAX_TOP_K");
+        return DKD_ERR_UNSUPPORTED;
+    }
+    dkd_ctx* ctx = new dkd_ctx();
+    ctx->p = *p;
+    ctx->use_graph = 1;
+    ctx->use_tma = 1;
+    ctx->err[0] = 0;
+    ctx->tick = 0;
+#define CKC(call)                                                                                        \
+    do {                                                                                                 \
+        cudaError_t e_ = (call);                                                                         \
+        if (e_ != cudaSuccess) {                                                                         \
+            snprintf(g_create_error, sizeof(g_create_error), "%s: %s", #call, cudaGetErrorString(e_));   \
+            dkd_destroy(ctx);                                                                            \
+            return DKD_ERR_CUDA;                                                                         \
+        }                                                                                                \
+    } while (0)
+    CKC(cudaSetDevice(p->device));
+    CKC(cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, p->device));
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+        ctx->encode = reinterpret_cast<PFN_tensorMapEncodeTiled>(fn);
+    (void)cudaGetLastError();
+    CKC(setup_nms<1>(ctx));
+    CKC(setup_nms<2>(ctx));
+    CKC(setup_nms<3>(ctx));
+    CKC(setup_nms<4>(ctx));
+    CKC(cudaFuncSetAttribute(k_select, cudaFuncAttributeMaxDynamicSharedMemorySize, SORT_CAP * sizeof(uint64_t)));
+    const size_t tx = (p->max_w + TW - 1) / TW, ty = (p->max_h + TH - 1) / TH;
+    ctx->max_tiles = tx * ty * p->max_batch;
+    const size_t b_cand = align256(ctx->max_tiles * TILE_PX * sizeof(uint64_t));
+    const size_t b_cnt = align256(ctx->max_tiles * sizeof(int));
+    const size_t b_sel = align256(static_cast<size_t>(p->max_batch) * p->max_top_k * sizeof(int32_t));
+    CKC(cudaMalloc(&ctx->cand, b_cand));
+    CKC(cudaMalloc(&ctx->tile_cnt, b_cnt));
+    CKC(cudaMalloc(&ctx->sel_idx, b_sel));
+    ctx->ws_bytes = b_cand + b_cnt + b_sel;
+#undef CKC
+    *out = ctx;
+    return DKD_OK;
+}
+
+int dkd_destroy(dkd_ctx* ctx) {
+    if (!ctx) return DKD_OK;
+    for (auto& g : ctx->graphs) cudaGraphExecDestroy(g.exec);
+    if (ctx->cand) cudaFree(ctx->cand);
+    if (ctx->tile_cnt) cudaFree(ctx->tile_cnt);
+    if (ctx->sel_idx) cudaFree(ctx->sel_idx);
+    if (ctx->st_score) cudaFree(ctx->st_score);
+    if (ctx->st_desc) cudaFree(ctx->st_desc);
+    if (ctx->st_out) cudaFree(ctx->st_out);
+    delete ctx;
+    return DKD_OK;
+}
+
+const char* dkd_last_error(const dkd_ctx* ctx) { return ctx ? ctx->err : g_create_error; }
+
+size_t dkd_workspace_bytes(const dkd_ctx* ctx) {
+    return ctx ? ctx->ws_bytes + ctx->st_score_bytes + ctx->st_desc_bytes + ctx->st_out_bytes : 0;
+}
+
+int dkd_set_option(dkd_ctx* ctx, int option, int value) {
+    if (!ctx) return DKD_ERR_INVALID_ARG;
+    switch (option) {
+        case DKD_OPT_USE_GRAPH: ctx->use_graph = value != 0; return DKD_OK;
+        case DKD_OPT_USE_TMA: ctx->use_tma = value != 0; return DKD_OK;
+        default: return fail(ctx, DKD_ERR_INVALID_ARG, "unknown option");
+    }
+}
+
+int dkd_launches_per_extract(const dkd_ctx* ctx, int with_desc) {
+    (void)ctx;
+    (void)with_desc;
+    return 3;                                               // k_nms_*, k_select, k_refine_gather
+}
+
+int dkd_extract_ex(dkd_ctx* ctx, const float* score, int B, int H, int W, const void* desc, int desc_dtype, int Hd,
+                   int Wd, int D, int stride, int r, float thresh, int top_k, float T, float* out_kpts,
+                   float* out_scores, void* out_desc, int32_t* out_count, int32_t* out_index, float* out_offset,
+                   void* stream) {
+    ExtractArgs a;
+    memset(&a, 0, sizeof(a));                               // key is compared with memcmp: no stray padding
+    a.score = score; a.B = B; a.H = H; a.W = W;
+    a.desc = desc; a.desc_dtype = desc ? desc_dtype : 0; a.Hd = desc ? Hd : 0; a.Wd = desc ? Wd : 0;
+    a.D = desc ? D : 0; a.stride = desc ? stride : 1; a.r = r; a.thresh = thresh; a.top_k = top_k; a.T = T;
+    a.out_kpts = out_kpts; a.out_scores = out_scores; a.out_desc = out_desc; a.out_count = out_count;
+    a.out_index = out_index; a.out_offset = out_offset;
+    return run(ctx, a, static_cast<cudaStream_t>(stream));
+}
+
+int dkd_extract(dkd_ctx* ctx, const float* score, int B, int H, int W, const void* desc, int desc_dtype, int Hd,
+                int Wd, int D, int stride, int r, float thresh, int top_k, float T, float* out_kpts, float* out_scores,
+                void* out_desc, int32_t* out_count, void* stream) {
+    return dkd_extract_ex(ctx, score, B, H, W, desc, desc_dtype, Hd, Wd, D, stride, r, thresh, top_k, T, out_kpts,
+                          out_scores, out_desc, out_count, nullptr, nullptr, stream);
+}
+
+int dkd_extract_host(dkd_ctx* ctx, const float* score, int B, int H, int W, const void* desc, int desc_dtype, int Hd,
+                     int Wd, int D, int stride, int r, float thresh, int top_k, float T, float* out_kpts,
+                     float* out_scores, void* out_desc, int32_t* out_count, int32_t* out_index, float* out_offset,
+                     int desc_resident, void* stream) {
+    if (!ctx) return DKD_ERR_INVALID_ARG;
+    if (!score || !out_kpts || !out_scores || !out_count || B < 1 || H < 1 || W < 1 || top_k < 1)
+        return fail(ctx, DKD_ERR_INVALID_ARG, "NULL required pointer or size < 1");
+    if ((desc == nullptr) != (out_desc == nullptr))
+        return fail(ctx, DKD_ERR_INVALID_ARG, "desc and out_desc must both be NULL or both be set");
+    if (desc && (Hd < 1 || Wd < 1 || D < 1 || (desc_dtype != DKD_F32 && desc_dtype != DKD_F16)))
+        return fail(ctx, DKD_ERR_INVALID_ARG, "bad descriptor-map shape or dtype");
+    if (B > ctx->p.max_batch || H > ctx->p.max_h || W > ctx->p.max_w || top_k > ctx->p.max_top_k)
+        return fail(ctx, DKD_ERR_CAPACITY, "B, H, W or top_k above the dkd_create maxima");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t esz = desc_dtype == DKD_F16 ? 2 : 4;
+    const size_t n_score = static_cast<size_t>(B) * H * W * 4;
+    const size_t n_desc = desc ? static_cast<size_t>(B) * Hd * Wd * D * esz : 0;
+    const size_t slots = static_cast<size_t>(B) * top_k;
+    const size_t o_kpts = 0, o_scores = align256(o_kpts + slots * 8), o_count = align256(o_scores + slots * 4);
+    const size_t o_index = align256(o_count + static_cast<size_t>(B) * 4), o_off = align256(o_index + slots * 4);
+    const size_t o_desc = align256(o_off + slots * 8), n_out = align256(o_desc + (desc ? slots * D * esz : 0));
+    int rc;
+    if ((rc = grow(ctx, &ctx->st_score, &ctx->st_score_bytes, n_score)) != DKD_OK) return rc;
+    if ((rc = grow(ctx, &ctx->st_out, &ctx->st_out_bytes, n_out)) != DKD_OK) return rc;
+    if (desc) {
+        const bool have = desc_resident && ctx->st_desc && ctx->st_desc_src == desc && ctx->st_desc_src_bytes == n_desc;
+        if (!have) {
+            if ((rc = grow(ctx, &ctx->st_desc, &ctx->st_desc_bytes, n_desc)) != DKD_OK) return rc;
+            CK(ctx, cudaMemcpyAsync(ctx->st_desc, desc, n_desc, cudaMemcpyHostToDevice, st));
+            ctx->st_desc_src = desc;
+            ctx->st_desc_src_bytes = n_desc;
+        }
+    }
+    CK(ctx, cudaMemcpyAsync(ctx->st_score, score, n_score, cudaMemcpyHostToDevice, st));
+    char* so = static_cast<char*>(ctx->st_out);
+    rc = dkd_extract_ex(ctx, static_cast<const float*>(ctx->st_score), B, H, W, desc ? ctx->st_desc : nullptr,
+                        desc_dtype, Hd, Wd, D, stride, r, thresh, top_k, T, reinterpret_cast<float*>(so + o_kpts),
+                        reinterpret_cast<float*>(so + o_scores), desc ? so + o_desc : nullptr,
+                        reinterpret_cast<int32_t*>(so + o_count),
+                        out_index ? reinterpret_cast<int32_t*>(so + o_index) : nullptr,
+                        out_offset ? reinterpret_cast<float*>(so + o_off) : nullptr, st);
+    if (rc != DKD_OK) return rc;
+    CK(ctx, cudaMemcpyAsync(out_kpts, so + o_kpts, slots * 8, cudaMemcpyDeviceToHost, st));
+    CK(ctx, cudaMemcpyAsync(out_scores, so + o_scores, slots * 4, cudaMemcpyDeviceToHost, st));
+    CK(ctx, cudaMemcpyAsync(out_count, so + o_count, static_cast<size_t>(B) * 4, cudaMemcpyDeviceToHost, st));
+    if (out_index) CK(ctx, cudaMemcpyAsync(out_index, so + o_index, slots * 4, cudaMemcpyDeviceToHost, st));
+    if (out_offset) CK(ctx, cudaMemcpyAsync(out_offset, so + o_off, slots * 8, cudaMemcpyDeviceToHost, st));
+    if (desc) CK(ctx, cudaMemcpyAsync(out_desc, so + o_desc, slots * D * esz, cudaMemcpyDeviceToHost, st));
+    CK(ctx, cudaStreamSynchronize(st));
+    return DKD_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,77 @@
+"""The C-ABI library builds for sm_100a, loads, and exports every symbol include/dkd.h declares.
+No compute calls (no GPU here); the product path must fail loudly, never fall back to a CPU path."""
+import ctypes
+import os
+import re
+import subprocess
+
+import pytest
+import torch
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2607_01757_b200 import build
+    path = build.build()
+    return ctypes.CDLL(path)
+
+
+def declared_symbols():
+    src = open(os.path.join(ROOT, "include", "dkd.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(dkd_[a-z_]+)\s*\(", src)))
+
+
+def test_header_symbols_are_exported(lib):
+    import paper_2607_01757_b200 as dkd
+    syms = declared_symbols()
+    assert "dkd_create" in syms and "dkd_extract" in syms and "dkd_destroy" in syms and "dkd_extract_host" in syms
+    for s in syms:
+        assert getattr(lib, s) is not None, s
+    assert sorted(dkd.EXPORTED_SYMBOLS) == syms                  # the binding covers the whole header
+
+
+def test_header_is_plain_c():
+    out = os.path.join(ROOT, "tests", "_hdr_check.o")
+    try:
+        subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Werror", "-pedantic", "-x", "c", "-c",
+                               os.path.join(ROOT, "include", "dkd.h"), "-o", out])
+    finally:
+        if os.path.exists(out):
+            os.remove(out)
+
+
+def test_library_is_sm100a_with_tma():
+    from paper_2607_01757_b200 import build
+    path = build.build()
+    elf = subprocess.run(["cuobjdump", "-lelf", path], capture_output=True, text=True).stdout
+    assert "sm_100a" in elf
+    sass = subprocess.run(["cuobjdump", "-sass", "-fun", "_ZN3dkd9k_nms_tmaILi2EEEv14CUtensorMap_stiiiiifPmPi", path],
+                          capture_output=True, text=True).stdout
+    assert "UTMALDG" in sass                                     # TMA tile loads in the NMS kernel
+    assert "SYNCS" in sass                                       # mbarrier pipeline
+
+
+@pytest.mark.skipif(torch.cuda.is_available(), reason="CPU-only behaviour")
+def test_fails_loudly_without_gpu(lib):
+    import paper_2607_01757_b200 as dkd
+    with pytest.raises(dkd.DKDError):
+        dkd.DKD(1, 64, 64, 16)
+    lib.dkd_last_error.restype = ctypes.c_char_p
+    lib.dkd_last_error.argtypes = [ctypes.c_void_p]
+    assert lib.dkd_destroy(None) == 0                            # NULL is a no-op
+
+
+def test_product_never_imports_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2607_01757_b200")
+    for dp, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dp, f)).read()
+                assert "oracle" not in txt.lower(), f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            txt = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "import paper_2607_01757_b200" not in txt and "libdkd.so" not in txt

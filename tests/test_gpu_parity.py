@@ -1,0 +1,290 @@
+"""GPU parity: the CUDA path (through the C-ABI) vs the CPU oracle, element by element, on the same
+seeded inputs.  Sizes span several 128x32 tiles with ragged tails; configs c1-c5 run at full size
+(c5 in the launch configuration bench.py times; its oracle runs on every image for steps 1-3 and on
+sampled images for step 4).  north_star tolerances live in tests/_parity.py."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import synth
+from _parity import compare, run_both
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    import paper_2607_01757_b200 as dkd
+    c = dkd.DKD(max_batch=4, max_h=1100, max_w=1930, max_top_k=8192, max_dim=1024)
+    yield c
+    c.close()
+
+
+def small_inputs(B, H, W, seed, nblobs, D, dtype, stride, base=0.1):
+    score = synth.score_maps(B, H, W, seed, base, nblobs)
+    desc = None
+    if D:
+        desc = synth.desc_maps(B, max(H // stride, 1), max(W // stride, 1), D, seed, dtype, "cuda")
+    return score, desc
+
+
+# ---- multi-tile small cases, ragged tails, every radius, both loaders ---------------------------
+@pytest.mark.parametrize("r", [1, 2, 3, 4])
+@pytest.mark.parametrize("HW", [(75, 300), (67, 301), (33, 129), (200, 136)])
+def test_small_multitile(ctx, r, HW):
+    H, W = HW
+    score, desc = small_inputs(3, H, W, seed=10 * r + H, nblobs=150, D=64, dtype=torch.float16, stride=1)
+    res, ref = run_both(ctx, score, desc, 1, r, 0.2, 96, 0.1)
+    st = compare(res, ref, torch.float16)
+    assert ref.count.min() > 10
+    assert st["max_offset_err"] <= 1e-5
+
+
+@pytest.mark.parametrize("dtype,D", [(torch.float32, 4), (torch.float32, 64), (torch.float32, 512),
+                                      (torch.float16, 8), (torch.float16, 128), (torch.float16, 256),
+                                      (torch.float16, 1024), (torch.float16, 72)])
+@pytest.mark.parametrize("stride", [1, 2, 8])
+def test_descriptor_shapes_and_strides(ctx, dtype, D, stride):
+    score, desc = small_inputs(2, 96, 160, seed=D + stride, nblobs=120, D=D, dtype=dtype, stride=stride)
+    res, ref = run_both(ctx, score, desc, stride, 2, 0.2, 128, 0.1)
+    compare(res, ref, dtype)
+
+
+def test_stride_clamp_and_nonmultiple_map(ctx):
+    # descriptor map smaller than H/s: positions clamp to the map (G13); r = 4 near the border
+    score = synth.score_maps(2, 80, 120, 5, 0.01, 200)
+    desc = synth.desc_maps(2, 9, 14, 64, 5, torch.float16, "cuda")
+    res, ref = run_both(ctx, score, desc, 8, 4, 0.005, 256, 0.1)
+    compare(res, ref, torch.float16)
+    u = (ref.kpts[..., 0] + 0.5) / 8 - 0.5
+    assert (u < 0).any() and (u > 13).any()                    # both clamps exercised
+
+
+@pytest.mark.parametrize("T", [0.03, 0.1, 1.0])
+def test_temperature(ctx, T):
+    score, desc = small_inputs(1, 64, 128, seed=3, nblobs=60, D=0, dtype=None, stride=1)
+    res, ref = run_both(ctx, score, None, 1, 2, 0.2, 64, T)
+    compare(res, ref)
+
+
+# ---- full-size configs c1-c4 ---------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["c1", "c2", "c3", "c4"])
+def test_config_full_size(name):
+    import paper_2607_01757_b200 as dkd
+    cfg = synth.CONFIGS[name]
+    c = dkd.DKD(cfg.B, cfg.H, cfg.W, cfg.top_k, cfg.D)
+    try:
+        score, desc = synth.make_inputs(cfg, device="cuda")
+        res, ref = run_both(c, score, desc, cfg.stride, cfg.r, cfg.thresh, cfg.top_k, cfg.T)
+        st = compare(res, ref, synth.torch_dtype(cfg.desc_dtype))
+        print(name, "counts", ref.count, st)
+        assert (ref.scores == 1.0).sum() > 10                   # exact-1.0 ties head every ranking (G1)
+        if name in ("c2", "c4"):
+            assert np.all(ref.count < cfg.top_k)                # K_b < k branch
+        else:
+            assert np.all(ref.count == cfg.top_k)
+    finally:
+        c.close()
+
+
+def test_config_c5_full_size_sampled():
+    """B=64 1080p in the launch configuration bench.py times.  Steps 1-3 are checked on EVERY image
+    (oracle without descriptors), step 4 on sampled images whose descriptor maps are copied back."""
+    import paper_2607_01757_b200 as dkd
+    cfg = synth.CONFIGS["c5"]
+    free, _ = torch.cuda.mem_get_info()
+    need = cfg.B * cfg.Hd * cfg.Wd * cfg.D * 2 + 4 * cfg.B * cfg.H * cfg.W * 4
+    if free < need + (4 << 30):
+        pytest.fail(f"c5 needs {need >> 30} GiB of device memory, {free >> 30} GiB free")
+    c = dkd.DKD(cfg.B, cfg.H, cfg.W, cfg.top_k, cfg.D)
+    try:
+        score = synth.score_maps(cfg.B, cfg.H, cfg.W, cfg.seed, cfg.base, cfg.nblobs)
+        desc = synth.desc_maps(cfg.B, cfg.Hd, cfg.Wd, cfg.D, cfg.seed, torch.float16, "cuda")
+        res = c.extract(score.cuda(), desc, cfg.stride, cfg.r, cfg.thresh, cfg.top_k, cfg.T)
+        torch.cuda.synchronize()
+        ref = oracle.extract(score.numpy(), None, 1, cfg.r, cfg.thresh, cfg.top_k, cfg.T)
+        res_nodesc = type(res)(res.kpts, res.scores, None, res.count, res.index, res.offsets)
+        st = compare(res_nodesc, ref)
+        assert np.all(ref.count == cfg.top_k)
+        for b in (0, 37, 63):
+            refb = oracle.extract(score[b:b + 1].numpy(), desc[b:b + 1].cpu().numpy(), 1, cfg.r, cfg.thresh,
+                                  cfg.top_k, cfg.T)
+            st = compare(res, refb, torch.float16, images=[b])
+        # properties that hold at any size, on all images
+        d = res.desc.float()
+        assert torch.all((d.norm(dim=-1) - 1).abs() < 2e-3)
+        # device-side generator == host evaluation on sampled elements
+        e = torch.randint(0, cfg.Hd * cfg.Wd * cfg.D, (100000,))
+        assert torch.equal(desc[11].view(-1)[e.cuda()].cpu(), synth.desc_elements(cfg.seed, 11, e, torch.float16))
+    finally:
+        c.close()
+
+
+# ---- degenerate and adversarial inputs -----------------------------------------------------------
+def test_no_candidates_and_tiny_images(ctx):
+    score = torch.full((2, 40, 140), 0.1)
+    desc = synth.desc_maps(2, 40, 140, 32, 1, torch.float16, "cuda")
+    res, ref = run_both(ctx, score, desc, 1, 2, 0.2, 16, 0.1)
+    compare(res, ref, torch.float16)
+    assert int(res.count.sum()) == 0 and float(res.kpts.abs().sum()) == 0 and int((res.index != -1).sum()) == 0
+    for H, W in [(4, 9), (5, 5), (1, 1), (9, 4)]:               # H or W < 2r+1 -> no interior (G18)
+        s = torch.ones((1, H, W))
+        res, ref = run_both(ctx, s, None, 1, 2, 0.2, 8, 0.1)
+        compare(res, ref)
+
+
+def test_threshold_is_strict_and_border_excluded(ctx):
+    s = torch.zeros((1, 40, 140))
+    s[0, 10, 20] = 0.5                   # == thresh -> dropped
+    s[0, 20, 30] = float(np.nextafter(np.float32(0.5), np.float32(1)))
+    s[0, 1, 50] = 0.9                    # inside the r-border -> dropped
+    s[0, 2, 60] = 0.9                    # first kept row
+    s[0, 37, 137] = 0.8                  # last kept row / column
+    s[0, 38, 100] = 0.9
+    res, ref = run_both(ctx, s, None, 1, 2, 0.5, 8, 0.1)
+    compare(res, ref)
+    assert int(res.count[0]) == 3
+
+
+def test_constant_map_worst_case_radix_select(ctx):
+    # every interior pixel is a candidate (n = 124*252 = 31248 > 8192): MSB radix select must walk
+    # into the index bits; result = the first top_k interior pixels in raster order
+    s = torch.full((2, 128, 256), 0.7)
+    s[1] = 0.3
+    for top_k in (1, 100, 8192):
+        res, ref = run_both(ctx, s, None, 1, 2, 0.2, top_k, 0.1)
+        compare(res, ref)
+        assert int(res.count[0]) == top_k
+        assert int(res.index[0, 0]) == 2 * 256 + 2
+
+
+def test_many_candidates_mixed_scores_radix_select(ctx):
+    # > 8192 candidates with few distinct scores and a big tie class straddling the k-th place
+    g = torch.Generator().manual_seed(5)
+    s = (torch.randint(0, 4, (1, 300, 400), generator=g).float() / 4.0)
+    s = torch.nn.functional.max_pool2d(s[None], 3, 1, 1)[0]     # plateaus -> lots of tied maxima
+    for top_k in (500, 4096, 8192):
+        res, ref = run_both(ctx, s, None, 1, 1, 0.2, top_k, 0.1)
+        compare(res, ref)
+    n = int(oracle.nms_mask(s[0].numpy(), 1, 0.2).sum())
+    assert n > 8192
+
+
+def test_ties_at_clamp_value_adjacent(ctx):
+    s = synth.score_maps(1, 96, 200, 8, 0.1, 900)               # dense blobs -> many exact 1.0, some adjacent
+    res, ref = run_both(ctx, s, None, 1, 2, 0.2, 512, 0.1)
+    compare(res, ref)
+    assert (ref.scores == 1.0).sum() > 20
+
+
+def test_negative_threshold_and_signed_zero(ctx):
+    s = torch.zeros((1, 40, 140))
+    s[0, 10, 10] = -0.0
+    s[0, 20, 20] = -0.25
+    s[0, 30, 30] = 0.25
+    res, ref = run_both(ctx, s - 0.0, None, 1, 2, -0.5, 4096, 0.1)
+    compare(res, ref)
+
+
+# ---- API surface -----------------------------------------------------------------------------------
+def test_loader_graph_and_literal_variants_agree(ctx):
+    from paper_2607_01757_b200.binding import OPT_USE_GRAPH, OPT_USE_TMA
+    score, desc = small_inputs(2, 100, 260, seed=21, nblobs=200, D=128, dtype=torch.float16, stride=1)
+    sd = score.cuda()
+    base = ctx.extract(sd, desc, 1, 2, 0.2, 256, 0.1)
+    torch.cuda.synchronize()
+    try:
+        for graph in (0, 1):
+            for tma in (0, 1):
+                ctx.set_option(OPT_USE_GRAPH, graph)
+                ctx.set_option(OPT_USE_TMA, tma)
+                for rep in range(2):                              # second call replays the cached graph
+                    r2 = ctx.extract(sd, desc, 1, 2, 0.2, 256, 0.1)
+                    torch.cuda.synchronize()
+                    for n in ("kpts", "scores", "desc", "count", "index", "offsets"):
+                        assert torch.equal(getattr(base, n), getattr(r2, n)), (graph, tma, n)
+    finally:
+        ctx.set_option(OPT_USE_GRAPH, 1)
+        ctx.set_option(OPT_USE_TMA, 1)
+    lit = ctx.alloc_outputs(2, 256, desc, 128, want_index=False, want_offsets=False)
+    ctx.extract_literal(sd, desc, 1, 2, 0.2, 256, 0.1, lit)
+    torch.cuda.synchronize()
+    for n in ("kpts", "scores", "desc", "count"):
+        assert torch.equal(getattr(base, n), getattr(lit, n)), n
+
+
+def test_batch_equals_single_images_and_keypoints_only(ctx):
+    score, desc = small_inputs(3, 90, 200, seed=2, nblobs=100, D=64, dtype=torch.float32, stride=1)
+    sd = score.cuda()
+    full = ctx.extract(sd, desc, 1, 2, 0.2, 64, 0.1)
+    nod = ctx.extract(sd, None, 1, 2, 0.2, 64, 0.1)             # LK pathway
+    torch.cuda.synchronize()
+    assert nod.desc is None and torch.equal(nod.kpts, full.kpts) and torch.equal(nod.index, full.index)
+    for b in range(3):
+        one = ctx.extract(sd[b:b + 1].contiguous(), desc[b:b + 1].contiguous(), 1, 2, 0.2, 64, 0.1)
+        torch.cuda.synchronize()
+        for n in ("kpts", "scores", "desc", "count", "index", "offsets"):
+            assert torch.equal(getattr(full, n)[b], getattr(one, n)[0]), n
+
+
+def test_host_path_matches_device_path(ctx):
+    score, desc = small_inputs(2, 90, 200, seed=4, nblobs=100, D=128, dtype=torch.float16, stride=1)
+    dev = ctx.extract(score.cuda(), desc, 1, 2, 0.2, 128, 0.1)
+    torch.cuda.synchronize()
+    sp, dp = score.pin_memory(), desc.cpu().pin_memory()
+    for resident in (False, True, True):
+        host = ctx.extract_host(sp, dp, 1, 2, 0.2, 128, 0.1, desc_resident=resident)
+        for n in ("kpts", "scores", "desc", "count", "index", "offsets"):
+            assert not getattr(host, n).is_cuda
+            assert torch.equal(getattr(dev, n).cpu(), getattr(host, n)), n
+
+
+def test_capture_safe_inside_a_user_graph(ctx):
+    score, desc = small_inputs(2, 64, 256, seed=6, nblobs=80, D=64, dtype=torch.float16, stride=1)
+    sd = score.cuda()
+    want = ctx.extract(sd, desc, 1, 2, 0.2, 64, 0.1)
+    out = ctx.alloc_outputs(2, 64, desc, 64)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):                                     # the caller captures: no sync / alloc inside
+        ctx.extract(sd, desc, 1, 2, 0.2, 64, 0.1, out=out)
+    for t in (out.kpts, out.scores, out.desc, out.count, out.index, out.offsets):
+        t.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    for n in ("kpts", "scores", "desc", "count", "index", "offsets"):
+        assert torch.equal(getattr(want, n), getattr(out, n)), n
+
+
+def test_deterministic_across_runs(ctx):
+    score, desc = small_inputs(2, 150, 400, seed=12, nblobs=500, D=64, dtype=torch.float16, stride=1)
+    sd = score.cuda()
+    a = ctx.extract(sd, desc, 1, 2, 0.2, 512, 0.1)
+    torch.cuda.synchronize()
+    for _ in range(5):
+        b = ctx.extract(sd, desc, 1, 2, 0.2, 512, 0.1)
+        torch.cuda.synchronize()
+        for n in ("kpts", "scores", "desc", "count", "index", "offsets"):
+            assert torch.equal(getattr(a, n), getattr(b, n)), n
+
+
+def test_error_codes(ctx):
+    import paper_2607_01757_b200 as dkd
+    s = torch.zeros((1, 32, 128), device="cuda")
+    d = torch.zeros((1, 32, 128, 64), device="cuda", dtype=torch.float16)
+    def code(fn):
+        with pytest.raises(dkd.DKDError) as e:
+            fn()
+        return e.value.code
+    assert code(lambda: ctx.extract(s, None, 1, 0, 0.2, 8, 0.1)) == -1          # r < 1
+    assert code(lambda: ctx.extract(s, None, 1, 2, 0.2, 8, 0.0)) == -1          # T <= 0
+    assert code(lambda: ctx.extract(s, None, 1, 2, 0.2, 8, float("inf"))) == -1
+    assert code(lambda: ctx.extract(s, None, 1, 2, 0.2, 0, 0.1)) == -1          # top_k < 1
+    assert code(lambda: ctx.extract(s, None, 1, 5, 0.2, 8, 0.1)) == -2          # r > DKD_MAX_RADIUS
+    assert code(lambda: ctx.extract(s, d[..., :4].contiguous(), 1, 2, 0.2, 8, 0.1)) == -2   # 8-byte rows
+    assert code(lambda: ctx.extract(s, None, 1, 2, 0.2, 9000, 0.1)) == -3       # top_k > max
+    big = torch.zeros((5, 32, 128), device="cuda")
+    assert code(lambda: ctx.extract(big, None, 1, 2, 0.2, 8, 0.1)) == -3        # B > max_batch
+    assert code(lambda: dkd.DKD(1, 8, 8, 9000)) == -2                           # max_top_k > DKD_MAX_TOP_K
+    assert ctx.workspace_bytes > 0 and ctx.launches_per_extract() == 3
