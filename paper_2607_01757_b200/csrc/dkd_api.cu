@@ -67,6 +67,7 @@ struct dkd_ctx {
     // options
     int use_graph, use_tma;
     std::vector<GraphEntry> graphs;
+    cudaStream_t cap_stream;  // capture-only stream for building the cached graphs
     unsigned long long tick;
     char err[512];
 };
@@ -217,9 +218,11 @@ int run(dkd_ctx* ctx, ExtractArgs a, cudaStream_t st) {
         }
     // first call with these arguments: capture the launches once, then replay as one graph launch
     cudaGraph_t graph = nullptr;
-    CK(ctx, cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
-    cudaError_t e = enqueue(ctx, a, st);
-    cudaError_t e2 = cudaStreamEndCapture(st, &graph);
+    // (captured on a context-owned stream: the caller's may be the legacy default stream, which
+    // cannot be captured; the instantiated graph is then launched on the caller's stream)
+    CK(ctx, cudaStreamBeginCapture(ctx->cap_stream, cudaStreamCaptureModeThreadLocal));
+    cudaError_t e = enqueue(ctx, a, ctx->cap_stream);
+    cudaError_t e2 = cudaStreamEndCapture(ctx->cap_stream, &graph);
     if (e != cudaSuccess || e2 != cudaSuccess) {
         if (graph) cudaGraphDestroy(graph);
         return fail_cuda(ctx, "graph capture", e != cudaSuccess ? e : e2);
@@ -308,6 +311,7 @@ int dkd_create(const dkd_create_params* p, dkd_ctx** out) {
     const size_t b_cand = align256(ctx->max_tiles * TILE_PX * sizeof(uint64_t));
     const size_t b_cnt = align256(ctx->max_tiles * sizeof(int));
     const size_t b_sel = align256(static_cast<size_t>(p->max_batch) * p->max_top_k * sizeof(int32_t));
+    CKC(cudaStreamCreateWithFlags(&ctx->cap_stream, cudaStreamNonBlocking));
     CKC(cudaMalloc(&ctx->cand, b_cand));
     CKC(cudaMalloc(&ctx->tile_cnt, b_cnt));
     CKC(cudaMalloc(&ctx->sel_idx, b_sel));
@@ -320,6 +324,7 @@ int dkd_create(const dkd_create_params* p, dkd_ctx** out) {
 int dkd_destroy(dkd_ctx* ctx) {
     if (!ctx) return DKD_OK;
     for (auto& g : ctx->graphs) cudaGraphExecDestroy(g.exec);
+    if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
     if (ctx->cand) cudaFree(ctx->cand);
     if (ctx->tile_cnt) cudaFree(ctx->tile_cnt);
     if (ctx->sel_idx) cudaFree(ctx->sel_idx);
