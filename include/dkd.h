@@ -51,8 +51,10 @@ enum {
     DKD_OPT_USE_GRAPH = 0,   /* [1] run each dkd_extract as ONE cached CUDA-graph launch (north_star:
                                 "the whole stereo pair in one CUDA-graph launch"); 0 = plain launches.
                                 Ignored (plain launches) while `stream` is being captured by the caller. */
-    DKD_OPT_USE_TMA   = 1    /* [1] NMS tiles staged by TMA (cp.async.bulk.tensor) when W % 4 == 0 and
+    DKD_OPT_USE_TMA   = 1,   /* [1] NMS tiles staged by TMA (cp.async.bulk.tensor) when W % 4 == 0 and
                                 score is 16-byte aligned; 0 = always the plain-load tile loader. */
+    DKD_OPT_PROFILE   = 2    /* [0] 1 = measurement mode: plain launches (no graph) with a CUDA event recorded
+                                on `stream` before and after every kernel; read with dkd_profile_read. */
 };
 
 typedef struct {
@@ -143,6 +145,14 @@ int dkd_extract_host(dkd_ctx* ctx,
                      float* out_kpts, float* out_scores, void* out_desc, int32_t* out_count,
                      int32_t* out_index, float* out_offset,
                      int desc_resident, void* stream);
+
+/* Measurement mode (DKD_OPT_PROFILE = 1): waits for the events of the most recent dkd_extract* call
+ * on this context and writes the device time of each of its kernels, in launch order, to
+ * ms[0..n) (host; milliseconds; entries past the launch count are left untouched).  Returns the
+ * number of kernels that call launched, or a negative error (no profiled call yet, CUDA failure).
+ * dkd_kernel_name(i) is the name of the i-th kernel of a launch ("nms", "select", "refine_gather"). */
+int dkd_profile_read(dkd_ctx* ctx, float* ms, int n);
+const char* dkd_kernel_name(int i);
 
 /* Number of kernels one dkd_extract launches for these arguments (for launch accounting). */
 int dkd_launches_per_extract(const dkd_ctx* ctx, int with_desc);

@@ -10,12 +10,13 @@ import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 F32, F16 = 0, 1
-OPT_USE_GRAPH, OPT_USE_TMA = 0, 1
+OPT_USE_GRAPH, OPT_USE_TMA, OPT_PROFILE = 0, 1, 2
 MAX_RADIUS, MAX_TOP_K, MAX_ROW_BYTES = 4, 8192, 2048
 
 EXPORTED_SYMBOLS = (
     "dkd_create", "dkd_destroy", "dkd_last_error", "dkd_workspace_bytes", "dkd_set_option",
     "dkd_extract", "dkd_extract_ex", "dkd_extract_host", "dkd_launches_per_extract", "dkd_version",
+    "dkd_profile_read", "dkd_kernel_name",
 )
 
 
@@ -61,6 +62,10 @@ def load_library():
     L.dkd_launches_per_extract.restype = i
     L.dkd_launches_per_extract.argtypes = [vp, i]
     L.dkd_version.restype = ctypes.c_char_p
+    L.dkd_profile_read.restype = i
+    L.dkd_profile_read.argtypes = [vp, ctypes.POINTER(ctypes.c_float), i]
+    L.dkd_kernel_name.restype = ctypes.c_char_p
+    L.dkd_kernel_name.argtypes = [i]
     common = [vp, vp, i, i, i, vp, i, i, i, i, i, i, f, i, f, vp, vp, vp, vp]
     L.dkd_extract.restype = i
     L.dkd_extract.argtypes = common + [vp]
@@ -138,6 +143,14 @@ class DKD:
     def launches_per_extract(self, with_desc: bool = True) -> int:
         return int(self._L.dkd_launches_per_extract(self._h, int(with_desc)))
 
+    def profile_read(self) -> dict:
+        """dkd_profile_read: {kernel name: ms} of the last call made with OPT_PROFILE set (waits for it)."""
+        buf = (ctypes.c_float * 8)()
+        n = self._L.dkd_profile_read(self._h, buf, 8)
+        if n < 0:
+            self._check(n)
+        return {self._L.dkd_kernel_name(j).decode(): float(buf[j]) for j in range(n)}
+
     # -- device buffers ---------------------------------------------------------------------
     def alloc_outputs(self, B: int, top_k: int, desc: Optional[torch.Tensor], D: int = 0,
                       want_index=True, want_offsets=True, device=None, pin=False) -> DKDResult:
@@ -174,6 +187,28 @@ class DKD:
                                     _ptr(out.index), _ptr(out.offsets), ctypes.c_void_p(st.cuda_stream))
         self._check(rc)
         return out
+
+    def bind(self, score, desc, stride, r, thresh, top_k, T, out: DKDResult, stream=None):
+        """Pre-marshals one dkd_extract_ex call (fixed buffers) and returns a zero-argument callable that
+        enqueues it — keeps Python's per-call marshalling out of a timed launch loop."""
+        B, H, W = score.shape
+        Hd = Wd = D = 0
+        if desc is not None:
+            _, Hd, Wd, D = desc.shape
+        st = torch.cuda.current_stream(self.device) if stream is None else stream
+        ci, cf = ctypes.c_int, ctypes.c_float
+        args = (self._h, _ptr(score), ci(B), ci(H), ci(W), _ptr(desc), ci(_dt(desc)), ci(Hd), ci(Wd), ci(D),
+                ci(int(stride)), ci(int(r)), cf(float(thresh)), ci(int(top_k)), cf(float(T)),
+                _ptr(out.kpts), _ptr(out.scores), _ptr(out.desc), _ptr(out.count),
+                _ptr(out.index), _ptr(out.offsets), ctypes.c_void_p(st.cuda_stream))
+        fn, check = self._L.dkd_extract_ex, self._check
+        keep = (score, desc, out)                                 # the call holds raw pointers
+
+        def call(_keep=keep):
+            rc = fn(*args)
+            if rc:
+                check(rc)
+        return call
 
     def extract_literal(self, score, desc, stride, r, thresh, top_k, T, out: DKDResult, stream=None):
         """dkd_extract (the literal north_star signature: no index / offset outputs)."""

@@ -45,6 +45,8 @@ struct GraphEntry {
 };
 
 constexpr size_t GRAPH_CACHE_CAP = 256;
+constexpr int MAX_KERNELS = 3;                              // kernels per extract, in launch order:
+const char* const KERNEL_NAMES[MAX_KERNELS] = {"nms", "select", "refine_gather"};
 
 }  // namespace
 
@@ -65,7 +67,9 @@ struct dkd_ctx {
     void* st_out;   size_t st_out_bytes;
     const void* st_desc_src; size_t st_desc_src_bytes;      // what st_desc currently holds
     // options
-    int use_graph, use_tma;
+    int use_graph, use_tma, profile;
+    cudaEvent_t prof_ev[MAX_KERNELS + 1];                   // measurement mode: event before/after every kernel
+    int prof_n;                                             // kernels of the last profiled call (0: none)
     std::vector<GraphEntry> graphs;
     cudaStream_t cap_stream;  // capture-only stream for building the cached graphs
     unsigned long long tick;
@@ -140,10 +144,14 @@ cudaError_t launch_rg(const ExtractArgs& a, const int32_t* sel, cudaStream_t st)
 }
 
 // Enqueue the three kernels of one extract on `st`.  No sync, no allocation: capture-safe.
-cudaError_t enqueue(dkd_ctx* ctx, const ExtractArgs& a, cudaStream_t st) {
+// prof: measurement mode, an event on `st` before and after every kernel.
+cudaError_t enqueue(dkd_ctx* ctx, const ExtractArgs& a, cudaStream_t st, bool prof = false) {
     const int tiles_x = (a.W + TW - 1) / TW, tiles_y = (a.H + TH - 1) / TH;
     const int tpi = tiles_x * tiles_y, total = tpi * a.B;
     cudaError_t e;
+    int nk = 0;
+    auto mark = [&]() { return prof ? cudaEventRecord(ctx->prof_ev[nk++], st) : cudaSuccess; };
+    if ((e = mark()) != cudaSuccess) return e;
     switch (a.r) {
         case 1: e = launch_nms<1>(ctx, a, tiles_x, tiles_y, total, st); break;
         case 2: e = launch_nms<2>(ctx, a, tiles_x, tiles_y, total, st); break;
@@ -151,17 +159,23 @@ cudaError_t enqueue(dkd_ctx* ctx, const ExtractArgs& a, cudaStream_t st) {
         default: e = launch_nms<4>(ctx, a, tiles_x, tiles_y, total, st); break;
     }
     if (e != cudaSuccess) return e;
+    if ((e = mark()) != cudaSuccess) return e;
     int32_t* sel = a.out_index ? a.out_index : ctx->sel_idx;
     k_select<<<a.B, SEL_THREADS, SORT_CAP * sizeof(uint64_t), st>>>(ctx->cand, ctx->tile_cnt, tpi, a.top_k, sel,
                                                                     a.out_count);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
+    if ((e = mark()) != cudaSuccess) return e;
     switch (a.r) {
-        case 1: return launch_rg<1>(a, sel, st);
-        case 2: return launch_rg<2>(a, sel, st);
-        case 3: return launch_rg<3>(a, sel, st);
-        default: return launch_rg<4>(a, sel, st);
+        case 1: e = launch_rg<1>(a, sel, st); break;
+        case 2: e = launch_rg<2>(a, sel, st); break;
+        case 3: e = launch_rg<3>(a, sel, st); break;
+        default: e = launch_rg<4>(a, sel, st); break;
     }
+    if (e != cudaSuccess) return e;
+    if ((e = mark()) != cudaSuccess) return e;
+    if (prof) ctx->prof_n = nk - 1;
+    return cudaSuccess;
 }
 
 int validate(dkd_ctx* ctx, const ExtractArgs& a) {
@@ -205,6 +219,11 @@ int run(dkd_ctx* ctx, ExtractArgs a, cudaStream_t st) {
 
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     CK(ctx, cudaStreamIsCapturing(st, &cap));
+    if (ctx->profile && cap == cudaStreamCaptureStatusNone) {
+        ctx->prof_n = 0;
+        CK(ctx, enqueue(ctx, a, st, true));
+        return DKD_OK;
+    }
     if (!ctx->use_graph || cap != cudaStreamCaptureStatusNone) {
         CK(ctx, enqueue(ctx, a, st));
         return DKD_OK;
@@ -312,6 +331,7 @@ int dkd_create(const dkd_create_params* p, dkd_ctx** out) {
     const size_t b_cnt = align256(ctx->max_tiles * sizeof(int));
     const size_t b_sel = align256(static_cast<size_t>(p->max_batch) * p->max_top_k * sizeof(int32_t));
     CKC(cudaStreamCreateWithFlags(&ctx->cap_stream, cudaStreamNonBlocking));
+    for (int i = 0; i <= MAX_KERNELS; ++i) CKC(cudaEventCreate(&ctx->prof_ev[i]));
     CKC(cudaMalloc(&ctx->cand, b_cand));
     CKC(cudaMalloc(&ctx->tile_cnt, b_cnt));
     CKC(cudaMalloc(&ctx->sel_idx, b_sel));
@@ -325,6 +345,8 @@ int dkd_destroy(dkd_ctx* ctx) {
     if (!ctx) return DKD_OK;
     for (auto& g : ctx->graphs) cudaGraphExecDestroy(g.exec);
     if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
+    for (int i = 0; i <= MAX_KERNELS; ++i)
+        if (ctx->prof_ev[i]) cudaEventDestroy(ctx->prof_ev[i]);
     if (ctx->cand) cudaFree(ctx->cand);
     if (ctx->tile_cnt) cudaFree(ctx->tile_cnt);
     if (ctx->sel_idx) cudaFree(ctx->sel_idx);
@@ -346,6 +368,7 @@ int dkd_set_option(dkd_ctx* ctx, int option, int value) {
     switch (option) {
         case DKD_OPT_USE_GRAPH: ctx->use_graph = value != 0; return DKD_OK;
         case DKD_OPT_USE_TMA: ctx->use_tma = value != 0; return DKD_OK;
+        case DKD_OPT_PROFILE: ctx->profile = value != 0; ctx->prof_n = 0; return DKD_OK;
         default: return fail(ctx, DKD_ERR_INVALID_ARG, "unknown option");
     }
 }
@@ -353,7 +376,17 @@ int dkd_set_option(dkd_ctx* ctx, int option, int value) {
 int dkd_launches_per_extract(const dkd_ctx* ctx, int with_desc) {
     (void)ctx;
     (void)with_desc;
-    return 3;                                               // k_nms_*, k_select, k_refine_gather
+    return MAX_KERNELS;                                     // k_nms_*, k_select, k_refine_gather
+}
+
+const char* dkd_kernel_name(int i) { return (i >= 0 && i < MAX_KERNELS) ? KERNEL_NAMES[i] : ""; }
+
+int dkd_profile_read(dkd_ctx* ctx, float* ms, int n) {
+    if (!ctx || !ms || n < 0) return DKD_ERR_INVALID_ARG;
+    if (ctx->prof_n <= 0) return fail(ctx, DKD_ERR_INVALID_ARG, "no profiled dkd_extract call (set DKD_OPT_PROFILE)");
+    CK(ctx, cudaEventSynchronize(ctx->prof_ev[ctx->prof_n]));
+    for (int i = 0; i < ctx->prof_n && i < n; ++i) CK(ctx, cudaEventElapsedTime(&ms[i], ctx->prof_ev[i], ctx->prof_ev[i + 1]));
+    return ctx->prof_n;
 }
 
 int dkd_extract_ex(dkd_ctx* ctx, const float* score, int B, int H, int W, const void* desc, int desc_dtype, int Hd,
