@@ -56,7 +56,7 @@ struct dkd_ctx {
     int nms_ctas_per_sm[MAX_R + 1];
     PFN_tensorMapEncodeTiled encode;
     // workspace (device)
-    uint64_t* cand;          // [max_tiles * TILE_PX] candidate keys, one private segment per tile
+    uint64_t* cand;          // [max_tiles * SEG_CAP] candidate keys, one private segment per tile
     int* tile_cnt;           // [max_tiles]
     int32_t* sel_idx;        // [max_batch * max_top_k]
     size_t max_tiles;
@@ -94,34 +94,36 @@ int fail_cuda(dkd_ctx* ctx, const char* what, cudaError_t e) {
 
 template <int R>
 cudaError_t setup_nms(dkd_ctx* ctx) {
-    cudaError_t e = cudaFuncSetAttribute(k_nms_tma<R>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         NMS_STAGES * stage_bytes(R));
+    cudaError_t e = cudaFuncSetAttribute(k_nms_tma<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, nms_smem_bytes(R));
     if (e != cudaSuccess) return e;
     int n = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_nms_tma<R>, NMS_THREADS, NMS_STAGES * stage_bytes(R));
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_nms_tma<R>, nms_warps(R) * 32, nms_smem_bytes(R));
     ctx->nms_ctas_per_sm[R] = n > 0 ? n : 1;
     return e;
 }
 
 template <int R>
-cudaError_t launch_nms(dkd_ctx* ctx, const ExtractArgs& a, int tiles_x, int tiles_y, int total, cudaStream_t st) {
+cudaError_t launch_nms(dkd_ctx* ctx, const ExtractArgs& a, int strips_x, int tiles_y, int total, cudaStream_t st) {
+    // S > thresh  <=>  S >= nextafter(thresh, +inf): the threshold joins the window maximum (dkd_kernels.cuh)
+    const float thr_up = nextafterf(a.thresh, INFINITY);
     if (a.use_tma) {
         CUtensorMap tmap;
         const cuuint64_t dims[3] = {(cuuint64_t)a.W, (cuuint64_t)a.H, (cuuint64_t)a.B};
         const cuuint64_t strides[2] = {(cuuint64_t)a.W * 4, (cuuint64_t)a.W * a.H * 4};
-        const cuuint32_t box[3] = {(cuuint32_t)PITCH, (cuuint32_t)tile_rows(R), 1};
+        const cuuint32_t box[3] = {(cuuint32_t)BOX_W, (cuuint32_t)box_rows(R), 1};
         const cuuint32_t estr[3] = {1, 1, 1};
         CUresult r = ctx->encode(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(a.score), dims, strides,
                                  box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                  CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+        constexpr int NW = nms_warps(R);
         int grid = ctx->num_sms * ctx->nms_ctas_per_sm[R];
-        if (grid > total) grid = total;
-        k_nms_tma<R><<<grid, NMS_THREADS, NMS_STAGES * stage_bytes(R), st>>>(tmap, a.H, a.W, tiles_x, tiles_y, total,
-                                                                             a.thresh, ctx->cand, ctx->tile_cnt);
+        if (grid > (total + NW - 1) / NW) grid = (total + NW - 1) / NW;
+        k_nms_tma<R><<<grid, NW * 32, nms_smem_bytes(R), st>>>(tmap, a.H, a.W, strips_x, tiles_y, total, thr_up,
+                                                                ctx->cand, ctx->tile_cnt);
     } else {
-        k_nms_plain<R><<<total, NMS_THREADS, 0, st>>>(a.score, a.H, a.W, tiles_x, tiles_y, a.thresh, ctx->cand,
-                                                      ctx->tile_cnt);
+        k_nms_plain<R><<<(total + PLAIN_WARPS - 1) / PLAIN_WARPS, PLAIN_WARPS * 32, 0, st>>>(
+            a.score, a.H, a.W, strips_x, tiles_y, total, thr_up, ctx->cand, ctx->tile_cnt);
     }
     return cudaGetLastError();
 }
@@ -146,7 +148,7 @@ cudaError_t launch_rg(const ExtractArgs& a, const int32_t* sel, cudaStream_t st)
 // Enqueue the three kernels of one extract on `st`.  No sync, no allocation: capture-safe.
 // prof: measurement mode, an event on `st` before and after every kernel.
 cudaError_t enqueue(dkd_ctx* ctx, const ExtractArgs& a, cudaStream_t st, bool prof = false) {
-    const int tiles_x = (a.W + TW - 1) / TW, tiles_y = (a.H + TH - 1) / TH;
+    const int tiles_x = (a.W + STRIP_W - 1) / STRIP_W, tiles_y = (a.H + TH - 1) / TH;
     const int tpi = tiles_x * tiles_y, total = tpi * a.B;
     cudaError_t e;
     int nk = 0;
@@ -325,9 +327,9 @@ int dkd_create(const dkd_create_params* p, dkd_ctx** out) {
     CKC(setup_nms<3>(ctx));
     CKC(setup_nms<4>(ctx));
     CKC(cudaFuncSetAttribute(k_select, cudaFuncAttributeMaxDynamicSharedMemorySize, SORT_CAP * sizeof(uint64_t)));
-    const size_t tx = (p->max_w + TW - 1) / TW, ty = (p->max_h + TH - 1) / TH;
+    const size_t tx = (p->max_w + STRIP_W - 1) / STRIP_W, ty = (p->max_h + TH - 1) / TH;
     ctx->max_tiles = tx * ty * p->max_batch;
-    const size_t b_cand = align256(ctx->max_tiles * TILE_PX * sizeof(uint64_t));
+    const size_t b_cand = align256(ctx->max_tiles * SEG_CAP * sizeof(uint64_t));
     const size_t b_cnt = align256(ctx->max_tiles * sizeof(int));
     const size_t b_sel = align256(static_cast<size_t>(p->max_batch) * p->max_top_k * sizeof(int32_t));
     CKC(cudaStreamCreateWithFlags(&ctx->cap_stream, cudaStreamNonBlocking));

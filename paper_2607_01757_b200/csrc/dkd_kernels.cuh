@@ -20,22 +20,26 @@
 namespace dkd {
 
 // ---- geometry -------------------------------------------------------------------------------
-constexpr int TW = 128;                  // tile width  (pixels)
-constexpr int TH = 32;                   // tile height (pixels)
-constexpr int HX = 4;                    // x halo kept in smem: >= max radius, multiple of 4 so the
-                                         // tile interior stays float4-aligned
-constexpr int PITCH = TW + 2 * HX;       // 136 floats = 544 B per smem row (= TMA box width)
-constexpr int TILE_PX = TW * TH;         // 4096 = worst-case candidates of a tile = segment capacity
+// Unit of NMS work = one STRIP-TILE: STRIP_W x TH output pixels, owned by ONE warp.  Its halo'd
+// input box is BOX_W x (TH + 2R) floats: 4 halo columns each side (>= max radius, keeps every lane's
+// float4 16-byte aligned) and R halo rows above and below.  Lane l owns box columns 4l..4l+3; lanes
+// 0 and 31 hold only halo columns, lanes 1..30 produce the 120 output columns.
+constexpr int STRIP_W = 120;             // output columns per strip
+constexpr int BOX_W = 128;               // box columns = one 512-byte shared-memory row (32 lanes x float4)
+constexpr int HALO_X = 4;
+constexpr int TH = 16;                   // output rows per strip-tile
+constexpr int SEG_CAP = STRIP_W * TH;    // 1920 = worst-case candidates of a strip-tile = segment capacity
 constexpr int MAX_R = 4;
-constexpr int NMS_THREADS = 256;
-constexpr int NMS_STAGES = 4;            // TMA pipeline depth per CTA
+constexpr int NMS_STAGES = 2;            // TMA boxes in flight / in use per warp
 constexpr int SEL_THREADS = 1024;
 constexpr int SORT_CAP = 8192;           // keys sorted in shared memory by k_select (64 KB)
 constexpr int RG_THREADS = 256;          // k_refine_gather: 8 warps, one warp per output slot
 
-__host__ __device__ constexpr int tile_rows(int R) { return TH + 2 * R; }
-__host__ __device__ constexpr int stage_bytes(int R) { return ((PITCH * tile_rows(R) * 4 + 127) / 128) * 128; }
-__host__ __device__ constexpr int box_bytes(int R) { return PITCH * tile_rows(R) * 4; }
+__host__ __device__ constexpr int box_rows(int R) { return TH + 2 * R; }
+__host__ __device__ constexpr int box_bytes(int R) { return BOX_W * box_rows(R) * 4; }     // multiple of 512
+// warps per CTA: 2 CTAs/SM must fit 227 KB of shared memory (R <= 3: 5 warps, 10 KB..11.3 KB boxes)
+__host__ __device__ constexpr int nms_warps(int R) { return R <= 3 ? 5 : 4; }
+__host__ __device__ constexpr int nms_smem_bytes(int R) { return nms_warps(R) * NMS_STAGES * box_bytes(R); }
 
 // ---- 64-bit selection key ---------------------------------------------------------------------
 // key = (orderable(score bits) << 32) | ~idx : a larger key is a better candidate, i.e. descending
@@ -88,142 +92,218 @@ __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* tmap) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(tmap)) : "memory");
 }
 
-// ---- step a1 + a1': one halo'd tile in shared memory -> candidate keys ------------------------------
-// tile: smem, tile_rows(R) x PITCH floats; tile[(row + R) * PITCH + HX + col] is pixel (x0+col, y0+row).
-// Pixels outside the image read 0 (never used: a kept pixel's window is inside the image, G3).
-// Candidates are appended (unordered) to this tile's private global segment `seg` (capacity TILE_PX);
-// the slot comes from a shared-memory counter, one atomic per warp-row (warp-ballot compaction).
-template <int R>
-__device__ __forceinline__ void process_tile(const float* __restrict__ tile, int x0, int y0, int H, int W,
-                                             float thresh, int* s_cnt, uint64_t* __restrict__ seg) {
-    const int lane = threadIdx.x & 31;
-    const int warp = threadIdx.x >> 5;
-    constexpr int ROWS_PER_WARP = TH / (NMS_THREADS / 32);
-    const int gx = x0 + 4 * lane;
-#pragma unroll
-    for (int rr = 0; rr < ROWS_PER_WARP; ++rr) {
-        const int row = warp * ROWS_PER_WARP + rr;
-        const int gy = y0 + row;
-        const float* ctr = tile + (row + R) * PITCH + HX + 4 * lane;
-        const float4 v4 = *reinterpret_cast<const float4*>(ctr);
-        const float v[4] = {v4.x, v4.y, v4.z, v4.w};
-        unsigned m = 0;
-        if (gy >= R && gy < H - R) {                         // warp-uniform
-#pragma unroll
-            for (int c = 0; c < 4; ++c)
-                if (v[c] > thresh && gx + c >= R && gx + c < W - R) m |= 1u << c;
-        }
-        if (m) {                                             // rare (a few % of pixels pass the threshold)
-#pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                if (m & (1u << c)) {
-                    const float* wp = ctr + c - R * PITCH - R;
-                    bool ismax = true;
-#pragma unroll
-                    for (int j = 0; j <= 2 * R; ++j)
-#pragma unroll
-                        for (int i = 0; i <= 2 * R; ++i) ismax &= !(wp[j * PITCH + i] > v[c]);   // ties keep (G1)
-                    if (!ismax) m &= ~(1u << c);
-                }
-            }
-        }
-        if (__any_sync(0xffffffffu, m != 0)) {
-            unsigned bal[4];
-            int tot = 0, mypos[4];
-#pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                bal[c] = __ballot_sync(0xffffffffu, (m >> c) & 1u);
-                mypos[c] = tot + __popc(bal[c] & ((1u << lane) - 1u));
-                tot += __popc(bal[c]);
-            }
-            int base = 0;
-            if (lane == 0) base = atomicAdd(s_cnt, tot);
-            base = __shfl_sync(0xffffffffu, base, 0);
-#pragma unroll
-            for (int c = 0; c < 4; ++c)
-                if ((m >> c) & 1u) seg[base + mypos[c]] = make_key(v[c], gy * W + gx + c);
-        }
-    }
+// 3-input max: one FMNMX3 on sm_100a (alu pipe), halves the op count of the window maxima
+__device__ __forceinline__ float fmax3(float a, float b, float c) {
+    float d;
+    asm("max.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
+    return d;
 }
 
-// ---- k_nms_tma: persistent, TMA-staged halo tiles, NMS_STAGES-deep mbarrier pipeline ----------------
-// grid = min(total_tiles, CTAs that fit); CTA c handles tiles c, c+grid, ... (image-major order).
-// Dynamic smem: NMS_STAGES * stage_bytes(R), 128-byte aligned.
+// ---- step a1 + a1': one halo'd strip-tile in shared memory -> candidate keys -------------------------
+// box: smem, box_rows(R) x BOX_W floats; box[q * BOX_W + j] is pixel (x0 - HALO_X + j, y0 - R + q).
+// Pixels outside the image read 0 (never used: a kept pixel's window is inside the image, G3).
+//
+// Separable window maximum, the same ~8 instructions per pixel on any input (no data-dependent
+// divergence): every lane walks down its 4 columns keeping the last 2R+1 rows in registers
+// (vertical max, 2 FMNMX3 per column for r = 2), takes the neighbouring lanes' column maxima by
+// shuffle (2R SHFL per row) and forms the horizontal max with the threshold folded in:
+//     m_k = max( max over the (2r+1)^2 window of pixel k ,  thr_up ),  thr_up = nextafter(thresh, +inf)
+// so that   S > thresh  AND  S >= every window value   <=>   S == m_k   <=>   S - m_k >= 0
+// (S <= m_k always; the subtraction of two different finite floats is never 0; -0/+0 compare equal).
+// The per-pixel test therefore costs 4 FADD + 2 FMNMX + 1 FSETP per lane-row; the exact mask, the
+// ballot compaction and the key stores run only in the rare warp-rows that hold a candidate.
+// Candidates are appended (unordered) to the strip-tile's private global segment `seg`
+// (capacity SEG_CAP); the running count lives in a warp-uniform register (no atomics).
 template <int R>
-__global__ void __launch_bounds__(NMS_THREADS) k_nms_tma(const __grid_constant__ CUtensorMap tmap, int H, int W,
-                                                         int tiles_x, int tiles_y, int total_tiles, float thresh,
-                                                         uint64_t* __restrict__ cand, int* __restrict__ tile_cnt) {
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    __shared__ __align__(8) uint64_t full_bar[NMS_STAGES];
-    __shared__ int s_cnt[2];
-    constexpr int SB = stage_bytes(R);
-    const int tid = threadIdx.x;
-    const int tpi = tiles_x * tiles_y;
-    const int first = blockIdx.x, step = gridDim.x;
-    const int n_my = first < total_tiles ? (total_tiles - first + step - 1) / step : 0;
+__device__ __forceinline__ int process_strip(const float* __restrict__ box, int x0, int y0, int H, int W,
+                                             float thr_up, uint64_t* __restrict__ seg) {
+    constexpr int N = 2 * R + 1;
+    constexpr unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    const int X = x0 - HALO_X + 4 * lane;                    // image column of this lane's first pixel
+    unsigned colmask = 0;                                    // output columns this lane may emit
+    if (lane >= 1 && lane <= 30) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+            if (X + k >= R && X + k < W - R) colmask |= 1u << k;
+    }
+    const float4* src = reinterpret_cast<const float4*>(box) + lane;   // row pitch = 32 float4
+    float4 ring[N];
+#pragma unroll
+    for (int q = 0; q < 2 * R; ++q) ring[q] = src[q * 32];
+    int cnt = 0;
+#pragma unroll
+    for (int o = 0; o < TH; ++o) {
+        ring[(o + 2 * R) % N] = src[(o + 2 * R) * 32];
+        const int y = y0 + o;
+        if (y < R || y >= H - R) continue;                   // warp-uniform (first / last tile rows only)
+        // vertical max of the 2R+1 rows, per column
+        float4 vm = ring[0];
+#pragma unroll
+        for (int q = 1; q + 1 < N; q += 2) {
+            vm.x = fmax3(vm.x, ring[q].x, ring[q + 1].x);
+            vm.y = fmax3(vm.y, ring[q].y, ring[q + 1].y);
+            vm.z = fmax3(vm.z, ring[q].z, ring[q + 1].z);
+            vm.w = fmax3(vm.w, ring[q].w, ring[q + 1].w);
+        }
+        // neighbours' column maxima: l[j] = column X-1-j, rt[j] = column X+4+j
+        float l[R], rt[R];
+        {
+            const float lv[4] = {vm.w, vm.z, vm.y, vm.x};    // sender's columns nearest the receiver first
+            const float rv[4] = {vm.x, vm.y, vm.z, vm.w};
+#pragma unroll
+            for (int j = 0; j < R; ++j) {
+                l[j] = __shfl_up_sync(FULL, lv[j], 1);
+                rt[j] = __shfl_down_sync(FULL, rv[j], 1);
+            }
+        }
+        // horizontal max with the threshold folded in
+        float m0, m1, m2, m3;
+        if constexpr (R == 1) {
+            const float p = fmax3(vm.y, vm.z, thr_up);
+            m0 = fmax3(l[0], vm.x, fmaxf(vm.y, thr_up));
+            m1 = fmaxf(p, vm.x);
+            m2 = fmaxf(p, vm.w);
+            m3 = fmax3(vm.z, vm.w, fmaxf(rt[0], thr_up));
+        } else if constexpr (R == 2) {
+            const float p = fmax3(vm.y, vm.z, thr_up);       // {1,2,thr}
+            const float q0 = fmax3(p, vm.x, l[0]);           // {-1..2,thr}
+            const float q1 = fmax3(p, vm.w, rt[0]);          // {1..4,thr}
+            m0 = fmaxf(q0, l[1]);                            // {-2..2}
+            m1 = fmaxf(q0, vm.w);                            // {-1..3}
+            m2 = fmaxf(q1, vm.x);                            // {0..4}
+            m3 = fmaxf(q1, rt[1]);                           // {1..5}
+        } else {
+            // R >= 3: every window contains the lane's own 4 columns
+            const float core = fmax3(fmax3(vm.x, vm.y, vm.z), vm.w, thr_up);
+            float lp[R], rp[R];                              // lp[j] = max(l[0..j]), rp[j] = max(rt[0..j])
+            lp[0] = l[0];
+            rp[0] = rt[0];
+#pragma unroll
+            for (int j = 1; j < R; ++j) {
+                lp[j] = fmaxf(lp[j - 1], l[j]);
+                rp[j] = fmaxf(rp[j - 1], rt[j]);
+            }
+            // pixel k spans columns k-R .. k+R: left part l[0..R-k-1], right part rt[0..k+R-4]
+            m0 = fmaxf(core, lp[R - 1]);
+            m1 = fmax3(core, lp[R - 2], rp[R - 3]);
+            m2 = fmax3(core, lp[R - 3], rp[R - 2]);
+            m3 = fmaxf(core, rp[R - 1]);
+            if constexpr (R == 4) m0 = fmaxf(m0, rp[0]), m3 = fmaxf(m3, lp[0]);
+        }
+        const float4 c = ring[(o + R) % N];                  // centre row
+        const float d0 = c.x - m0, d1 = c.y - m1, d2 = c.z - m2, d3 = c.w - m3;
+        const float e = fmax3(fmaxf(d0, d1), d2, d3);
+        if (__any_sync(FULL, e >= 0.0f && colmask != 0u)) {  // rare: some lane holds a candidate
+            unsigned m = (d0 >= 0.0f ? 1u : 0u) | (d1 >= 0.0f ? 2u : 0u) | (d2 >= 0.0f ? 4u : 0u) |
+                         (d3 >= 0.0f ? 8u : 0u);
+            m &= colmask;
+            const float v[4] = {c.x, c.y, c.z, c.w};
+            int tot = 0, mypos[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const unsigned bal = __ballot_sync(FULL, (m >> k) & 1u);
+                mypos[k] = tot + __popc(bal & ((1u << lane) - 1u));
+                tot += __popc(bal);
+            }
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                if ((m >> k) & 1u) seg[cnt + mypos[k]] = make_key(v[k], y * W + X + k);
+            cnt += tot;
+        }
+    }
+    return cnt;
+}
 
-    auto issue = [&](int it) {
-        const int t = first + it * step;
-        const int b = t / tpi, rem = t - b * tpi;
-        const int ty = rem / tiles_x, tx = rem - ty * tiles_x;
+// strip-tile index -> (image, tile row, strip)
+__device__ __forceinline__ void tile_coords(int t, int strips_x, int tiles_y, int& b, int& y0, int& x0) {
+    const int spi = strips_x * tiles_y;
+    b = t / spi;
+    const int rem = t - b * spi;
+    const int ty = rem / strips_x;
+    x0 = (rem - ty * strips_x) * STRIP_W;
+    y0 = ty * TH;
+}
+
+// ---- k_nms_tma: persistent; every warp runs its own NMS_STAGES-deep TMA/mbarrier pipeline ------------
+// grid = min(ceil(total / warps), CTAs that fit); warp g handles strip-tiles g, g + G, ... (image-major,
+// row-major, strips fastest: neighbouring warps load neighbouring boxes, so halo re-reads hit L2).
+// No CTA-wide barrier after set-up: a warp only ever waits for its own box.
+// Dynamic smem: nms_smem_bytes(R), 128-byte aligned; box of (warp w, stage s) at (w*NMS_STAGES+s)*box_bytes.
+template <int R>
+__global__ void __launch_bounds__(nms_warps(R) * 32, 2) k_nms_tma(const __grid_constant__ CUtensorMap tmap, int H,
+                                                                  int W, int strips_x, int tiles_y, int total,
+                                                                  float thr_up, uint64_t* __restrict__ cand,
+                                                                  int* __restrict__ tile_cnt) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ __align__(8) uint64_t full_bar[nms_warps(R) * NMS_STAGES];
+    constexpr int NW = nms_warps(R);
+    constexpr int BB = box_bytes(R);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int first = blockIdx.x * NW + warp, step = gridDim.x * NW;
+    const int n_my = first < total ? (total - first + step - 1) / step : 0;
+    unsigned char* my_smem = smem_raw + warp * NMS_STAGES * BB;
+    uint64_t* my_bar = full_bar + warp * NMS_STAGES;
+
+    auto issue = [&](int it) {                               // lane 0 only
+        int b, y0, x0;
+        tile_coords(first + it * step, strips_x, tiles_y, b, y0, x0);
         const int s = it % NMS_STAGES;
-        mbar_arrive_expect_tx(&full_bar[s], box_bytes(R));
-        tma_load_tile(smem_raw + s * SB, &tmap, &full_bar[s], tx * TW - HX, ty * TH - R, b);
+        mbar_arrive_expect_tx(&my_bar[s], BB);
+        tma_load_tile(my_smem + s * BB, &tmap, &my_bar[s], x0 - HALO_X, y0 - R, b);
     };
 
-    if (tid == 0) {
-        tma_prefetch_desc(&tmap);
+    if (lane == 0) {
+        if (warp == 0) tma_prefetch_desc(&tmap);
 #pragma unroll
-        for (int s = 0; s < NMS_STAGES; ++s) mbar_init(&full_bar[s], 1);
-        s_cnt[0] = 0;
-        s_cnt[1] = 0;
+        for (int s = 0; s < NMS_STAGES; ++s) mbar_init(&my_bar[s], 1);
         fence_mbar_init();
-    }
-    __syncthreads();
-    if (tid == 0) {
         const int pre = n_my < NMS_STAGES ? n_my : NMS_STAGES;
         for (int it = 0; it < pre; ++it) issue(it);
     }
+    __syncwarp();
     for (int it = 0; it < n_my; ++it) {
         const int t = first + it * step;
-        const int b = t / tpi, rem = t - b * tpi;
-        const int ty = rem / tiles_x, tx = rem - ty * tiles_x;
+        int b, y0, x0;
+        tile_coords(t, strips_x, tiles_y, b, y0, x0);
         const int s = it % NMS_STAGES;
-        mbar_wait(&full_bar[s], (it / NMS_STAGES) & 1);
-        process_tile<R>(reinterpret_cast<const float*>(smem_raw + s * SB), tx * TW, ty * TH, H, W, thresh,
-                        &s_cnt[it & 1], cand + static_cast<size_t>(t) * TILE_PX);
-        __syncthreads();                                     // every warp is done with stage s and s_cnt[it&1]
-        if (tid == 0) {
-            tile_cnt[t] = s_cnt[it & 1];
-            s_cnt[it & 1] = 0;
+        mbar_wait(&my_bar[s], (it / NMS_STAGES) & 1);
+        const int cnt = process_strip<R>(reinterpret_cast<const float*>(my_smem + s * BB), x0, y0, H, W, thr_up,
+                                         cand + static_cast<size_t>(t) * SEG_CAP);
+        __syncwarp();                                        // every lane is done reading stage s
+        if (lane == 0) {
+            tile_cnt[t] = cnt;
             if (it + NMS_STAGES < n_my) issue(it + NMS_STAGES);
         }
     }
 }
 
-// ---- k_nms_plain: same tile math, tile staged with ordinary loads (any W, any alignment) ------------
+// ---- k_nms_plain: same strip math, box staged with ordinary loads (any W, any alignment) ------------
+constexpr int PLAIN_WARPS = 4;
 template <int R>
-__global__ void __launch_bounds__(NMS_THREADS) k_nms_plain(const float* __restrict__ score, int H, int W,
-                                                           int tiles_x, int tiles_y, float thresh,
-                                                           uint64_t* __restrict__ cand, int* __restrict__ tile_cnt) {
-    __shared__ __align__(16) float tile[PITCH * tile_rows(R)];
-    __shared__ int s_cnt;
-    const int t = blockIdx.x;
-    const int tpi = tiles_x * tiles_y;
-    const int b = t / tpi, rem = t - b * tpi;
-    const int ty = rem / tiles_x, tx = rem - ty * tiles_x;
-    const int x0 = tx * TW, y0 = ty * TH;
+__global__ void __launch_bounds__(PLAIN_WARPS * 32) k_nms_plain(const float* __restrict__ score, int H, int W,
+                                                                int strips_x, int tiles_y, int total, float thr_up,
+                                                                uint64_t* __restrict__ cand,
+                                                                int* __restrict__ tile_cnt) {
+    __shared__ __align__(16) float boxes[PLAIN_WARPS][BOX_W * box_rows(R)];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int t = blockIdx.x * PLAIN_WARPS + warp;
+    if (t >= total) return;
+    int b, y0, x0;
+    tile_coords(t, strips_x, tiles_y, b, y0, x0);
     const float* img = score + static_cast<size_t>(b) * H * W;
-    if (threadIdx.x == 0) s_cnt = 0;
-    for (int e = threadIdx.x; e < PITCH * tile_rows(R); e += NMS_THREADS) {
-        const int ry = e / PITCH, rx = e - ry * PITCH;
-        const int gy = y0 - R + ry, gx = x0 - HX + rx;
-        tile[e] = (gy >= 0 && gy < H && gx >= 0 && gx < W) ? __ldg(img + static_cast<size_t>(gy) * W + gx) : 0.0f;
+    float* box = boxes[warp];
+    for (int q = 0; q < box_rows(R); ++q) {
+        const int gy = y0 - R + q;
+#pragma unroll
+        for (int j = lane; j < BOX_W; j += 32) {
+            const int gx = x0 - HALO_X + j;
+            box[q * BOX_W + j] = (gy >= 0 && gy < H && gx >= 0 && gx < W) ? __ldg(img + static_cast<size_t>(gy) * W + gx) : 0.0f;
+        }
     }
-    __syncthreads();
-    process_tile<R>(tile, x0, y0, H, W, thresh, &s_cnt, cand + static_cast<size_t>(t) * TILE_PX);
-    __syncthreads();
-    if (threadIdx.x == 0) tile_cnt[t] = s_cnt;
+    __syncwarp();
+    const int cnt = process_strip<R>(box, x0, y0, H, W, thr_up, cand + static_cast<size_t>(t) * SEG_CAP);
+    if (lane == 0) tile_cnt[t] = cnt;
 }
 
 // ---- k_select: per-image top-k select + order ---------------------------------------------------
@@ -259,7 +339,7 @@ __global__ void __launch_bounds__(SEL_THREADS) k_select(const uint64_t* __restri
     constexpr int NW = SEL_THREADS / 32;
     const int b = blockIdx.x;
     const int* cnt = tile_cnt + static_cast<size_t>(b) * tpi;
-    const uint64_t* seg0 = cand + static_cast<size_t>(b) * tpi * TILE_PX;
+    const uint64_t* seg0 = cand + static_cast<size_t>(b) * tpi * SEG_CAP;
 
     int local = 0;
     for (int t = tid; t < tpi; t += SEL_THREADS) local += cnt[t];
@@ -275,7 +355,7 @@ __global__ void __launch_bounds__(SEL_THREADS) k_select(const uint64_t* __restri
             __syncthreads();
             for (int t = warp; t < tpi; t += NW) {
                 const int c = cnt[t];
-                const uint64_t* seg = seg0 + static_cast<size_t>(t) * TILE_PX;
+                const uint64_t* seg = seg0 + static_cast<size_t>(t) * SEG_CAP;
                 for (int e0 = 0; e0 < c; e0 += 32) {
                     const int e = e0 + lane;
                     int digit = 256;                        // dummy bin: past the end / outside the prefix
@@ -330,7 +410,7 @@ __global__ void __launch_bounds__(SEL_THREADS) k_select(const uint64_t* __restri
     for (int t = warp; t < tpi; t += NW) {
         const int c = cnt[t];
         if (c == 0) continue;
-        const uint64_t* seg = seg0 + static_cast<size_t>(t) * TILE_PX;
+        const uint64_t* seg = seg0 + static_cast<size_t>(t) * SEG_CAP;
         if (lo == 0) {
             int base = 0;
             if (lane == 0) base = atomicAdd(&s_n, c);
