@@ -131,12 +131,14 @@ __device__ __forceinline__ int process_strip(const float* __restrict__ box, int 
     float4 ring[N];
 #pragma unroll
     for (int q = 0; q < 2 * R; ++q) ring[q] = src[q * 32];
-    int cnt = 0;
+    // neg[h]: nibble o&7 of word o>>3 holds, for output row o, one bit per pixel k that is NOT a candidate
+    // (sign bit of S - m_k).  The 16-row body is branch-free, so the rows interleave freely.
+    unsigned neg[TH / 8];
+#pragma unroll
+    for (int h = 0; h < TH / 8; ++h) neg[h] = 0u;
 #pragma unroll
     for (int o = 0; o < TH; ++o) {
         ring[(o + 2 * R) % N] = src[(o + 2 * R) * 32];
-        const int y = y0 + o;
-        if (y < R || y >= H - R) continue;                   // warp-uniform (first / last tile rows only)
         // vertical max of the 2R+1 rows, per column
         float4 vm = ring[0];
 #pragma unroll
@@ -191,28 +193,49 @@ __device__ __forceinline__ int process_strip(const float* __restrict__ box, int 
             m3 = fmaxf(core, rp[R - 1]);
             if constexpr (R == 4) m0 = fmaxf(m0, rp[0]), m3 = fmaxf(m3, lp[0]);
         }
+        // S - m_k: +0 for a candidate, negative otherwise (S + 0.0f folds -0 onto +0 first)
         const float4 c = ring[(o + R) % N];                  // centre row
-        const float d0 = c.x - m0, d1 = c.y - m1, d2 = c.z - m2, d3 = c.w - m3;
-        const float e = fmax3(fmaxf(d0, d1), d2, d3);
-        if (__any_sync(FULL, e >= 0.0f && colmask != 0u)) {  // rare: some lane holds a candidate
-            unsigned m = (d0 >= 0.0f ? 1u : 0u) | (d1 >= 0.0f ? 2u : 0u) | (d2 >= 0.0f ? 4u : 0u) |
-                         (d3 >= 0.0f ? 8u : 0u);
-            m &= colmask;
-            const float v[4] = {c.x, c.y, c.z, c.w};
-            int tot = 0, mypos[4];
+        const unsigned s0 = __float_as_uint((c.x + 0.0f) - m0) >> 31, s1 = __float_as_uint((c.y + 0.0f) - m1) >> 31;
+        const unsigned s2 = __float_as_uint((c.z + 0.0f) - m2) >> 31, s3 = __float_as_uint((c.w + 0.0f) - m3) >> 31;
+        neg[o >> 3] |= (s0 | (s1 << 1) | (s2 << 2) | (s3 << 3)) << (4 * (o & 7));
+    }
+    // candidate bits of this lane: valid rows (R <= y < H-R) x valid columns, not negative
+    unsigned cm[TH / 8];
+    int n = 0;
+    {
+        const int o_lo = R - y0 > 0 ? R - y0 : 0;            // first valid output row
+        const int o_hi = H - R - y0 < TH ? H - R - y0 : TH;  // one past the last valid output row
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const unsigned bal = __ballot_sync(FULL, (m >> k) & 1u);
-                mypos[k] = tot + __popc(bal & ((1u << lane) - 1u));
-                tot += __popc(bal);
-            }
-#pragma unroll
-            for (int k = 0; k < 4; ++k)
-                if ((m >> k) & 1u) seg[cnt + mypos[k]] = make_key(v[k], y * W + X + k);
-            cnt += tot;
+        for (int h = 0; h < TH / 8; ++h) {
+            int a = o_lo - 8 * h, b = o_hi - 8 * h;          // valid rows of this word: [a, b) clipped to [0, 8]
+            a = a < 0 ? 0 : (a > 8 ? 8 : a);
+            b = b < 0 ? 0 : (b > 8 ? 8 : b);
+            const unsigned rows = b > a ? static_cast<unsigned>(((1ull << (4 * b)) - 1ull) & ~((1ull << (4 * a)) - 1ull)) : 0u;
+            cm[h] = ~neg[h] & rows & (colmask * 0x11111111u);
+            n += __popc(cm[h]);
         }
     }
-    return cnt;
+    if (!__any_sync(FULL, n != 0)) return 0;
+    int incl = n;                                            // warp inclusive scan of the per-lane counts
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const int up = __shfl_up_sync(FULL, incl, d);
+        if (lane >= d) incl += up;
+    }
+    const int total = __shfl_sync(FULL, incl, 31);
+    int pos = incl - n;
+#pragma unroll
+    for (int h = 0; h < TH / 8; ++h) {
+        unsigned bits = cm[h];
+        while (bits) {                                       // rare: a few set bits per strip-tile
+            const int bit = __ffs(bits) - 1;
+            bits &= bits - 1;
+            const int o = 8 * h + (bit >> 2), k = bit & 3;
+            const float v = box[(o + R) * BOX_W + 4 * lane + k];
+            seg[pos++] = make_key(v, (y0 + o) * W + X + k);
+        }
+    }
+    return total;
 }
 
 // strip-tile index -> (image, tile row, strip)
