@@ -128,21 +128,57 @@ cudaError_t launch_nms(dkd_ctx* ctx, const ExtractArgs& a, int strips_x, int til
     return cudaGetLastError();
 }
 
-template <int R>
-cudaError_t launch_rg(const ExtractArgs& a, const int32_t* sel, cudaStream_t st) {
-    const int nslots = a.B * a.top_k;
-    const int grid = (nslots + RG_THREADS / 32 - 1) / (RG_THREADS / 32);
-    const unsigned char* d = static_cast<const unsigned char*>(a.desc);
-    unsigned char* od = static_cast<unsigned char*>(a.out_desc);
-#define RG_ARGS a.score, a.H, a.W, sel, nslots, a.top_k, a.T, d, a.Hd, a.Wd, a.D, a.stride, a.out_kpts, a.out_scores, a.out_offset, od
-    if (a.desc == nullptr)
-        k_refine_gather<R, -1><<<grid, RG_THREADS, 0, st>>>(RG_ARGS);
-    else if (a.desc_dtype == DKD_F16)
-        k_refine_gather<R, DKD_F16><<<grid, RG_THREADS, 0, st>>>(RG_ARGS);
-    else
-        k_refine_gather<R, DKD_F32><<<grid, RG_THREADS, 0, st>>>(RG_ARGS);
-#undef RG_ARGS
+FastDiv make_fastdiv(uint32_t d) {                          // exact n / d for every 32-bit n (d >= 1)
+    uint32_t l = 0;
+    while ((1ull << l) < d) ++l;
+    FastDiv f;
+    f.m = static_cast<uint32_t>(((1ull << 32) * ((1ull << l) - d)) / d + 1);
+    f.s1 = l < 1 ? l : 1;
+    f.s2 = l > 0 ? l - 1 : 0;
+    return f;
+}
+
+SampleAxis make_axis(int stride, int n) {
+    SampleAxis a;
+    a.den = make_fastdiv(2u * static_cast<uint32_t>(stride));
+    a.s = stride;
+    a.inv_den = 1.0f / (2.0f * static_cast<float>(stride));
+    a.inv_s = 1.0f / static_cast<float>(stride);
+    a.n = n;
+    return a;
+}
+
+template <int DT, int G>
+cudaError_t launch_rg_g(const RGParams& p, int B, cudaStream_t st) {
+    const dim3 grid((p.top_k + RG_THREADS / G - 1) / (RG_THREADS / G), B);
+    k_refine_gather<DT, G><<<grid, RG_THREADS, 0, st>>>(p);
     return cudaGetLastError();
+}
+
+template <int DT>
+cudaError_t launch_rg_dt(const RGParams& p, int B, cudaStream_t st) {
+    if (p.nchunk <= 8) return launch_rg_g<DT, 8>(p, B, st);
+    if (p.nchunk <= 16) return launch_rg_g<DT, 16>(p, B, st);
+    return launch_rg_g<DT, 32>(p, B, st);
+}
+
+cudaError_t launch_rg(const ExtractArgs& a, const int32_t* sel, cudaStream_t st) {
+    RGParams p;
+    memset(&p, 0, sizeof(p));
+    p.score = a.score; p.H = a.H; p.W = a.W;
+    p.divW = make_fastdiv(static_cast<uint32_t>(a.W));
+    p.sel_idx = sel; p.top_k = a.top_k; p.r = a.r;
+    p.kscale = static_cast<float>(1.4426950408889634 / static_cast<double>(a.T));
+    p.out_kpts = a.out_kpts; p.out_scores = a.out_scores; p.out_off = a.out_offset;
+    if (a.desc == nullptr) return launch_rg_g<-1, 8>(p, a.B, st);
+    const size_t esz = a.desc_dtype == DKD_F16 ? 2 : 4;
+    p.desc = static_cast<const unsigned char*>(a.desc);
+    p.nchunk = static_cast<int>(a.D * esz / 16);
+    p.img_bytes = static_cast<size_t>(a.Hd) * a.Wd * a.D * esz;
+    p.ax = make_axis(a.stride, a.Wd);
+    p.ay = make_axis(a.stride, a.Hd);
+    p.out_desc = static_cast<unsigned char*>(a.out_desc);
+    return a.desc_dtype == DKD_F16 ? launch_rg_dt<DKD_F16>(p, a.B, st) : launch_rg_dt<DKD_F32>(p, a.B, st);
 }
 
 // Enqueue the three kernels of one extract on `st`.  No sync, no allocation: capture-safe.
@@ -168,12 +204,7 @@ cudaError_t enqueue(dkd_ctx* ctx, const ExtractArgs& a, cudaStream_t st, bool pr
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if ((e = mark()) != cudaSuccess) return e;
-    switch (a.r) {
-        case 1: e = launch_rg<1>(a, sel, st); break;
-        case 2: e = launch_rg<2>(a, sel, st); break;
-        case 3: e = launch_rg<3>(a, sel, st); break;
-        default: e = launch_rg<4>(a, sel, st); break;
-    }
+    e = launch_rg(a, sel, st);
     if (e != cudaSuccess) return e;
     if ((e = mark()) != cudaSuccess) return e;
     if (prof) ctx->prof_n = nk - 1;
@@ -197,6 +228,7 @@ int validate(dkd_ctx* ctx, const ExtractArgs& a) {
             return fail(ctx, DKD_ERR_UNSUPPORTED, "desc_dtype must be DKD_F32 or DKD_F16");
     }
     if (a.r > DKD_MAX_RADIUS) return fail(ctx, DKD_ERR_UNSUPPORTED, "r > DKD_MAX_RADIUS");
+    if (a.B > 65535) return fail(ctx, DKD_ERR_UNSUPPORTED, "B > 65535");
     if (reinterpret_cast<uintptr_t>(a.score) & 3) return fail(ctx, DKD_ERR_UNSUPPORTED, "score not 4-byte aligned");
     if (a.desc) {
         const size_t rowb = static_cast<size_t>(a.D) * (a.desc_dtype == DKD_F16 ? 2 : 4);
@@ -205,7 +237,7 @@ int validate(dkd_ctx* ctx, const ExtractArgs& a) {
         if ((reinterpret_cast<uintptr_t>(a.desc) & 15) || (reinterpret_cast<uintptr_t>(a.out_desc) & 15))
             return fail(ctx, DKD_ERR_UNSUPPORTED, "desc / out_desc not 16-byte aligned");
         if (a.D > ctx->p.max_dim) return fail(ctx, DKD_ERR_CAPACITY, "D > max_dim");
-        if (static_cast<long long>(a.stride) * 2 > 0x3fffffff) return fail(ctx, DKD_ERR_UNSUPPORTED, "stride too large");
+        if (a.stride > (1 << 20)) return fail(ctx, DKD_ERR_UNSUPPORTED, "stride too large");
     }
     if (a.B > ctx->p.max_batch || a.H > ctx->p.max_h || a.W > ctx->p.max_w || a.top_k > ctx->p.max_top_k)
         return fail(ctx, DKD_ERR_CAPACITY, "B, H, W or top_k above the dkd_create maxima");

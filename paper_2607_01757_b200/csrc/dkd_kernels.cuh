@@ -33,7 +33,7 @@ constexpr int MAX_R = 4;
 constexpr int NMS_STAGES = 2;            // TMA boxes in flight / in use per warp
 constexpr int SEL_THREADS = 1024;
 constexpr int SORT_CAP = 8192;           // keys sorted in shared memory by k_select (64 KB)
-constexpr int RG_THREADS = 256;          // k_refine_gather: 8 warps, one warp per output slot
+constexpr int RG_THREADS = 256;          // k_refine_gather: 8 warps, 8..32 keypoints per CTA
 
 __host__ __device__ constexpr int box_rows(int R) { return TH + 2 * R; }
 __host__ __device__ constexpr int box_bytes(int R) { return BOX_W * box_rows(R) * 4; }     // multiple of 512
@@ -484,12 +484,51 @@ __global__ void __launch_bounds__(SEL_THREADS) k_select(const uint64_t* __restri
     if (tid == 0) out_count[b] = K;
 }
 
-// ---- k_refine_gather: one warp per output slot (b, i) -----------------------------------------------
-__device__ __forceinline__ float warp_sum(float v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
+// ---- k_refine_gather: one G-lane group per output slot (b, i) ---------------------------------------
+// G = 8, 16 or 32 lanes = the number of 16-byte chunks of one descriptor row rounded up to a power of
+// two (D=128 f16 / D=64 f32: 16 lanes, two keypoints per warp; D=256 f16: 32; D=64 f16: 8), so every
+// lane issues exactly one 16-byte load per corner row and no lane idles in the gather.
+// grid = (ceil(top_k / (RG_THREADS / G)), B): the image index is blockIdx.y (no division by top_k).
+
+// exact unsigned division by a runtime constant (Granlund-Montgomery): q = (t + ((n - t) >> s1)) >> s2,
+// t = umulhi(m, n); host-computed by make_fastdiv; exact for every 32-bit n.
+struct FastDiv {
+    uint32_t m, s1, s2;
+};
+__device__ __forceinline__ uint32_t fast_div(uint32_t n, const FastDiv d) {
+    const uint32_t t = __umulhi(d.m, n);
+    return (t + ((n - t) >> d.s1)) >> d.s2;
 }
+
+struct SampleAxis {          // u = (p + 0.5)/s - 0.5 along one axis, p = xi + d (G12, G13)
+    FastDiv den;             // division by 2s
+    int s;                   // stride
+    float inv_den, inv_s;    // 1/(2s), 1/s (exact for power-of-two strides)
+    int n;                   // map extent along this axis
+};
+// Splits u into an integer cell and a fraction without ever forming the large coordinate in fp32:
+// 2u = (2 xi + 1 - s)/s + 2d/s, so u = q + rem/(2s) + d/s with (q, rem) an exact integer division
+// (biased by +2s to keep the numerator non-negative).  Clamped to [0, n-1].
+__device__ __forceinline__ void sample_axis(int xi, float d, const SampleAxis a, int& i0, int& i1, float& f) {
+    float t;
+    int q;
+    if (a.s == 1) {                                          // warp-uniform
+        q = xi;
+        t = d;
+    } else {
+        const uint32_t num = static_cast<uint32_t>(2 * xi + 1 + a.s);    // (2 xi + 1 - s) + 2s  >= 2
+        const uint32_t qq = fast_div(num, a.den);
+        q = static_cast<int>(qq) - 1;
+        t = fmaf(static_cast<float>(num - qq * 2u * static_cast<uint32_t>(a.s)), a.inv_den, d * a.inv_s);
+    }
+    const float ft = floorf(t);
+    i0 = q + static_cast<int>(ft);
+    f = t - ft;
+    if (i0 < 0) { i0 = 0; f = 0.0f; }
+    else if (i0 >= a.n - 1) { i0 = a.n - 1; f = 0.0f; }
+    i1 = i0 + 1 < a.n - 1 ? i0 + 1 : a.n - 1;
+}
+
 __device__ __forceinline__ uint4 ld_stream16(const void* p) {
     uint4 r;
     asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
@@ -497,20 +536,10 @@ __device__ __forceinline__ uint4 ld_stream16(const void* p) {
                  : "l"(p));
     return r;
 }
-// sample position along one axis: u = (p + 0.5)/s - 0.5 with p = xi + d, split into an integer cell and
-// a fraction without ever forming the large coordinate in fp32 (G12); clamped to [0, n-1].
-__device__ __forceinline__ void sample_axis(int xi, float d, int s, int n, int& i0, int& i1, float& f) {
-    const int num = 2 * xi + 1 - s, den = 2 * s;
-    int q = num / den;
-    int rem = num - q * den;
-    if (rem < 0) { rem += den; --q; }
-    const float t = static_cast<float>(rem) / static_cast<float>(den) + d / static_cast<float>(s);
-    const float ft = floorf(t);
-    i0 = q + static_cast<int>(ft);
-    f = t - ft;
-    if (i0 < 0) { i0 = 0; f = 0.0f; }
-    else if (i0 >= n - 1) { i0 = n - 1; f = 0.0f; }
-    i1 = i0 + 1 < n - 1 ? i0 + 1 : n - 1;
+__device__ __forceinline__ float ex2_approx(float x) {      // 2^x, MUFU.EX2 (max 2 ulp)
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
 }
 
 template <int DT> struct ChunkT;                            // one 16-byte chunk of a descriptor row
@@ -550,91 +579,107 @@ __device__ __forceinline__ uint4 float_to_chunk(const float* f) {
     return q;
 }
 
-constexpr int MAX_CHUNK_ITERS = DKD_MAX_ROW_BYTES / 16 / 32;          // 4
+struct RGParams {
+    const float* score;
+    int H, W;
+    FastDiv divW;                       // idx -> (y, x)
+    const int32_t* sel_idx;             // [B, top_k] linear index, -1 in padding
+    int top_k, r;
+    float kscale;                       // log2(e) / T : w = 2^((S - S_c) * kscale) = exp((S - S_c)/T)
+    const unsigned char* desc;
+    int nchunk;                         // D * elemsize / 16
+    size_t img_bytes;                   // Hd * Wd * D * elemsize
+    SampleAxis ax, ay;
+    float* out_kpts;
+    float* out_scores;
+    float* out_off;
+    unsigned char* out_desc;
+};
 
-// R: window radius; DT: DKD_F32 / DKD_F16 descriptor maps, or -1 for keypoints only.
-template <int R, int DT>
-__global__ void __launch_bounds__(RG_THREADS) k_refine_gather(
-    const float* __restrict__ score, int H, int W, const int32_t* __restrict__ sel_idx, int nslots, int top_k,
-    float T, const unsigned char* __restrict__ desc, int Hd, int Wd, int D, int stride,
-    float* __restrict__ out_kpts, float* __restrict__ out_scores, float* __restrict__ out_off,
-    unsigned char* __restrict__ out_desc) {
-    const int lane = threadIdx.x & 31;
-    const int slot = blockIdx.x * (RG_THREADS / 32) + (threadIdx.x >> 5);
-    if (slot >= nslots) return;
-    const int idx = sel_idx[slot];
+// DT: DKD_F32 / DKD_F16 descriptor maps, or -1 for keypoints only.  G: lanes per keypoint.
+template <int DT, int G>
+__global__ void __launch_bounds__(RG_THREADS) k_refine_gather(const __grid_constant__ RGParams p) {
+    constexpr int ITERS = (G == 32) ? DKD_MAX_ROW_BYTES / 16 / 32 : 1;   // chunks per lane
+    const int gl = threadIdx.x & (G - 1);                   // lane within the group
+    const unsigned gmask = (G == 32) ? 0xffffffffu : (((1u << G) - 1u) << ((threadIdx.x & 31) & ~(G - 1)));
+    const int i_img = blockIdx.x * (RG_THREADS / G) + threadIdx.x / G;
+    if (i_img >= p.top_k) return;                           // whole groups leave together
+    const int b = blockIdx.y;
+    const size_t slot = static_cast<size_t>(b) * p.top_k + i_img;
+    const int idx = __ldg(p.sel_idx + slot);
     constexpr int ESZ = (DT == DKD_F16) ? 2 : 4;
-    const int nchunk = (DT >= 0) ? (D * ESZ) >> 4 : 0;
 
     if (idx < 0) {                                          // step a5: zero padding
-        if (lane < 2) out_kpts[2 * static_cast<size_t>(slot) + lane] = 0.0f;
-        if (lane == 2) out_scores[slot] = 0.0f;
-        if (out_off != nullptr && lane >= 4 && lane < 6) out_off[2 * static_cast<size_t>(slot) + lane - 4] = 0.0f;
+        if (gl < 2) p.out_kpts[2 * slot + gl] = 0.0f;
+        if (gl == 2) p.out_scores[slot] = 0.0f;
+        if (p.out_off != nullptr && gl >= 4 && gl < 6) p.out_off[2 * slot + gl - 4] = 0.0f;
         if constexpr (DT >= 0) {
-            uint4* o = reinterpret_cast<uint4*>(out_desc + static_cast<size_t>(slot) * D * ESZ);
-            for (int ch = lane; ch < nchunk; ch += 32) o[ch] = make_uint4(0u, 0u, 0u, 0u);
+            uint4* o = reinterpret_cast<uint4*>(p.out_desc + slot * p.nchunk * 16);
+            for (int ch = gl; ch < p.nchunk; ch += G) o[ch] = make_uint4(0u, 0u, 0u, 0u);
         }
         return;
     }
 
-    // ---- step a3: soft-argmax over the (2R+1)^2 window.  Lane q < (R+1)^2 owns the mirror orbit
-    // {(+-i, +-j)}, i, j >= 0; differences of mirrored weights are formed first, so a symmetric
-    // window refines to exactly (0, 0).
-    const int b = slot / top_k;
-    const int y = idx / W, x = idx - y * W;
-    const float* S = score + static_cast<size_t>(b) * H * W;
+    // ---- step a3: soft-argmax over the (2r+1)^2 window.  Orbit q < (r+1)^2 = the mirror images
+    // {(+-i, +-j)}, i, j >= 0, of one window element; differences of mirrored weights are formed
+    // first, so a window symmetric about an axis refines to exactly 0 along it.
+    const int W = p.W;
+    const int y = static_cast<int>(fast_div(static_cast<uint32_t>(idx), p.divW)), x = idx - y * W;
+    const float* S = p.score + static_cast<size_t>(b) * p.H * W;
     const float c = __ldg(S + idx);
+    const int r1 = p.r + 1, norb = r1 * r1, inv_r1 = (256 + p.r) / r1;   // j = q / r1 for q < 25
     float sx = 0.0f, sy = 0.0f, z = 0.0f;
-    if (lane < (R + 1) * (R + 1)) {
-        const int j = lane / (R + 1), i = lane - j * (R + 1);
+    for (int q = gl; q < norb; q += G) {
+        const int j = (q * inv_r1) >> 8, i = q - j * r1;
         const float vpp = __ldg(S + (y + j) * W + (x + i));
         const float vmp = __ldg(S + (y + j) * W + (x - i));
         const float vpm = __ldg(S + (y - j) * W + (x + i));
         const float vmm = __ldg(S + (y - j) * W + (x - i));
-        const float wpp = expf(__fdiv_rn(vpp - c, T));
-        const float wmp = expf(__fdiv_rn(vmp - c, T));
-        const float wpm = expf(__fdiv_rn(vpm - c, T));
-        const float wmm = expf(__fdiv_rn(vmm - c, T));
+        const float wpp = ex2_approx((vpp - c) * p.kscale);
+        const float wmp = ex2_approx((vmp - c) * p.kscale);
+        const float wpm = ex2_approx((vpm - c) * p.kscale);
+        const float wmm = ex2_approx((vmm - c) * p.kscale);
         const float mi = i > 0 ? 1.0f : 0.0f, mj = j > 0 ? 1.0f : 0.0f;
-        sx = static_cast<float>(i) * ((wpp - wmp) + mj * (wpm - wmm));
-        sy = static_cast<float>(j) * ((wpp - wpm) + mi * (wmp - wmm));
-        z = wpp + mi * wmp + mj * (wpm + mi * wmm);
+        sx += static_cast<float>(i) * ((wpp - wmp) + mj * (wpm - wmm));
+        sy += static_cast<float>(j) * ((wpp - wpm) + mi * (wmp - wmm));
+        z += wpp + mi * wmp + mj * (wpm + mi * wmm);
     }
-    sx = warp_sum(sx);
-    sy = warp_sum(sy);
-    z = warp_sum(z);
-    const float dx = __fdiv_rn(sx, z), dy = __fdiv_rn(sy, z);
-    if (lane == 0) {
-        out_kpts[2 * static_cast<size_t>(slot)] = static_cast<float>(x) + dx;
-        out_kpts[2 * static_cast<size_t>(slot) + 1] = static_cast<float>(y) + dy;
-        out_scores[slot] = c;                               // raw S at the integer peak (G7)
-        if (out_off != nullptr) {
-            out_off[2 * static_cast<size_t>(slot)] = dx;
-            out_off[2 * static_cast<size_t>(slot) + 1] = dy;
-        }
+#pragma unroll
+    for (int o = G / 2; o > 0; o >>= 1) {
+        sx += __shfl_xor_sync(gmask, sx, o);
+        sy += __shfl_xor_sync(gmask, sy, o);
+        z += __shfl_xor_sync(gmask, z, o);
+    }
+    const float inv_z = __frcp_rn(z);                        // z >= 1 (the centre weight is exactly 1)
+    const float dx = sx * inv_z, dy = sy * inv_z;
+    if (gl == 0) {
+        *reinterpret_cast<float2*>(p.out_kpts + 2 * slot) = make_float2(static_cast<float>(x) + dx, static_cast<float>(y) + dy);
+        p.out_scores[slot] = c;                              // raw S at the integer peak (G7)
+        if (p.out_off != nullptr) *reinterpret_cast<float2*>(p.out_off + 2 * slot) = make_float2(dx, dy);
     }
 
     // ---- step a4: bilinear gather of the four corner rows (16-byte loads), fp32 accumulate, L2 norm
     if constexpr (DT >= 0) {
         int x0, x1, y0, y1;
         float fx, fy;
-        sample_axis(x, dx, stride, Wd, x0, x1, fx);
-        sample_axis(y, dy, stride, Hd, y0, y1, fy);
+        sample_axis(x, dx, p.ax, x0, x1, fx);
+        sample_axis(y, dy, p.ay, y0, y1, fy);
         const float w00 = (1.0f - fy) * (1.0f - fx), w01 = (1.0f - fy) * fx;
         const float w10 = fy * (1.0f - fx), w11 = fy * fx;
-        const size_t rowb = static_cast<size_t>(D) * ESZ;
-        const unsigned char* base = desc + static_cast<size_t>(b) * Hd * Wd * rowb;
+        const size_t rowb = static_cast<size_t>(p.nchunk) * 16;
+        const int Wd = p.ax.n;
+        const unsigned char* base = p.desc + static_cast<size_t>(b) * p.img_bytes;
         const uint4* p00 = reinterpret_cast<const uint4*>(base + (static_cast<size_t>(y0) * Wd + x0) * rowb);
         const uint4* p01 = reinterpret_cast<const uint4*>(base + (static_cast<size_t>(y0) * Wd + x1) * rowb);
         const uint4* p10 = reinterpret_cast<const uint4*>(base + (static_cast<size_t>(y1) * Wd + x0) * rowb);
         const uint4* p11 = reinterpret_cast<const uint4*>(base + (static_cast<size_t>(y1) * Wd + x1) * rowb);
         constexpr int N = ChunkT<DT >= 0 ? DT : 0>::N;
-        float acc[MAX_CHUNK_ITERS][N];
+        float acc[ITERS][N];
         float ss = 0.0f;
 #pragma unroll
-        for (int it = 0; it < MAX_CHUNK_ITERS; ++it) {
-            const int ch = lane + 32 * it;
-            if (ch < nchunk) {
+        for (int it = 0; it < ITERS; ++it) {
+            const int ch = gl + G * it;
+            if (ch < p.nchunk) {
                 const uint4 q00 = ld_stream16(p00 + ch), q01 = ld_stream16(p01 + ch);
                 const uint4 q10 = ld_stream16(p10 + ch), q11 = ld_stream16(p11 + ch);
                 float a[N], bq[N], cq[N], dq[N];
@@ -650,13 +695,14 @@ __global__ void __launch_bounds__(RG_THREADS) k_refine_gather(
                 }
             }
         }
-        ss = warp_sum(ss);
-        const float inv = __fdiv_rn(1.0f, fmaxf(sqrtf(ss), 1e-12f));
-        uint4* o = reinterpret_cast<uint4*>(out_desc + static_cast<size_t>(slot) * rowb);
 #pragma unroll
-        for (int it = 0; it < MAX_CHUNK_ITERS; ++it) {
-            const int ch = lane + 32 * it;
-            if (ch < nchunk) {
+        for (int o = G / 2; o > 0; o >>= 1) ss += __shfl_xor_sync(gmask, ss, o);
+        const float inv = __frcp_rn(fmaxf(sqrtf(ss), 1e-12f));
+        uint4* o = reinterpret_cast<uint4*>(p.out_desc + slot * rowb);
+#pragma unroll
+        for (int it = 0; it < ITERS; ++it) {
+            const int ch = gl + G * it;
+            if (ch < p.nchunk) {
                 float f[N];
 #pragma unroll
                 for (int e = 0; e < N; ++e) f[e] = acc[it][e] * inv;
