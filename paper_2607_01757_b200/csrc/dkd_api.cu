@@ -199,7 +199,7 @@ cudaError_t enqueue(dkd_ctx* ctx, const ExtractArgs& a, cudaStream_t st, bool pr
     if (e != cudaSuccess) return e;
     if ((e = mark()) != cudaSuccess) return e;
     int32_t* sel = a.out_index ? a.out_index : ctx->sel_idx;
-    k_select<<<a.B, SEL_THREADS, SORT_CAP * sizeof(uint64_t), st>>>(ctx->cand, ctx->tile_cnt, tpi, a.top_k, sel,
+    k_select<<<a.B, SEL_THREADS, SEL_SMEM_BYTES, st>>>(ctx->cand, ctx->tile_cnt, tpi, a.top_k, sel,
                                                                     a.out_count);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
@@ -358,7 +358,7 @@ int dkd_create(const dkd_create_params* p, dkd_ctx** out) {
     CKC(setup_nms<2>(ctx));
     CKC(setup_nms<3>(ctx));
     CKC(setup_nms<4>(ctx));
-    CKC(cudaFuncSetAttribute(k_select, cudaFuncAttributeMaxDynamicSharedMemorySize, SORT_CAP * sizeof(uint64_t)));
+    CKC(cudaFuncSetAttribute(k_select, cudaFuncAttributeMaxDynamicSharedMemorySize, SEL_SMEM_BYTES));
     const size_t tx = (p->max_w + STRIP_W - 1) / STRIP_W, ty = (p->max_h + TH - 1) / TH;
     ctx->max_tiles = tx * ty * p->max_batch;
     const size_t b_cand = align256(ctx->max_tiles * SEG_CAP * sizeof(uint64_t));

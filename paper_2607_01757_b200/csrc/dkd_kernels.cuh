@@ -32,7 +32,7 @@ constexpr int SEG_CAP = STRIP_W * TH;    // 1920 = worst-case candidates of a st
 constexpr int MAX_R = 4;
 constexpr int NMS_STAGES = 2;            // TMA boxes in flight / in use per warp
 constexpr int SEL_THREADS = 1024;
-constexpr int SORT_CAP = 8192;           // keys sorted in shared memory by k_select (64 KB)
+constexpr int SORT_CAP = 8192;           // keys ordered in shared memory by k_select
 constexpr int RG_THREADS = 256;          // k_refine_gather: 8 warps, 8..32 keypoints per CTA
 
 __host__ __device__ constexpr int box_rows(int R) { return TH + 2 * R; }
@@ -330,11 +330,22 @@ __global__ void __launch_bounds__(PLAIN_WARPS * 32) k_nms_plain(const float* __r
 }
 
 // ---- k_select: per-image top-k select + order ---------------------------------------------------
-// One CTA per image.  n = sum of the image's tile counts.
-//   n <= SORT_CAP : gather every key into shared memory, bitonic sort (descending), emit the first K.
+// One CTA per image.  n = sum of the image's strip-tile counts.
 //   n >  SORT_CAP : MSB-first radix select (8-bit digits, warp-aggregated shared-memory histogram)
-//                   narrows to a lower bound `lo` with  top_k <= #{key >= lo} <= SORT_CAP, then as above.
+//                   narrows to a lower bound `lo` with  top_k <= #{key >= lo} <= SORT_CAP.
+//   gather        : every key >= lo (all keys when n <= SORT_CAP) is copied into shared memory.
+//   order         : bucket rank (the common case) — one pass of a monotone bucket function over the
+//                   score bits (NB buckets spanning [min, max] of the gathered scores), an exclusive
+//                   scan of the bucket counts, a scatter into bucket order, and an exact rank
+//                   = keys in better buckets + keys of the own bucket with a larger key.  ~100
+//                   lane-instructions per key instead of the ~550 of a 64-bit bitonic network.
+//                   Falls back to the in-smem bitonic sort when one bucket holds more than
+//                   BUCKET_LIMIT keys (near-constant maps).
 // Keys are unique (they embed the pixel index) so the result is the unique (score desc, idx asc) order.
+constexpr int NB = 4096;                 // buckets of the rank pass
+constexpr int BUCKET_LIMIT = 1024;       // largest bucket the rank pass accepts
+constexpr int SEL_SMEM_BYTES = 2 * SORT_CAP * 8 + 2 * NB * 4;     // keys | sorted | base | cur = 160 KB
+
 __device__ __forceinline__ int block_sum_1024(int v, int* s_red) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 #pragma unroll
@@ -348,25 +359,32 @@ __device__ __forceinline__ int block_sum_1024(int v, int* s_red) {
     return r;
 }
 
-__global__ void __launch_bounds__(SEL_THREADS) k_select(const uint64_t* __restrict__ cand,
-                                                        const int* __restrict__ tile_cnt, int tpi, int top_k,
-                                                        int32_t* __restrict__ sel_idx,
-                                                        int32_t* __restrict__ out_count) {
+__global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __restrict__ cand,
+                                                           const int* __restrict__ tile_cnt, int tpi, int top_k,
+                                                           int32_t* __restrict__ sel_idx,
+                                                           int32_t* __restrict__ out_count) {
     extern __shared__ __align__(16) unsigned char sel_smem[];
-    uint64_t* keys = reinterpret_cast<uint64_t*>(sel_smem);            // SORT_CAP entries
+    uint64_t* keys = reinterpret_cast<uint64_t*>(sel_smem);            // SORT_CAP entries (gathered, unordered)
+    uint64_t* sorted = keys + SORT_CAP;                                // SORT_CAP entries (bucket order)
+    int* base = reinterpret_cast<int*>(sorted + SORT_CAP);             // NB
+    int* cur = base + NB;                                              // NB
     __shared__ int s_hist[257];
     __shared__ int s_red[32];
-    __shared__ int s_n, s_digit, s_cum, s_h;
+    __shared__ int s_n, s_digit, s_cum, s_h, s_maxb;
+    __shared__ unsigned s_hi, s_lo;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     constexpr int NW = SEL_THREADS / 32;
+    constexpr unsigned FULL = 0xffffffffu;
     const int b = blockIdx.x;
     const int* cnt = tile_cnt + static_cast<size_t>(b) * tpi;
     const uint64_t* seg0 = cand + static_cast<size_t>(b) * tpi * SEG_CAP;
 
     int local = 0;
     for (int t = tid; t < tpi; t += SEL_THREADS) local += cnt[t];
-    const int n = block_sum_1024(local, s_red);
+    if (tid == 0) { s_n = 0; s_hi = 0u; s_lo = 0xffffffffu; s_maxb = 0; }
+    for (int i = tid; i < NB; i += SEL_THREADS) { base[i] = 0; cur[i] = 0; }
+    const int n = block_sum_1024(local, s_red);             // (its barriers also publish the initialisers)
 
     uint64_t lo = 0;                                        // gather keys >= lo (0: all of them)
     if (n > SORT_CAP) {
@@ -387,7 +405,7 @@ __global__ void __launch_bounds__(SEL_THREADS) k_select(const uint64_t* __restri
                         const bool match = (shift == 56) || ((k >> (shift + 8)) == (prefix >> (shift + 8)));
                         if (match) digit = static_cast<int>((k >> shift) & 255u);
                     }
-                    const unsigned peers = __match_any_sync(0xffffffffu, digit);
+                    const unsigned peers = __match_any_sync(FULL, digit);
                     if (lane == __ffs(peers) - 1) atomicAdd(&s_hist[digit], __popc(peers));
                 }
             }
@@ -399,10 +417,10 @@ __global__ void __launch_bounds__(SEL_THREADS) k_select(const uint64_t* __restri
                 int incl = grp;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) {
-                    const int up = __shfl_up_sync(0xffffffffu, incl, o);
+                    const int up = __shfl_up_sync(FULL, incl, o);
                     if (lane >= o) incl += up;
                 }
-                const unsigned hit = __ballot_sync(0xffffffffu, incl >= need);
+                const unsigned hit = __ballot_sync(FULL, incl >= need);
                 const int owner = __ffs(hit) - 1;           // exists: need <= keys in the bucket
                 if (lane == owner) {
                     int cum = incl - grp;
@@ -428,60 +446,149 @@ __global__ void __launch_bounds__(SEL_THREADS) k_select(const uint64_t* __restri
         lo = prefix;
     }
 
-    if (tid == 0) s_n = 0;
-    __syncthreads();
-    for (int t = warp; t < tpi; t += NW) {
-        const int c = cnt[t];
-        if (c == 0) continue;
-        const uint64_t* seg = seg0 + static_cast<size_t>(t) * SEG_CAP;
-        if (lo == 0) {
-            int base = 0;
-            if (lane == 0) base = atomicAdd(&s_n, c);
-            base = __shfl_sync(0xffffffffu, base, 0);
-            for (int e = lane; e < c; e += 32) keys[base + e] = seg[e];
-        } else {
-            for (int e0 = 0; e0 < c; e0 += 32) {
-                const int e = e0 + lane;
-                const uint64_t k = e < c ? seg[e] : 0ull;
-                const bool take = (e < c) && (k >= lo);
-                const unsigned bal = __ballot_sync(0xffffffffu, take);
+    // ---- gather: 32 strip-tiles per warp iteration; lane l reads tile l's count, the warp copies the
+    // concatenation of the 32 segments with every lane busy (a 5-step search finds an item's tile)
+    unsigned khi = 0u, klo = 0xffffffffu;                   // range of the gathered score words
+    for (int t0 = warp * 32; t0 < tpi; t0 += NW * 32) {
+        const int t = t0 + lane;
+        const int c = t < tpi ? cnt[t] : 0;
+        int incl = c;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int up = __shfl_up_sync(FULL, incl, o);
+            if (lane >= o) incl += up;
+        }
+        const int total = __shfl_sync(FULL, incl, 31);
+        if (total == 0) continue;                           // warp-uniform
+        int gbase = 0;
+        if (lo == 0) {                                      // all keys are kept: reserve the slots at once
+            if (lane == 0) gbase = atomicAdd(&s_n, total);
+            gbase = __shfl_sync(FULL, gbase, 0);
+        }
+        for (int e0 = 0; e0 < total; e0 += 32) {
+            const int e = e0 + lane;
+            int tl = 0;                                     // first lane whose inclusive count exceeds e
+#pragma unroll
+            for (int step = 16; step > 0; step >>= 1) {
+                const int v = __shfl_sync(FULL, incl, tl + step - 1);
+                if (v <= e) tl += step;
+            }
+            const int excl = __shfl_sync(FULL, incl - c, tl);
+            uint64_t k = 0ull;
+            if (e < total) k = seg0[static_cast<size_t>(t0 + tl) * SEG_CAP + (e - excl)];
+            if (lo == 0) {
+                if (e < total) keys[gbase + e] = k;
+            } else {
+                const bool take = (e < total) && (k >= lo);
+                const unsigned bal = __ballot_sync(FULL, take);
                 if (bal) {
-                    int base = 0;
-                    if (lane == 0) base = atomicAdd(&s_n, __popc(bal));
-                    base = __shfl_sync(0xffffffffu, base, 0);
-                    if (take) keys[base + __popc(bal & ((1u << lane) - 1u))] = k;
+                    int pb = 0;
+                    if (lane == 0) pb = atomicAdd(&s_n, __popc(bal));
+                    pb = __shfl_sync(FULL, pb, 0);
+                    if (take) keys[pb + __popc(bal & ((1u << lane) - 1u))] = k;
                 }
+                if (!take) k = 0ull;
+            }
+            if (k != 0ull) {
+                const unsigned kb = static_cast<unsigned>(k >> 32);
+                khi = kb > khi ? kb : khi;
+                klo = kb < klo ? kb : klo;
             }
         }
     }
+    khi = __reduce_max_sync(FULL, khi);
+    klo = __reduce_min_sync(FULL, klo);
+    if (lane == 0 && khi >= klo) { atomicMax(&s_hi, khi); atomicMin(&s_lo, klo); }
     __syncthreads();
     const int m = s_n;
+    const int K = m < top_k ? m : top_k;
+    int32_t* out = sel_idx + static_cast<size_t>(b) * top_k;
+    for (int i = K + tid; i < top_k; i += SEL_THREADS) out[i] = -1;    // step a5: padding slots
+    if (tid == 0) out_count[b] = K;
+    if (m == 0) return;
+
+    // ---- order, common case: bucket rank ------------------------------------------------------------
+    const unsigned hi = s_hi;
+    const unsigned range = hi - s_lo;
+    const int shift = range >= static_cast<unsigned>(NB) ? (32 - __clz(range)) - 12 : 0;   // (range >> shift) < NB
+    for (int i = tid; i < m; i += SEL_THREADS) atomicAdd(&cur[(hi - static_cast<unsigned>(keys[i] >> 32)) >> shift], 1);
+    __syncthreads();
+    {   // exclusive scan of the NB bucket counts (4 consecutive buckets per thread), largest bucket
+        int c4[NB / SEL_THREADS];
+        int sum = 0, mx = 0;
+#pragma unroll
+        for (int q = 0; q < NB / SEL_THREADS; ++q) {
+            c4[q] = cur[tid * (NB / SEL_THREADS) + q];
+            sum += c4[q];
+            mx = c4[q] > mx ? c4[q] : mx;
+        }
+        int incl = sum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int up = __shfl_up_sync(FULL, incl, o);
+            if (lane >= o) incl += up;
+        }
+        mx = __reduce_max_sync(FULL, mx);
+        if (lane == 31) s_red[warp] = incl;
+        if (lane == 0) atomicMax(&s_maxb, mx);
+        __syncthreads();
+        int woff = s_red[lane];                             // 32 warp totals -> exclusive offsets
+        int wincl = woff;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int up = __shfl_up_sync(FULL, wincl, o);
+            if (lane >= o) wincl += up;
+        }
+        woff = __shfl_sync(FULL, wincl - woff, warp);
+        int run = woff + incl - sum;
+#pragma unroll
+        for (int q = 0; q < NB / SEL_THREADS; ++q) {
+            base[tid * (NB / SEL_THREADS) + q] = run;
+            cur[tid * (NB / SEL_THREADS) + q] = 0;
+            run += c4[q];
+        }
+        __syncthreads();
+    }
+    if (s_maxb <= BUCKET_LIMIT) {                           // block-uniform
+        for (int i = tid; i < m; i += SEL_THREADS) {        // scatter into bucket order
+            const uint64_t k = keys[i];
+            const int d = (hi - static_cast<unsigned>(k >> 32)) >> shift;
+            sorted[base[d] + atomicAdd(&cur[d], 1)] = k;
+        }
+        __syncthreads();
+        for (int i = tid; i < m; i += SEL_THREADS) {        // exact rank inside the own bucket
+            const uint64_t k = sorted[i];
+            const int d = (hi - static_cast<unsigned>(k >> 32)) >> shift;
+            const int s0 = base[d], s1 = s0 + cur[d];
+            int rank = s0;
+            for (int j = s0; j < s1; ++j) rank += sorted[j] > k ? 1 : 0;
+            if (rank < K) out[rank] = key_index(k);
+        }
+        return;
+    }
+
+    // ---- order, fallback: bitonic sort (descending) of the gathered keys in shared memory --------------
     int P = 1;
     while (P < m) P <<= 1;
     for (int i = m + tid; i < P; i += SEL_THREADS) keys[i] = 0ull;     // 0 < every real key
     __syncthreads();
-
     for (int k2 = 2; k2 <= P; k2 <<= 1) {
         for (int j = k2 >> 1; j > 0; j >>= 1) {
             for (int i = tid; i < P; i += SEL_THREADS) {
-                const int p = i ^ j;
-                if (p > i) {
-                    const uint64_t a = keys[i], c = keys[p];
+                const int q = i ^ j;
+                if (q > i) {
+                    const uint64_t a = keys[i], c = keys[q];
                     const bool desc = (i & k2) == 0;
                     if (desc ? (a < c) : (a > c)) {
                         keys[i] = c;
-                        keys[p] = a;
+                        keys[q] = a;
                     }
                 }
             }
             __syncthreads();
         }
     }
-
-    const int K = m < top_k ? m : top_k;
-    int32_t* out = sel_idx + static_cast<size_t>(b) * top_k;
-    for (int i = tid; i < top_k; i += SEL_THREADS) out[i] = i < K ? key_index(keys[i]) : -1;
-    if (tid == 0) out_count[b] = K;
+    for (int i = tid; i < K; i += SEL_THREADS) out[i] = key_index(keys[i]);
 }
 
 // ---- k_refine_gather: one G-lane group per output slot (b, i) ---------------------------------------
