@@ -70,6 +70,20 @@ def peaks():
     return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
+def ncu_traffic(kernel):
+    """dram read + write bytes of one launch of `kernel` at c5, from the committed ncu --set full summary
+    (profiles/traffic_c5.csv: a text table copied from the capture, not something measured in this run)."""
+    tp = os.path.join(ROOT, "profiles", "traffic_c5.csv")
+    try:
+        import csv
+        for row in csv.DictReader(open(tp)):
+            if row["kernel"] == kernel:
+                return int(row["dram_read_bytes"]) + int(row["dram_write_bytes"])
+    except Exception:                                            # noqa: BLE001
+        pass
+    return None
+
+
 class ClockSampler:
     """Samples SM clock + throttle reasons through NVML while `active` (DURING the timed regions)."""
 
@@ -376,13 +390,7 @@ def run_ours(args):
             #   nms: the score maps, read once;  refine_gather: corner rows + outputs;  select: candidate keys
             algo = {"nms": cb5["score"], "refine_gather": cb5["corners"] + cb5["outputs"], "select": 0}
             dom = max(kt5, key=kt5.get)
-            traffic = None
-            tp = os.path.join(ROOT, "profiles", "traffic.json")  # ncu --set full dram bytes per launch, if captured
-            if os.path.exists(tp):
-                try:
-                    traffic = json.load(open(tp)).get(dom)
-                except Exception:                                # noqa: BLE001
-                    traffic = None
+            traffic = ncu_traffic(dom)
             ach = algo.get(dom, 0) / (kt5[dom] * 1e-6) / 1e9
             roof = {"bound": "hbm", "kernel": dom, "workload": "c5 (B=64 1920x1080)", "achieved": ach, "peak": hbm_peak,
                     "unit": "GB/s", "frac": ach / hbm_peak, "traffic": traffic, "peak_source": peak_src,
