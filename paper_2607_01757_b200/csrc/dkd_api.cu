@@ -5,6 +5,7 @@
 #include <math.h>
 #include <stdio.h>
 #include <string.h>
+#include <stdlib.h>
 
 #include <vector>
 
@@ -94,36 +95,61 @@ int fail_cuda(dkd_ctx* ctx, const char* what, cudaError_t e) {
 
 template <int R>
 cudaError_t setup_nms(dkd_ctx* ctx) {
-    cudaError_t e = cudaFuncSetAttribute(k_nms_tma<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, nms_smem_bytes(R));
+    cudaError_t e = cudaFuncSetAttribute(k_nms_tma<R, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, NMS_SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(k_nms_tma<R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, NMS_SMEM_BYTES);
     if (e != cudaSuccess) return e;
     int n = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_nms_tma<R>, nms_warps(R) * 32, nms_smem_bytes(R));
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_nms_tma<R, true>, NMS_WARPS * 32, NMS_SMEM_BYTES);
     ctx->nms_ctas_per_sm[R] = n > 0 ? n : 1;
     return e;
 }
 
-template <int R>
-cudaError_t launch_nms(dkd_ctx* ctx, const ExtractArgs& a, int strips_x, int tiles_y, int total, cudaStream_t st) {
+// Strip-tiles per unit: as many as possible (the 2R rows above a unit are fetched once per unit) while
+// the units still fill the machine several times over.
+NmsPlan nms_plan(const dkd_ctx* ctx, const ExtractArgs& a) {
+    NmsPlan p;
+    p.H = a.H; p.W = a.W;
+    p.strips_x = (a.W + STRIP_W - 1) / STRIP_W;
+    p.chunks_y = (a.H + TH - 1) / TH;
     // S > thresh  <=>  S >= nextafter(thresh, +inf): the threshold joins the window maximum (dkd_kernels.cuh)
-    const float thr_up = nextafterf(a.thresh, INFINITY);
+    p.thr_up = nextafterf(a.thresh, INFINITY);
+    const long long slots = 2LL * ctx->num_sms * NMS_WARPS;  // resident warps
+    int best = 1;
+    for (int cpu = MAX_CPU; cpu >= 1; --cpu) {
+        const int segs = (p.chunks_y + cpu - 1) / cpu;
+        if (static_cast<long long>(p.strips_x) * segs * a.B >= 4 * slots) { best = cpu; break; }
+    }
+    if (getenv("DKD_CPU")) best = atoi(getenv("DKD_CPU"));
+    p.cpu = best;
+    p.segs = (p.chunks_y + best - 1) / best;
+    p.units = p.strips_x * p.segs * a.B;
+    return p;
+}
+
+template <int R>
+cudaError_t launch_nms(dkd_ctx* ctx, const ExtractArgs& a, cudaStream_t st) {
+    const NmsPlan p = nms_plan(ctx, a);
     if (a.use_tma) {
         CUtensorMap tmap;
         const cuuint64_t dims[3] = {(cuuint64_t)a.W, (cuuint64_t)a.H, (cuuint64_t)a.B};
         const cuuint64_t strides[2] = {(cuuint64_t)a.W * 4, (cuuint64_t)a.W * a.H * 4};
-        const cuuint32_t box[3] = {(cuuint32_t)BOX_W, (cuuint32_t)box_rows(R), 1};
+        const cuuint32_t box[3] = {(cuuint32_t)BOX_W, (cuuint32_t)TH, 1};
         const cuuint32_t estr[3] = {1, 1, 1};
-        CUresult r = ctx->encode(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(a.score), dims, strides,
-                                 box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                                 CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-        if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
-        constexpr int NW = nms_warps(R);
+        if (ctx->encode(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(a.score), dims, strides, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+            return cudaErrorInvalidValue;
         int grid = ctx->num_sms * ctx->nms_ctas_per_sm[R];
-        if (grid > (total + NW - 1) / NW) grid = (total + NW - 1) / NW;
-        k_nms_tma<R><<<grid, NW * 32, nms_smem_bytes(R), st>>>(tmap, a.H, a.W, strips_x, tiles_y, total, thr_up,
-                                                                ctx->cand, ctx->tile_cnt);
+        if (grid > (p.units + NMS_WARPS - 1) / NMS_WARPS) grid = (p.units + NMS_WARPS - 1) / NMS_WARPS;
+        if (p.thr_up > 0.0f)
+            k_nms_tma<R, false><<<grid, NMS_WARPS * 32, NMS_SMEM_BYTES, st>>>(tmap, p, a.score, ctx->cand, ctx->tile_cnt);
+        else                                                 // a -0.0 score may be a candidate: fold it onto +0
+            k_nms_tma<R, true><<<grid, NMS_WARPS * 32, NMS_SMEM_BYTES, st>>>(tmap, p, a.score, ctx->cand, ctx->tile_cnt);
     } else {
-        k_nms_plain<R><<<(total + PLAIN_WARPS - 1) / PLAIN_WARPS, PLAIN_WARPS * 32, 0, st>>>(
-            a.score, a.H, a.W, strips_x, tiles_y, total, thr_up, ctx->cand, ctx->tile_cnt);
+        const int total = p.strips_x * p.chunks_y * a.B;
+        k_nms_plain<R><<<(total + PLAIN_WARPS - 1) / PLAIN_WARPS, PLAIN_WARPS * 32, 0, st>>>(a.score, p, total, ctx->cand,
+                                                                                             ctx->tile_cnt);
     }
     return cudaGetLastError();
 }
@@ -185,16 +211,16 @@ cudaError_t launch_rg(const ExtractArgs& a, const int32_t* sel, cudaStream_t st)
 // prof: measurement mode, an event on `st` before and after every kernel.
 cudaError_t enqueue(dkd_ctx* ctx, const ExtractArgs& a, cudaStream_t st, bool prof = false) {
     const int tiles_x = (a.W + STRIP_W - 1) / STRIP_W, tiles_y = (a.H + TH - 1) / TH;
-    const int tpi = tiles_x * tiles_y, total = tpi * a.B;
+    const int tpi = tiles_x * tiles_y;                      // strip-tiles (candidate segments) per image
     cudaError_t e;
     int nk = 0;
     auto mark = [&]() { return prof ? cudaEventRecord(ctx->prof_ev[nk++], st) : cudaSuccess; };
     if ((e = mark()) != cudaSuccess) return e;
     switch (a.r) {
-        case 1: e = launch_nms<1>(ctx, a, tiles_x, tiles_y, total, st); break;
-        case 2: e = launch_nms<2>(ctx, a, tiles_x, tiles_y, total, st); break;
-        case 3: e = launch_nms<3>(ctx, a, tiles_x, tiles_y, total, st); break;
-        default: e = launch_nms<4>(ctx, a, tiles_x, tiles_y, total, st); break;
+        case 1: e = launch_nms<1>(ctx, a, st); break;
+        case 2: e = launch_nms<2>(ctx, a, st); break;
+        case 3: e = launch_nms<3>(ctx, a, st); break;
+        default: e = launch_nms<4>(ctx, a, st); break;
     }
     if (e != cudaSuccess) return e;
     if ((e = mark()) != cudaSuccess) return e;

@@ -20,26 +20,29 @@
 namespace dkd {
 
 // ---- geometry -------------------------------------------------------------------------------
-// Unit of NMS work = one STRIP-TILE: STRIP_W x TH output pixels, owned by ONE warp.  Its halo'd
-// input box is BOX_W x (TH + 2R) floats: 4 halo columns each side (>= max radius, keeps every lane's
-// float4 16-byte aligned) and R halo rows above and below.  Lane l owns box columns 4l..4l+3; lanes
-// 0 and 31 hold only halo columns, lanes 1..30 produce the 120 output columns.
+// NMS work is cut into STRIP-TILES of STRIP_W x TH output pixels (one candidate segment each).  A
+// warp owns a UNIT = up to MAX_CPU vertically consecutive strip-tiles of one strip and walks down it
+// keeping the last 2R rows in registers, so the R halo rows above a strip-tile are fetched only once
+// per unit.  Shared-memory boxes are BOX_W = 128 floats wide: 4 halo columns each side (>= max
+// radius, keeps every lane's float4 16-byte aligned) — one 512-byte row per image row.  Lane l owns
+// box columns 4l..4l+3; lanes 0 and 31 hold only halo columns, lanes 1..30 produce the 120 outputs.
 constexpr int STRIP_W = 120;             // output columns per strip
 constexpr int BOX_W = 128;               // box columns = one 512-byte shared-memory row (32 lanes x float4)
 constexpr int HALO_X = 4;
-constexpr int TH = 16;                   // output rows per strip-tile
-constexpr int SEG_CAP = STRIP_W * TH;    // 1920 = worst-case candidates of a strip-tile = segment capacity
+constexpr int TH = 8;                    // output rows per strip-tile = rows of one TMA box
+constexpr int SEG_CAP = STRIP_W * TH;    // 960 = worst-case candidates of a strip-tile = segment capacity
 constexpr int MAX_R = 4;
-constexpr int NMS_STAGES = 2;            // TMA boxes in flight / in use per warp
+constexpr int MAX_CPU = 8;               // strip-tiles (chunks) per unit, chosen per call (nms_plan)
 constexpr int SEL_THREADS = 1024;
 constexpr int SORT_CAP = 8192;           // keys ordered in shared memory by k_select
 constexpr int RG_THREADS = 256;          // k_refine_gather: 8 warps, 8..32 keypoints per CTA
 
-__host__ __device__ constexpr int box_rows(int R) { return TH + 2 * R; }
-__host__ __device__ constexpr int box_bytes(int R) { return BOX_W * box_rows(R) * 4; }     // multiple of 512
-// warps per CTA: 2 CTAs/SM must fit 227 KB of shared memory (R <= 3: 5 warps, 10 KB..11.3 KB boxes)
-__host__ __device__ constexpr int nms_warps(int R) { return R <= 3 ? 5 : 4; }
-__host__ __device__ constexpr int nms_smem_bytes(int R) { return nms_warps(R) * NMS_STAGES * box_bytes(R); }
+constexpr int BOX_BYTES = BOX_W * TH * 4;                                                // 4 KB
+// Every resident warp keeps NMS_STAGES-1 boxes in flight while it works on one: bytes in flight per
+// SM >= 2 CTAs x warps x (stages-1) x 4 KB = 128 KB (HBM latency x bandwidth needs ~50 KB per SM).
+constexpr int NMS_WARPS = 8;             // per CTA, 2 CTAs/SM: 16 warps x <= 128 registers
+constexpr int NMS_STAGES = 3;
+constexpr int NMS_SMEM_BYTES = NMS_WARPS * NMS_STAGES * BOX_BYTES;                        // 96 KB per CTA
 
 // ---- 64-bit selection key ---------------------------------------------------------------------
 // key = (orderable(score bits) << 32) | ~idx : a larger key is a better candidate, i.e. descending
@@ -99,54 +102,36 @@ __device__ __forceinline__ float fmax3(float a, float b, float c) {
     return d;
 }
 
-// ---- step a1 + a1': one halo'd strip-tile in shared memory -> candidate keys -------------------------
-// box: smem, box_rows(R) x BOX_W floats; box[q * BOX_W + j] is pixel (x0 - HALO_X + j, y0 - R + q).
-// Pixels outside the image read 0 (never used: a kept pixel's window is inside the image, G3).
+// ---- step a1: TH new rows of one strip -> candidate bit mask ----------------------------------------
+// cat[q] = image row yc-R+q of this lane's 4 columns, q = 0 .. TH+2R-1 (registers): output row yc+o
+// needs cat[o] .. cat[o+2R], its centre is cat[o+R].  Pixels outside the image read 0 (never used: a
+// kept pixel's window is inside the image, G3).
 //
-// Separable window maximum, the same ~8 instructions per pixel on any input (no data-dependent
-// divergence): every lane walks down its 4 columns keeping the last 2R+1 rows in registers
-// (vertical max, 2 FMNMX3 per column for r = 2), takes the neighbouring lanes' column maxima by
-// shuffle (2R SHFL per row) and forms the horizontal max with the threshold folded in:
+// Separable window maximum, the same ~9 instructions per pixel on any input (no data-dependent
+// divergence): vertical max of the 2R+1 rows per column from registers (2 FMNMX3 per column for
+// r = 2), the neighbouring lanes' column maxima by shuffle (2R SHFL per row), and the horizontal max
+// with the threshold folded in:
 //     m_k = max( max over the (2r+1)^2 window of pixel k ,  thr_up ),  thr_up = nextafter(thresh, +inf)
-// so that   S > thresh  AND  S >= every window value   <=>   S == m_k   <=>   S - m_k >= 0
-// (S <= m_k always; the subtraction of two different finite floats is never 0; -0/+0 compare equal).
-// The per-pixel test therefore costs 4 FADD + 2 FMNMX + 1 FSETP per lane-row; the exact mask, the
-// ballot compaction and the key stores run only in the rare warp-rows that hold a candidate.
-// Candidates are appended (unordered) to the strip-tile's private global segment `seg`
-// (capacity SEG_CAP); the running count lives in a warp-uniform register (no atomics).
-template <int R>
-__device__ __forceinline__ int process_strip(const float* __restrict__ box, int x0, int y0, int H, int W,
-                                             float thr_up, uint64_t* __restrict__ seg) {
+// so that   S > thresh  AND  S >= every window value   <=>   S == m_k   <=>   S - m_k = +0
+// (S <= m_k always; the difference of two different finite floats is never 0; S + 0.0f folds -0 onto
+// +0; needed only when thr_up <= 0, i.e. NEGT).  neg[k] collects, for pixel column k, the sign bit of
+// S - m_k of output rows 0..TH-1 in bits TH-1..0 (one funnel shift per pixel): a 0 bit = candidate.
+// The body is branch-free and fully unrolled.
+template <int R, bool NEGT>
+__device__ __forceinline__ void nms_rows(const float4 (&cat)[TH + 2 * R], float thr_up, unsigned (&neg)[4]) {
     constexpr int N = 2 * R + 1;
     constexpr unsigned FULL = 0xffffffffu;
-    const int lane = threadIdx.x & 31;
-    const int X = x0 - HALO_X + 4 * lane;                    // image column of this lane's first pixel
-    unsigned colmask = 0;                                    // output columns this lane may emit
-    if (lane >= 1 && lane <= 30) {
-#pragma unroll
-        for (int k = 0; k < 4; ++k)
-            if (X + k >= R && X + k < W - R) colmask |= 1u << k;
-    }
-    const float4* src = reinterpret_cast<const float4*>(box) + lane;   // row pitch = 32 float4
-    float4 ring[N];
-#pragma unroll
-    for (int q = 0; q < 2 * R; ++q) ring[q] = src[q * 32];
-    // neg[h]: nibble o&7 of word o>>3 holds, for output row o, one bit per pixel k that is NOT a candidate
-    // (sign bit of S - m_k).  The 16-row body is branch-free, so the rows interleave freely.
-    unsigned neg[TH / 8];
-#pragma unroll
-    for (int h = 0; h < TH / 8; ++h) neg[h] = 0u;
+    static_assert(TH == 8, "8 rows per mask byte");
+    neg[0] = neg[1] = neg[2] = neg[3] = 0u;
 #pragma unroll
     for (int o = 0; o < TH; ++o) {
-        ring[(o + 2 * R) % N] = src[(o + 2 * R) * 32];
-        // vertical max of the 2R+1 rows, per column
-        float4 vm = ring[0];
+        float4 vm = cat[o];                                  // vertical max of the 2R+1 rows, per column
 #pragma unroll
         for (int q = 1; q + 1 < N; q += 2) {
-            vm.x = fmax3(vm.x, ring[q].x, ring[q + 1].x);
-            vm.y = fmax3(vm.y, ring[q].y, ring[q + 1].y);
-            vm.z = fmax3(vm.z, ring[q].z, ring[q + 1].z);
-            vm.w = fmax3(vm.w, ring[q].w, ring[q + 1].w);
+            vm.x = fmax3(vm.x, cat[o + q].x, cat[o + q + 1].x);
+            vm.y = fmax3(vm.y, cat[o + q].y, cat[o + q + 1].y);
+            vm.z = fmax3(vm.z, cat[o + q].z, cat[o + q + 1].z);
+            vm.w = fmax3(vm.w, cat[o + q].w, cat[o + q + 1].w);
         }
         // neighbours' column maxima: l[j] = column X-1-j, rt[j] = column X+4+j
         float l[R], rt[R];
@@ -193,139 +178,233 @@ __device__ __forceinline__ int process_strip(const float* __restrict__ box, int 
             m3 = fmaxf(core, rp[R - 1]);
             if constexpr (R == 4) m0 = fmaxf(m0, rp[0]), m3 = fmaxf(m3, lp[0]);
         }
-        // S - m_k: +0 for a candidate, negative otherwise (S + 0.0f folds -0 onto +0 first)
-        const float4 c = ring[(o + R) % N];                  // centre row
-        const unsigned s0 = __float_as_uint((c.x + 0.0f) - m0) >> 31, s1 = __float_as_uint((c.y + 0.0f) - m1) >> 31;
-        const unsigned s2 = __float_as_uint((c.z + 0.0f) - m2) >> 31, s3 = __float_as_uint((c.w + 0.0f) - m3) >> 31;
-        neg[o >> 3] |= (s0 | (s1 << 1) | (s2 << 2) | (s3 << 3)) << (4 * (o & 7));
+        // S - m_k: +0 for a candidate, negative otherwise
+        float4 c = cat[o + R];                               // centre row
+        if constexpr (NEGT) c = make_float4(c.x + 0.0f, c.y + 0.0f, c.z + 0.0f, c.w + 0.0f);
+        neg[0] = __funnelshift_l(__float_as_uint(c.x - m0), neg[0], 1);
+        neg[1] = __funnelshift_l(__float_as_uint(c.y - m1), neg[1], 1);
+        neg[2] = __funnelshift_l(__float_as_uint(c.z - m2), neg[2], 1);
+        neg[3] = __funnelshift_l(__float_as_uint(c.w - m3), neg[3], 1);
     }
-    // candidate bits of this lane: valid rows (R <= y < H-R) x valid columns, not negative
-    unsigned cm[TH / 8];
-    int n = 0;
-    {
-        const int o_lo = R - y0 > 0 ? R - y0 : 0;            // first valid output row
-        const int o_hi = H - R - y0 < TH ? H - R - y0 : TH;  // one past the last valid output row
-#pragma unroll
-        for (int h = 0; h < TH / 8; ++h) {
-            int a = o_lo - 8 * h, b = o_hi - 8 * h;          // valid rows of this word: [a, b) clipped to [0, 8]
-            a = a < 0 ? 0 : (a > 8 ? 8 : a);
-            b = b < 0 ? 0 : (b > 8 ? 8 : b);
-            const unsigned rows = b > a ? static_cast<unsigned>(((1ull << (4 * b)) - 1ull) & ~((1ull << (4 * a)) - 1ull)) : 0u;
-            cm[h] = ~neg[h] & rows & (colmask * 0x11111111u);
-            n += __popc(cm[h]);
-        }
-    }
-    if (!__any_sync(FULL, n != 0)) return 0;
-    int incl = n;                                            // warp inclusive scan of the per-lane counts
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        const int up = __shfl_up_sync(FULL, incl, d);
-        if (lane >= d) incl += up;
-    }
-    const int total = __shfl_sync(FULL, incl, 31);
-    int pos = incl - n;
-#pragma unroll
-    for (int h = 0; h < TH / 8; ++h) {
-        unsigned bits = cm[h];
-        while (bits) {                                       // rare: a few set bits per strip-tile
-            const int bit = __ffs(bits) - 1;
-            bits &= bits - 1;
-            const int o = 8 * h + (bit >> 2), k = bit & 3;
-            const float v = box[(o + R) * BOX_W + 4 * lane + k];
-            seg[pos++] = make_key(v, (y0 + o) * W + X + k);
-        }
-    }
-    return total;
 }
 
-// strip-tile index -> (image, tile row, strip)
-__device__ __forceinline__ void tile_coords(int t, int strips_x, int tiles_y, int& b, int& y0, int& x0) {
-    const int spi = strips_x * tiles_y;
-    b = t / spi;
-    const int rem = t - b * spi;
-    const int ty = rem / strips_x;
-    x0 = (rem - ty * strips_x) * STRIP_W;
-    y0 = ty * TH;
-}
-
-// ---- k_nms_tma: persistent; every warp runs its own NMS_STAGES-deep TMA/mbarrier pipeline ------------
-// grid = min(ceil(total / warps), CTAs that fit); warp g handles strip-tiles g, g + G, ... (image-major,
-// row-major, strips fastest: neighbouring warps load neighbouring boxes, so halo re-reads hit L2).
-// No CTA-wide barrier after set-up: a warp only ever waits for its own box.
-// Dynamic smem: nms_smem_bytes(R), 128-byte aligned; box of (warp w, stage s) at (w*NMS_STAGES+s)*box_bytes.
+// ---- step a1': candidate masks of one strip-tile -> keys in its private segment --------------------
+// Row validity (R <= y < H-R) and column validity (colmask, one bit per owned column that may emit)
+// are applied here.  Candidates are rare (a few per strip-tile): every round, each lane that still
+// holds one appends its next candidate at a ballot-ranked slot; the running count is warp-uniform
+// (no atomics, no shared counter).  The score of a candidate is re-read from the box `rows` (output
+// row o >= R has its centre in box row o - R) or, for the first R rows, from the rows still in
+// registers.  Returns the segment's count.
 template <int R>
-__global__ void __launch_bounds__(nms_warps(R) * 32, 2) k_nms_tma(const __grid_constant__ CUtensorMap tmap, int H,
-                                                                  int W, int strips_x, int tiles_y, int total,
-                                                                  float thr_up, uint64_t* __restrict__ cand,
-                                                                  int* __restrict__ tile_cnt) {
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    __shared__ __align__(8) uint64_t full_bar[nms_warps(R) * NMS_STAGES];
-    constexpr int NW = nms_warps(R);
-    constexpr int BB = box_bytes(R);
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int first = blockIdx.x * NW + warp, step = gridDim.x * NW;
-    const int n_my = first < total ? (total - first + step - 1) / step : 0;
-    unsigned char* my_smem = smem_raw + warp * NMS_STAGES * BB;
-    uint64_t* my_bar = full_bar + warp * NMS_STAGES;
+__device__ __forceinline__ int nms_emit(const unsigned (&neg)[4], unsigned colmask, int X, int yc, int H, int W,
+                                        const float4 (&cat)[TH + 2 * R], const float* __restrict__ rows,
+                                        uint64_t* __restrict__ seg) {
+    constexpr unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    unsigned rowmask = 0xffu;                                // bit TH-1-o = output row o is valid
+    if (yc < R || yc + TH > H - R) {                         // warp-uniform: first / last strip-tiles only
+        int a = R - yc, b = H - R - yc;                      // valid output rows [a, b) clipped to [0, TH]
+        a = a < 0 ? 0 : (a > TH ? TH : a);
+        b = b < 0 ? 0 : (b > TH ? TH : b);
+        rowmask = b > a ? ((1u << (TH - a)) - 1u) & ~((1u << (TH - b)) - 1u) : 0u;
+    }
+    unsigned w = 0u;                                         // bit 8k + (TH-1-o): pixel k of output row o is a candidate
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+        if ((colmask >> k) & 1u) w |= (~neg[k] & rowmask) << (8 * k);
+    int cnt = 0;
+    unsigned bal = __ballot_sync(FULL, w != 0u);
+    while (bal) {                                            // warp-uniform; usually one round
+        if (w != 0u) {
+            const int bit = __ffs(w) - 1;
+            w &= w - 1u;
+            const int k = bit >> 3, o = TH - 1 - (bit & 7);
+            float v;
+            if (o >= R) {
+                v = rows[(o - R) * BOX_W + 4 * lane + k];
+            } else {
+                float4 tr = cat[R];
+#pragma unroll
+                for (int j = 1; j < R; ++j)
+                    if (o == j) tr = cat[R + j];
+                v = k == 0 ? tr.x : (k == 1 ? tr.y : (k == 2 ? tr.z : tr.w));
+            }
+            seg[cnt + __popc(bal & ((1u << lane) - 1u))] = make_key(v, (yc + o) * W + X + k);
+        }
+        cnt += __popc(bal);
+        bal = __ballot_sync(FULL, w != 0u);
+    }
+    return cnt;
+}
 
-    auto issue = [&](int it) {                               // lane 0 only
-        int b, y0, x0;
-        tile_coords(first + it * step, strips_x, tiles_y, b, y0, x0);
-        const int s = it % NMS_STAGES;
-        mbar_arrive_expect_tx(&my_bar[s], BB);
-        tma_load_tile(my_smem + s * BB, &tmap, &my_bar[s], x0 - HALO_X, y0 - R, b);
+__device__ __forceinline__ unsigned strip_colmask(int X, int W, int R) {
+    const int lane = threadIdx.x & 31;
+    unsigned colmask = 0;                                    // output columns this lane may emit
+    if (lane >= 1 && lane <= 30) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+            if (X + k >= R && X + k < W - R) colmask |= 1u << k;
+    }
+    return colmask;
+}
+
+// ---- work decomposition (host: nms_plan) -----------------------------------------------------------
+// strip-tile index t = (b * chunks_y + cy) * strips_x + sx  (segment t of `cand`, tile_cnt[t]).
+// unit u = (b * segs + sg) * strips_x + sx  covers strip-tiles cy = sg*cpu .. min(sg*cpu + cpu, chunks_y) - 1.
+struct NmsPlan {
+    int H, W;
+    int strips_x, chunks_y;  // strip-tiles per image row / column
+    int cpu, segs;           // strip-tiles per unit, units per strip
+    int units;               // strips_x * segs * B
+    float thr_up;            // nextafter(thresh, +inf)
+};
+struct UnitCoords {
+    int b, x0, y0, nch, t0;  // image, first output column / row, strip-tiles in the unit, first strip-tile index
+};
+__device__ __forceinline__ UnitCoords unit_coords(int u, const NmsPlan& p) {
+    const int upi = p.strips_x * p.segs;
+    UnitCoords c;
+    c.b = u / upi;
+    const int rem = u - c.b * upi;
+    const int sg = rem / p.strips_x, sx = rem - sg * p.strips_x;
+    c.x0 = sx * STRIP_W;
+    c.y0 = sg * p.cpu * TH;
+    c.nch = p.chunks_y - sg * p.cpu < p.cpu ? p.chunks_y - sg * p.cpu : p.cpu;
+    c.t0 = (c.b * p.chunks_y + sg * p.cpu) * p.strips_x + sx;
+    return c;
+}
+
+// the 2R rows above a unit (image rows y0-R .. y0+R-1), one float4 per lane and row, straight from
+// global memory (once per unit; mostly L2 hits: the unit above has just streamed them); 0 outside the image
+template <int R>
+__device__ __forceinline__ void load_head(float4 (&cat)[TH + 2 * R], const float* __restrict__ img, int X, int y0,
+                                          int H, int W) {
+#pragma unroll
+    for (int q = 0; q < 2 * R; ++q) {
+        const int y = y0 - R + q;
+        cat[q] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+        if (y >= 0 && y < H && X >= 0 && X < W)              // W % 4 == 0 and X % 4 == 0: all four or none
+            cat[q] = __ldg(reinterpret_cast<const float4*>(img + static_cast<size_t>(y) * W + X));
+    }
+}
+
+// ---- k_nms_tma: persistent; every warp runs its own TMA/mbarrier pipeline ---------------------------
+// grid = min(ceil(units / warps), CTAs that fit); warp g handles units g, g + G, ... (image-major,
+// segment-major, strips fastest: neighbouring warps load neighbouring boxes, so the 4 halo columns hit L2).
+// Per strip-tile one TMA box of TH rows (image rows yc+R .. yc+R+TH-1, the newest rows its outputs
+// need) through a NMS_STAGES-deep ring: while a warp works on one box (8 LDS.128 into registers, the
+// arithmetic, the candidate scores picked out of the box), its other NMS_STAGES-1 boxes stay in flight.
+// No CTA-wide barrier after set-up: a warp only ever waits for its own boxes.  Dynamic smem:
+// NMS_SMEM_BYTES, 128-byte aligned; warp w owns NMS_STAGES boxes.  NEGT: thr_up <= 0 (see nms_rows).
+template <int R, bool NEGT>
+__global__ void __launch_bounds__(NMS_WARPS * 32, 2) k_nms_tma(const __grid_constant__ CUtensorMap tmap,
+                                                               const __grid_constant__ NmsPlan p,
+                                                               const float* __restrict__ score,
+                                                               uint64_t* __restrict__ cand,
+                                                               int* __restrict__ tile_cnt) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ __align__(8) uint64_t bars[NMS_WARPS * NMS_STAGES];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int first = blockIdx.x * NMS_WARPS + warp, step = gridDim.x * NMS_WARPS;
+    const int n_my = first < p.units ? (p.units - first + step - 1) / step : 0;
+    if (n_my == 0) return;
+    unsigned char* my_smem = smem_raw + warp * NMS_STAGES * BOX_BYTES;
+    uint64_t* bar = bars + warp * NMS_STAGES;
+
+    // issue side (every lane tracks the cursor, lane 0 issues): next box = chunk ic of unit iteration iit
+    int iit = 0, ic = 0, issued = 0;
+    UnitCoords iu = unit_coords(first, p);
+    auto issue_box = [&]() {
+        if (iit >= n_my) return;
+        const int s = issued % NMS_STAGES;
+        if (lane == 0) {
+            mbar_arrive_expect_tx(&bar[s], BOX_BYTES);
+            tma_load_tile(my_smem + s * BOX_BYTES, &tmap, &bar[s], iu.x0 - HALO_X, iu.y0 + R + TH * ic, iu.b);
+        }
+        ++issued;
+        if (++ic == iu.nch) {
+            ic = 0;
+            if (++iit < n_my) iu = unit_coords(first + iit * step, p);
+        }
     };
 
+    UnitCoords cu = iu;
     if (lane == 0) {
-        if (warp == 0) tma_prefetch_desc(&tmap);
+        tma_prefetch_desc(&tmap);
 #pragma unroll
-        for (int s = 0; s < NMS_STAGES; ++s) mbar_init(&my_bar[s], 1);
+        for (int s = 0; s < NMS_STAGES; ++s) mbar_init(&bar[s], 1);
         fence_mbar_init();
-        const int pre = n_my < NMS_STAGES ? n_my : NMS_STAGES;
-        for (int it = 0; it < pre; ++it) issue(it);
     }
     __syncwarp();
+#pragma unroll
+    for (int s = 0; s < NMS_STAGES; ++s) issue_box();
+
+    int consumed = 0;
     for (int it = 0; it < n_my; ++it) {
-        const int t = first + it * step;
-        int b, y0, x0;
-        tile_coords(t, strips_x, tiles_y, b, y0, x0);
-        const int s = it % NMS_STAGES;
-        mbar_wait(&my_bar[s], (it / NMS_STAGES) & 1);
-        const int cnt = process_strip<R>(reinterpret_cast<const float*>(my_smem + s * BB), x0, y0, H, W, thr_up,
-                                         cand + static_cast<size_t>(t) * SEG_CAP);
-        __syncwarp();                                        // every lane is done reading stage s
-        if (lane == 0) {
-            tile_cnt[t] = cnt;
-            if (it + NMS_STAGES < n_my) issue(it + NMS_STAGES);
+        const int X = cu.x0 - HALO_X + 4 * lane;             // image column of this lane's first pixel
+        float4 cat[TH + 2 * R];                              // rows yc-R .. yc+R+TH-1 of the current strip-tile
+        load_head<R>(cat, score + static_cast<size_t>(cu.b) * p.H * p.W, X, cu.y0, p.H, p.W);
+        const unsigned colmask = strip_colmask(X, p.W, R);
+        for (int c = 0; c < cu.nch; ++c) {
+            const int s = consumed % NMS_STAGES;
+            mbar_wait(&bar[s], (consumed / NMS_STAGES) & 1);
+            const float* rows = reinterpret_cast<const float*>(my_smem + s * BOX_BYTES);
+            {
+                const float4* src = reinterpret_cast<const float4*>(rows) + lane;
+#pragma unroll
+                for (int o = 0; o < TH; ++o) cat[2 * R + o] = src[o * 32];
+            }
+            unsigned neg[4];
+            nms_rows<R, NEGT>(cat, p.thr_up, neg);
+            const int t = cu.t0 + c * p.strips_x;
+            const int cnt = nms_emit<R>(neg, colmask, X, cu.y0 + TH * c, p.H, p.W, cat, rows,
+                                        cand + static_cast<size_t>(t) * SEG_CAP);
+            __syncwarp();                                    // every lane is done with stage s
+            issue_box();                                     // (the other NMS_STAGES-1 boxes stay in flight meanwhile)
+            ++consumed;
+            if (lane == 0) tile_cnt[t] = cnt;
+#pragma unroll
+            for (int q = 0; q < 2 * R; ++q) cat[q] = cat[TH + q];   // the 2R rows above the next strip-tile
         }
+        if (it + 1 < n_my) cu = unit_coords(first + (it + 1) * step, p);
     }
 }
 
-// ---- k_nms_plain: same strip math, box staged with ordinary loads (any W, any alignment) ------------
+// ---- k_nms_plain: same strip math, one strip-tile per warp, rows fetched with ordinary loads ---------
+// (any W, any alignment: scalar loads, 0 outside the image)
 constexpr int PLAIN_WARPS = 4;
 template <int R>
-__global__ void __launch_bounds__(PLAIN_WARPS * 32) k_nms_plain(const float* __restrict__ score, int H, int W,
-                                                                int strips_x, int tiles_y, int total, float thr_up,
+__global__ void __launch_bounds__(PLAIN_WARPS * 32) k_nms_plain(const float* __restrict__ score,
+                                                                const __grid_constant__ NmsPlan p, int total,
                                                                 uint64_t* __restrict__ cand,
                                                                 int* __restrict__ tile_cnt) {
-    __shared__ __align__(16) float boxes[PLAIN_WARPS][BOX_W * box_rows(R)];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int t = blockIdx.x * PLAIN_WARPS + warp;
     if (t >= total) return;
-    int b, y0, x0;
-    tile_coords(t, strips_x, tiles_y, b, y0, x0);
-    const float* img = score + static_cast<size_t>(b) * H * W;
-    float* box = boxes[warp];
-    for (int q = 0; q < box_rows(R); ++q) {
-        const int gy = y0 - R + q;
+    const int tpi = p.strips_x * p.chunks_y;
+    const int b = t / tpi, rem = t - b * tpi;
+    const int cy = rem / p.strips_x, x0 = (rem - cy * p.strips_x) * STRIP_W, y0 = cy * TH;
+    const float* img = score + static_cast<size_t>(b) * p.H * p.W;
+    const int X = x0 - HALO_X + 4 * lane;
+    float4 cat[TH + 2 * R];
 #pragma unroll
-        for (int j = lane; j < BOX_W; j += 32) {
-            const int gx = x0 - HALO_X + j;
-            box[q * BOX_W + j] = (gy >= 0 && gy < H && gx >= 0 && gx < W) ? __ldg(img + static_cast<size_t>(gy) * W + gx) : 0.0f;
-        }
+    for (int q = 0; q < TH + 2 * R; ++q) {
+        const int gy = y0 - R + q;
+        float v[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+            v[k] = (gy >= 0 && gy < p.H && X + k >= 0 && X + k < p.W) ? __ldg(img + static_cast<size_t>(gy) * p.W + X + k) : 0.0f;
+        cat[q] = make_float4(v[0], v[1], v[2], v[3]);
     }
+    __shared__ __align__(16) float boxes[PLAIN_WARPS][BOX_W * TH];
+    float4* box = reinterpret_cast<float4*>(boxes[warp]) + lane;
+#pragma unroll
+    for (int o = 0; o < TH; ++o) box[o * 32] = cat[2 * R + o];
     __syncwarp();
-    const int cnt = process_strip<R>(box, x0, y0, H, W, thr_up, cand + static_cast<size_t>(t) * SEG_CAP);
+    unsigned neg[4];
+    nms_rows<R, true>(cat, p.thr_up, neg);
+    const int cnt = nms_emit<R>(neg, strip_colmask(X, p.W, R), X, y0, p.H, p.W, cat, boxes[warp],
+                                cand + static_cast<size_t>(t) * SEG_CAP);
     if (lane == 0) tile_cnt[t] = cnt;
 }
 
@@ -561,7 +640,14 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
             const int d = (hi - static_cast<unsigned>(k >> 32)) >> shift;
             const int s0 = base[d], s1 = s0 + cur[d];
             int rank = s0;
-            for (int j = s0; j < s1; ++j) rank += sorted[j] > k ? 1 : 0;
+            int j = s0;
+            for (; j + 8 <= s1; j += 8) {                    // 8 independent loads in flight (tie clusters:
+                int r8 = 0;                                  //  the clamp at 1.0 puts hundreds of keys in one bucket)
+#pragma unroll
+                for (int u = 0; u < 8; ++u) r8 += sorted[j + u] > k ? 1 : 0;
+                rank += r8;
+            }
+            for (; j < s1; ++j) rank += sorted[j] > k ? 1 : 0;
             if (rank < K) out[rank] = key_index(k);
         }
         return;
@@ -714,7 +800,6 @@ __global__ void __launch_bounds__(RG_THREADS) k_refine_gather(const __grid_const
     const int b = blockIdx.y;
     const size_t slot = static_cast<size_t>(b) * p.top_k + i_img;
     const int idx = __ldg(p.sel_idx + slot);
-    constexpr int ESZ = (DT == DKD_F16) ? 2 : 4;
 
     if (idx < 0) {                                          // step a5: zero padding
         if (gl < 2) p.out_kpts[2 * slot + gl] = 0.0f;
