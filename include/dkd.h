@@ -53,8 +53,14 @@ enum {
                                 Ignored (plain launches) while `stream` is being captured by the caller. */
     DKD_OPT_USE_TMA   = 1,   /* [1] NMS tiles staged by TMA (cp.async.bulk.tensor) when W % 4 == 0 and
                                 score is 16-byte aligned; 0 = always the plain-load tile loader. */
-    DKD_OPT_PROFILE   = 2    /* [0] 1 = measurement mode: plain launches (no graph) with a CUDA event recorded
+    DKD_OPT_PROFILE   = 2,   /* [0] 1 = measurement mode: plain launches (no graph) with a CUDA event recorded
                                 on `stream` before and after every kernel; read with dkd_profile_read. */
+    DKD_OPT_USE_PDL   = 3,   /* [1] the select and refine/gather kernels are launched with programmatic
+                                stream serialization (they start while their predecessor drains and wait
+                                on-device for its results): hides the launch latency between the kernels. */
+    DKD_OPT_NMS_UNIT  = 4    /* [0] strip-tiles (8 output rows each) a warp of the NMS kernel walks down before it
+                                moves to another strip: 0 = chosen per call from the problem size, 1..8 = forced
+                                (tuning / test knob; results do not depend on it). */
 };
 
 typedef struct {

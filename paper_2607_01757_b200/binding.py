@@ -10,7 +10,7 @@ import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 F32, F16 = 0, 1
-OPT_USE_GRAPH, OPT_USE_TMA, OPT_PROFILE = 0, 1, 2
+OPT_USE_GRAPH, OPT_USE_TMA, OPT_PROFILE, OPT_USE_PDL, OPT_NMS_UNIT = 0, 1, 2, 3, 4
 MAX_RADIUS, MAX_TOP_K, MAX_ROW_BYTES = 4, 8192, 2048
 
 EXPORTED_SYMBOLS = (

@@ -5,7 +5,6 @@
 #include <math.h>
 #include <stdio.h>
 #include <string.h>
-#include <stdlib.h>
 
 #include <vector>
 
@@ -68,7 +67,7 @@ struct dkd_ctx {
     void* st_out;   size_t st_out_bytes;
     const void* st_desc_src; size_t st_desc_src_bytes;      // what st_desc currently holds
     // options
-    int use_graph, use_tma, profile;
+    int use_graph, use_tma, use_pdl, profile, nms_cpu;
     cudaEvent_t prof_ev[MAX_KERNELS + 1];                   // measurement mode: event before/after every kernel
     int prof_n;                                             // kernels of the last profiled call (0: none)
     std::vector<GraphEntry> graphs;
@@ -120,7 +119,7 @@ NmsPlan nms_plan(const dkd_ctx* ctx, const ExtractArgs& a) {
         const int segs = (p.chunks_y + cpu - 1) / cpu;
         if (static_cast<long long>(p.strips_x) * segs * a.B >= 4 * slots) { best = cpu; break; }
     }
-    if (getenv("DKD_CPU")) best = atoi(getenv("DKD_CPU"));
+    if (ctx->nms_cpu > 0) best = ctx->nms_cpu < MAX_CPU ? ctx->nms_cpu : MAX_CPU;
     p.cpu = best;
     p.segs = (p.chunks_y + best - 1) / best;
     p.units = p.strips_x * p.segs * a.B;
@@ -174,21 +173,37 @@ SampleAxis make_axis(int stride, int n) {
     return a;
 }
 
+// Launch with (pdl) or without the programmatic-stream-serialization attribute: with it the kernel may be
+// scheduled while its predecessor in the stream still runs (it calls griddepcontrol.wait before it reads
+// the predecessor's results), which hides the launch latency between the three kernels of an extract.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, bool pdl,
+                       Args... args) {
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr;
+    attr.id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr.val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = &attr;
+    cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+
 template <int DT, int G>
-cudaError_t launch_rg_g(const RGParams& p, int B, cudaStream_t st) {
+cudaError_t launch_rg_g(const RGParams& p, int B, cudaStream_t st, bool pdl) {
     const dim3 grid((p.top_k + RG_THREADS / G - 1) / (RG_THREADS / G), B);
-    k_refine_gather<DT, G><<<grid, RG_THREADS, 0, st>>>(p);
-    return cudaGetLastError();
+    return launch_pdl(k_refine_gather<DT, G>, grid, dim3(RG_THREADS), 0, st, pdl, p);
 }
 
 template <int DT>
-cudaError_t launch_rg_dt(const RGParams& p, int B, cudaStream_t st) {
-    if (p.nchunk <= 8) return launch_rg_g<DT, 8>(p, B, st);
-    if (p.nchunk <= 16) return launch_rg_g<DT, 16>(p, B, st);
-    return launch_rg_g<DT, 32>(p, B, st);
+cudaError_t launch_rg_dt(const RGParams& p, int B, cudaStream_t st, bool pdl) {
+    if (p.nchunk <= 8) return launch_rg_g<DT, 8>(p, B, st, pdl);
+    if (p.nchunk <= 16) return launch_rg_g<DT, 16>(p, B, st, pdl);
+    return launch_rg_g<DT, 32>(p, B, st, pdl);
 }
 
-cudaError_t launch_rg(const ExtractArgs& a, const int32_t* sel, cudaStream_t st) {
+cudaError_t launch_rg(const ExtractArgs& a, const int32_t* sel, cudaStream_t st, bool pdl) {
     RGParams p;
     memset(&p, 0, sizeof(p));
     p.score = a.score; p.H = a.H; p.W = a.W;
@@ -196,7 +211,7 @@ cudaError_t launch_rg(const ExtractArgs& a, const int32_t* sel, cudaStream_t st)
     p.sel_idx = sel; p.top_k = a.top_k; p.r = a.r;
     p.kscale = static_cast<float>(1.4426950408889634 / static_cast<double>(a.T));
     p.out_kpts = a.out_kpts; p.out_scores = a.out_scores; p.out_off = a.out_offset;
-    if (a.desc == nullptr) return launch_rg_g<-1, 8>(p, a.B, st);
+    if (a.desc == nullptr) return launch_rg_g<-1, 8>(p, a.B, st, pdl);
     const size_t esz = a.desc_dtype == DKD_F16 ? 2 : 4;
     p.desc = static_cast<const unsigned char*>(a.desc);
     p.nchunk = static_cast<int>(a.D * esz / 16);
@@ -204,7 +219,7 @@ cudaError_t launch_rg(const ExtractArgs& a, const int32_t* sel, cudaStream_t st)
     p.ax = make_axis(a.stride, a.Wd);
     p.ay = make_axis(a.stride, a.Hd);
     p.out_desc = static_cast<unsigned char*>(a.out_desc);
-    return a.desc_dtype == DKD_F16 ? launch_rg_dt<DKD_F16>(p, a.B, st) : launch_rg_dt<DKD_F32>(p, a.B, st);
+    return a.desc_dtype == DKD_F16 ? launch_rg_dt<DKD_F16>(p, a.B, st, pdl) : launch_rg_dt<DKD_F32>(p, a.B, st, pdl);
 }
 
 // Enqueue the three kernels of one extract on `st`.  No sync, no allocation: capture-safe.
@@ -225,12 +240,12 @@ cudaError_t enqueue(dkd_ctx* ctx, const ExtractArgs& a, cudaStream_t st, bool pr
     if (e != cudaSuccess) return e;
     if ((e = mark()) != cudaSuccess) return e;
     int32_t* sel = a.out_index ? a.out_index : ctx->sel_idx;
-    k_select<<<a.B, SEL_THREADS, SEL_SMEM_BYTES, st>>>(ctx->cand, ctx->tile_cnt, tpi, a.top_k, sel,
-                                                                    a.out_count);
-    e = cudaGetLastError();
+    const bool pdl = ctx->use_pdl && !prof;                  // (events between the kernels would serialise them anyway)
+    e = launch_pdl(k_select, dim3(a.B), dim3(SEL_THREADS), SEL_SMEM_BYTES, st, pdl, ctx->cand, ctx->tile_cnt, tpi, a.top_k,
+                   sel, a.out_count);
     if (e != cudaSuccess) return e;
     if ((e = mark()) != cudaSuccess) return e;
-    e = launch_rg(a, sel, st);
+    e = launch_rg(a, sel, st, pdl);
     if (e != cudaSuccess) return e;
     if ((e = mark()) != cudaSuccess) return e;
     if (prof) ctx->prof_n = nk - 1;
@@ -361,6 +376,8 @@ int dkd_create(const dkd_create_params* p, dkd_ctx** out) {
     ctx->p = *p;
     ctx->use_graph = 1;
     ctx->use_tma = 1;
+    ctx->use_pdl = 1;
+    ctx->nms_cpu = 0;
     ctx->err[0] = 0;
     ctx->tick = 0;
 #define CKC(call)                                                                                        \
@@ -429,6 +446,13 @@ int dkd_set_option(dkd_ctx* ctx, int option, int value) {
         case DKD_OPT_USE_GRAPH: ctx->use_graph = value != 0; return DKD_OK;
         case DKD_OPT_USE_TMA: ctx->use_tma = value != 0; return DKD_OK;
         case DKD_OPT_PROFILE: ctx->profile = value != 0; ctx->prof_n = 0; return DKD_OK;
+        case DKD_OPT_USE_PDL:                               // part of what a cached graph contains: drop the cache
+        case DKD_OPT_NMS_UNIT:
+            for (auto& g : ctx->graphs) cudaGraphExecDestroy(g.exec);
+            ctx->graphs.clear();
+            if (option == DKD_OPT_USE_PDL) ctx->use_pdl = value != 0;
+            else ctx->nms_cpu = value > 0 ? value : 0;
+            return DKD_OK;
         default: return fail(ctx, DKD_ERR_INVALID_ARG, "unknown option");
     }
 }

@@ -95,6 +95,12 @@ __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* tmap) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(tmap)) : "memory");
 }
 
+// programmatic dependent launch (PDL): a kernel launched with the programmatic-stream-serialization
+// attribute may start while its predecessor still runs; pdl_wait() blocks until the predecessor grid
+// has completed and its writes are visible, pdl_launch_dependents() lets the successor be scheduled.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
+
 // 3-input max: one FMNMX3 on sm_100a (alu pipe), halves the op count of the window maxima
 __device__ __forceinline__ float fmax3(float a, float b, float c) {
     float d;
@@ -307,6 +313,7 @@ __global__ void __launch_bounds__(NMS_WARPS * 32, 2) k_nms_tma(const __grid_cons
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int first = blockIdx.x * NMS_WARPS + warp, step = gridDim.x * NMS_WARPS;
     const int n_my = first < p.units ? (p.units - first + step - 1) / step : 0;
+    pdl_launch_dependents();                                 // k_select may fill the SMs this grid leaves
     if (n_my == 0) return;
     unsigned char* my_smem = smem_raw + warp * NMS_STAGES * BOX_BYTES;
     uint64_t* bar = bars + warp * NMS_STAGES;
@@ -459,10 +466,12 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
     const int* cnt = tile_cnt + static_cast<size_t>(b) * tpi;
     const uint64_t* seg0 = cand + static_cast<size_t>(b) * tpi * SEG_CAP;
 
-    int local = 0;
-    for (int t = tid; t < tpi; t += SEL_THREADS) local += cnt[t];
+    pdl_launch_dependents();
     if (tid == 0) { s_n = 0; s_hi = 0u; s_lo = 0xffffffffu; s_maxb = 0; }
     for (int i = tid; i < NB; i += SEL_THREADS) { base[i] = 0; cur[i] = 0; }
+    pdl_wait();                                              // the candidates of k_nms_* are complete and visible
+    int local = 0;
+    for (int t = tid; t < tpi; t += SEL_THREADS) local += cnt[t];
     const int n = block_sum_1024(local, s_red);             // (its barriers also publish the initialisers)
 
     uint64_t lo = 0;                                        // gather keys >= lo (0: all of them)
@@ -799,6 +808,7 @@ __global__ void __launch_bounds__(RG_THREADS) k_refine_gather(const __grid_const
     if (i_img >= p.top_k) return;                           // whole groups leave together
     const int b = blockIdx.y;
     const size_t slot = static_cast<size_t>(b) * p.top_k + i_img;
+    pdl_wait();                                              // the selection of k_select is complete and visible
     const int idx = __ldg(p.sel_idx + slot);
 
     if (idx < 0) {                                          // step a5: zero padding

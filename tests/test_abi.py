@@ -48,9 +48,12 @@ def test_library_is_sm100a_with_tma():
     path = build.build()
     elf = subprocess.run(["cuobjdump", "-lelf", path], capture_output=True, text=True).stdout
     assert "sm_100a" in elf
-    sass = subprocess.run(["cuobjdump", "-sass", "-fun", "_ZN3dkd9k_nms_tmaILi2EEEv14CUtensorMap_stiiiiifPmPi", path],
-                          capture_output=True, text=True).stdout
+    full = subprocess.run(["cuobjdump", "-sass", path], capture_output=True, text=True).stdout
+    funcs = [f for f in full.split("Function : ")[1:] if "k_nms_tma" in f.split("\n")[0]]
+    assert len(funcs) == 8                                       # radius 1..4 x {thr_up > 0, thr_up <= 0}
+    sass = funcs[0]
     assert "UTMALDG" in sass                                     # TMA tile loads in the NMS kernel
+    assert "FMNMX3" in sass                                      # 3-input max of the separable window maximum
     assert "SYNCS" in sass                                       # mbarrier pipeline
 
 

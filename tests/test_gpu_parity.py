@@ -41,6 +41,22 @@ def test_small_multitile(ctx, r, HW):
     assert st["max_offset_err"] <= 1e-5
 
 
+@pytest.mark.parametrize("r", [1, 2, 3, 4])
+@pytest.mark.parametrize("unit", [2, 3, 8])
+def test_nms_units_of_several_strip_tiles(ctx, r, unit):
+    # a warp walks down `unit` strip-tiles carrying the last 2r rows in registers (the default picks
+    # units > 1 only for large batches): tall image, ragged last unit, every radius
+    from paper_2607_01757_b200.binding import OPT_NMS_UNIT
+    score, _ = small_inputs(2, 203, 250, seed=100 + 10 * r + unit, nblobs=500, D=0, dtype=None, stride=1)
+    try:
+        ctx.set_option(OPT_NMS_UNIT, unit)
+        res, ref = run_both(ctx, score, None, 1, r, 0.15, 512, 0.1)
+        compare(res, ref)
+    finally:
+        ctx.set_option(OPT_NMS_UNIT, 0)
+    assert ref.count.min() > 100
+
+
 @pytest.mark.parametrize("dtype,D", [(torch.float32, 4), (torch.float32, 64), (torch.float32, 512),
                                       (torch.float16, 8), (torch.float16, 128), (torch.float16, 256),
                                       (torch.float16, 1024), (torch.float16, 72)])
@@ -189,7 +205,7 @@ def test_negative_threshold_and_signed_zero(ctx):
 
 # ---- API surface -----------------------------------------------------------------------------------
 def test_loader_graph_and_literal_variants_agree(ctx):
-    from paper_2607_01757_b200.binding import OPT_USE_GRAPH, OPT_USE_TMA
+    from paper_2607_01757_b200.binding import OPT_USE_GRAPH, OPT_USE_TMA, OPT_USE_PDL
     score, desc = small_inputs(2, 100, 260, seed=21, nblobs=200, D=128, dtype=torch.float16, stride=1)
     sd = score.cuda()
     base = ctx.extract(sd, desc, 1, 2, 0.2, 256, 0.1)
@@ -197,16 +213,19 @@ def test_loader_graph_and_literal_variants_agree(ctx):
     try:
         for graph in (0, 1):
             for tma in (0, 1):
-                ctx.set_option(OPT_USE_GRAPH, graph)
-                ctx.set_option(OPT_USE_TMA, tma)
-                for rep in range(2):                              # second call replays the cached graph
-                    r2 = ctx.extract(sd, desc, 1, 2, 0.2, 256, 0.1)
-                    torch.cuda.synchronize()
-                    for n in ("kpts", "scores", "desc", "count", "index", "offsets"):
-                        assert torch.equal(getattr(base, n), getattr(r2, n)), (graph, tma, n)
+                for pdl in (0, 1):
+                    ctx.set_option(OPT_USE_GRAPH, graph)
+                    ctx.set_option(OPT_USE_TMA, tma)
+                    ctx.set_option(OPT_USE_PDL, pdl)
+                    for rep in range(3):                          # later calls replay the cached graph
+                        r2 = ctx.extract(sd, desc, 1, 2, 0.2, 256, 0.1)
+                        torch.cuda.synchronize()
+                        for n in ("kpts", "scores", "desc", "count", "index", "offsets"):
+                            assert torch.equal(getattr(base, n), getattr(r2, n)), (graph, tma, pdl, n)
     finally:
         ctx.set_option(OPT_USE_GRAPH, 1)
         ctx.set_option(OPT_USE_TMA, 1)
+        ctx.set_option(OPT_USE_PDL, 1)
     lit = ctx.alloc_outputs(2, 256, desc, 128, want_index=False, want_offsets=False)
     ctx.extract_literal(sd, desc, 1, 2, 0.2, 256, 0.1, lit)
     torch.cuda.synchronize()
