@@ -417,9 +417,10 @@ __global__ void __launch_bounds__(PLAIN_WARPS * 32) k_nms_plain(const float* __r
 
 // ---- k_select: per-image top-k select + order ---------------------------------------------------
 // One CTA per image.  n = sum of the image's strip-tile counts.
-//   n >  SORT_CAP : MSB-first radix select (8-bit digits, warp-aggregated shared-memory histogram)
-//                   narrows to a lower bound `lo` with  top_k <= #{key >= lo} <= SORT_CAP.
-//   gather        : every key >= lo (all keys when n <= SORT_CAP) is copied into shared memory.
+//   gather        : every key (n = sum of the image's strip-tile counts) is copied into shared memory.
+//   n >  SORT_CAP : (rare) MSB-first radix select (8-bit digits, warp-aggregated shared-memory histogram)
+//                   narrows to a lower bound `lo` with  top_k <= #{key >= lo} <= SORT_CAP; gather again,
+//                   keys >= lo only.
 //   order         : bucket rank (the common case) — one pass of a monotone bucket function over the
 //                   score bits (NB buckets spanning [min, max] of the gathered scores), an exclusive
 //                   scan of the bucket counts, a scatter into bucket order, and an exact rank
@@ -468,126 +469,129 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
 
     pdl_launch_dependents();
     if (tid == 0) { s_n = 0; s_hi = 0u; s_lo = 0xffffffffu; s_maxb = 0; }
-    for (int i = tid; i < NB; i += SEL_THREADS) { base[i] = 0; cur[i] = 0; }
+    for (int i = tid; i < NB; i += SEL_THREADS) cur[i] = 0;
     pdl_wait();                                              // the candidates of k_nms_* are complete and visible
-    int local = 0;
-    for (int t = tid; t < tpi; t += SEL_THREADS) local += cnt[t];
-    const int n = block_sum_1024(local, s_red);             // (its barriers also publish the initialisers)
+    __syncthreads();
 
     uint64_t lo = 0;                                        // gather keys >= lo (0: all of them)
-    if (n > SORT_CAP) {
-        uint64_t prefix = 0;
-        int need = top_k;                                   // rank (1-based, from the top) inside the prefix bucket
-        int above = 0;                                      // keys strictly above the prefix bucket
-        for (int shift = 56; shift >= 0; shift -= 8) {
-            for (int i = tid; i < 257; i += SEL_THREADS) s_hist[i] = 0;
-            __syncthreads();
-            for (int t = warp; t < tpi; t += NW) {
-                const int c = cnt[t];
-                const uint64_t* seg = seg0 + static_cast<size_t>(t) * SEG_CAP;
-                for (int e0 = 0; e0 < c; e0 += 32) {
-                    const int e = e0 + lane;
-                    int digit = 256;                        // dummy bin: past the end / outside the prefix
-                    if (e < c) {
-                        const uint64_t k = seg[e];
-                        const bool match = (shift == 56) || ((k >> (shift + 8)) == (prefix >> (shift + 8)));
-                        if (match) digit = static_cast<int>((k >> shift) & 255u);
+    for (int pass = 0; pass < 2; ++pass) {                  // second pass only if the first found n > SORT_CAP
+        // ---- gather: 32 strip-tiles per warp iteration; lane l reads tile l's count, the warp copies the
+        // concatenation of the 32 segments with every lane busy (a 5-step search finds an item's tile)
+        unsigned khi = 0u, klo = 0xffffffffu;                   // range of the gathered score words
+        for (int t0 = warp * 32; t0 < tpi; t0 += NW * 32) {
+            const int t = t0 + lane;
+            const int c = t < tpi ? cnt[t] : 0;
+            int incl = c;
+    #pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int up = __shfl_up_sync(FULL, incl, o);
+                if (lane >= o) incl += up;
+            }
+            const int total = __shfl_sync(FULL, incl, 31);
+            if (total == 0) continue;                           // warp-uniform
+            int gbase = 0;
+            if (lo == 0) {                                      // all keys are kept: reserve the slots at once
+                if (lane == 0) gbase = atomicAdd(&s_n, total);
+                gbase = __shfl_sync(FULL, gbase, 0);
+                if (gbase + total > SORT_CAP) continue;         // too many candidates (rare): counted, radix select below
+            }
+            for (int e0 = 0; e0 < total; e0 += 32) {
+                const int e = e0 + lane;
+                int tl = 0;                                     // first lane whose inclusive count exceeds e
+    #pragma unroll
+                for (int step = 16; step > 0; step >>= 1) {
+                    const int v = __shfl_sync(FULL, incl, tl + step - 1);
+                    if (v <= e) tl += step;
+                }
+                const int excl = __shfl_sync(FULL, incl - c, tl);
+                uint64_t k = 0ull;
+                if (e < total) k = seg0[static_cast<size_t>(t0 + tl) * SEG_CAP + (e - excl)];
+                if (lo == 0) {
+                    if (e < total) keys[gbase + e] = k;
+                } else {
+                    const bool take = (e < total) && (k >= lo);
+                    const unsigned bal = __ballot_sync(FULL, take);
+                    if (bal) {
+                        int pb = 0;
+                        if (lane == 0) pb = atomicAdd(&s_n, __popc(bal));
+                        pb = __shfl_sync(FULL, pb, 0);
+                        if (take) keys[pb + __popc(bal & ((1u << lane) - 1u))] = k;
                     }
-                    const unsigned peers = __match_any_sync(FULL, digit);
-                    if (lane == __ffs(peers) - 1) atomicAdd(&s_hist[digit], __popc(peers));
+                    if (!take) k = 0ull;
+                }
+                if (k != 0ull) {
+                    const unsigned kb = static_cast<unsigned>(k >> 32);
+                    khi = kb > khi ? kb : khi;
+                    klo = kb < klo ? kb : klo;
                 }
             }
-            __syncthreads();
-            if (warp == 0) {                                // find the digit holding the need-th largest key
-                int grp = 0;                                // lane l owns bins 255-8l .. 248-8l (descending)
-#pragma unroll
-                for (int q = 0; q < 8; ++q) grp += s_hist[255 - 8 * lane - q];
-                int incl = grp;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const int up = __shfl_up_sync(FULL, incl, o);
-                    if (lane >= o) incl += up;
-                }
-                const unsigned hit = __ballot_sync(FULL, incl >= need);
-                const int owner = __ffs(hit) - 1;           // exists: need <= keys in the bucket
-                if (lane == owner) {
-                    int cum = incl - grp;
-                    int d = 255 - 8 * lane;
-                    for (int q = 0; q < 8; ++q, --d) {
-                        const int h = s_hist[d];
-                        if (cum + h >= need) break;
-                        cum += h;
+        }
+        khi = __reduce_max_sync(FULL, khi);
+        klo = __reduce_min_sync(FULL, klo);
+        if (lane == 0 && khi >= klo) { atomicMax(&s_hi, khi); atomicMin(&s_lo, klo); }
+        __syncthreads();
+        if (s_n <= SORT_CAP) break;                         // block-uniform; always true in the second pass
+        {
+            uint64_t prefix = 0;
+            int need = top_k;                                   // rank (1-based, from the top) inside the prefix bucket
+            int above = 0;                                      // keys strictly above the prefix bucket
+            for (int shift = 56; shift >= 0; shift -= 8) {
+                for (int i = tid; i < 257; i += SEL_THREADS) s_hist[i] = 0;
+                __syncthreads();
+                for (int t = warp; t < tpi; t += NW) {
+                    const int c = cnt[t];
+                    const uint64_t* seg = seg0 + static_cast<size_t>(t) * SEG_CAP;
+                    for (int e0 = 0; e0 < c; e0 += 32) {
+                        const int e = e0 + lane;
+                        int digit = 256;                        // dummy bin: past the end / outside the prefix
+                        if (e < c) {
+                            const uint64_t k = seg[e];
+                            const bool match = (shift == 56) || ((k >> (shift + 8)) == (prefix >> (shift + 8)));
+                            if (match) digit = static_cast<int>((k >> shift) & 255u);
+                        }
+                        const unsigned peers = __match_any_sync(FULL, digit);
+                        if (lane == __ffs(peers) - 1) atomicAdd(&s_hist[digit], __popc(peers));
                     }
-                    s_digit = d;
-                    s_cum = cum;
-                    s_h = s_hist[d];
                 }
-            }
-            __syncthreads();
-            prefix |= static_cast<uint64_t>(s_digit) << shift;
-            above += s_cum;
-            need -= s_cum;
-            const bool done = (above + s_h <= SORT_CAP);
-            __syncthreads();
-            if (done) break;
-        }
-        lo = prefix;
-    }
-
-    // ---- gather: 32 strip-tiles per warp iteration; lane l reads tile l's count, the warp copies the
-    // concatenation of the 32 segments with every lane busy (a 5-step search finds an item's tile)
-    unsigned khi = 0u, klo = 0xffffffffu;                   // range of the gathered score words
-    for (int t0 = warp * 32; t0 < tpi; t0 += NW * 32) {
-        const int t = t0 + lane;
-        const int c = t < tpi ? cnt[t] : 0;
-        int incl = c;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int up = __shfl_up_sync(FULL, incl, o);
-            if (lane >= o) incl += up;
-        }
-        const int total = __shfl_sync(FULL, incl, 31);
-        if (total == 0) continue;                           // warp-uniform
-        int gbase = 0;
-        if (lo == 0) {                                      // all keys are kept: reserve the slots at once
-            if (lane == 0) gbase = atomicAdd(&s_n, total);
-            gbase = __shfl_sync(FULL, gbase, 0);
-        }
-        for (int e0 = 0; e0 < total; e0 += 32) {
-            const int e = e0 + lane;
-            int tl = 0;                                     // first lane whose inclusive count exceeds e
-#pragma unroll
-            for (int step = 16; step > 0; step >>= 1) {
-                const int v = __shfl_sync(FULL, incl, tl + step - 1);
-                if (v <= e) tl += step;
-            }
-            const int excl = __shfl_sync(FULL, incl - c, tl);
-            uint64_t k = 0ull;
-            if (e < total) k = seg0[static_cast<size_t>(t0 + tl) * SEG_CAP + (e - excl)];
-            if (lo == 0) {
-                if (e < total) keys[gbase + e] = k;
-            } else {
-                const bool take = (e < total) && (k >= lo);
-                const unsigned bal = __ballot_sync(FULL, take);
-                if (bal) {
-                    int pb = 0;
-                    if (lane == 0) pb = atomicAdd(&s_n, __popc(bal));
-                    pb = __shfl_sync(FULL, pb, 0);
-                    if (take) keys[pb + __popc(bal & ((1u << lane) - 1u))] = k;
+                __syncthreads();
+                if (warp == 0) {                                // find the digit holding the need-th largest key
+                    int grp = 0;                                // lane l owns bins 255-8l .. 248-8l (descending)
+    #pragma unroll
+                    for (int q = 0; q < 8; ++q) grp += s_hist[255 - 8 * lane - q];
+                    int incl = grp;
+    #pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const int up = __shfl_up_sync(FULL, incl, o);
+                        if (lane >= o) incl += up;
+                    }
+                    const unsigned hit = __ballot_sync(FULL, incl >= need);
+                    const int owner = __ffs(hit) - 1;           // exists: need <= keys in the bucket
+                    if (lane == owner) {
+                        int cum = incl - grp;
+                        int d = 255 - 8 * lane;
+                        for (int q = 0; q < 8; ++q, --d) {
+                            const int h = s_hist[d];
+                            if (cum + h >= need) break;
+                            cum += h;
+                        }
+                        s_digit = d;
+                        s_cum = cum;
+                        s_h = s_hist[d];
+                    }
                 }
-                if (!take) k = 0ull;
+                __syncthreads();
+                prefix |= static_cast<uint64_t>(s_digit) << shift;
+                above += s_cum;
+                need -= s_cum;
+                const bool done = (above + s_h <= SORT_CAP);
+                __syncthreads();
+                if (done) break;
             }
-            if (k != 0ull) {
-                const unsigned kb = static_cast<unsigned>(k >> 32);
-                khi = kb > khi ? kb : khi;
-                klo = kb < klo ? kb : klo;
-            }
+            lo = prefix;
         }
+        if (tid == 0) { s_n = 0; s_hi = 0u; s_lo = 0xffffffffu; }
+        __syncthreads();
     }
-    khi = __reduce_max_sync(FULL, khi);
-    klo = __reduce_min_sync(FULL, klo);
-    if (lane == 0 && khi >= klo) { atomicMax(&s_hi, khi); atomicMin(&s_lo, klo); }
-    __syncthreads();
     const int m = s_n;
     const int K = m < top_k ? m : top_k;
     int32_t* out = sel_idx + static_cast<size_t>(b) * top_k;
