@@ -85,11 +85,18 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 // 3-D tiled TMA load (x, y, image) -> shared memory, completion signalled on `bar` (complete_tx).
 // Out-of-bounds elements (negative or past-the-end coordinates) are zero-filled by the hardware.
 __device__ __forceinline__ void tma_load_tile(void* dst, const CUtensorMap* tmap, uint64_t* bar, int x, int y,
-                                              int b) {
+                                              int b, uint64_t policy) {
     asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
-        ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(tmap)), "r"(smem_u32(bar)), "r"(x), "r"(y), "r"(b)
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%3, %4, %5}], [%2], %6;"
+        ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(tmap)), "r"(smem_u32(bar)), "r"(x), "r"(y), "r"(b), "l"(policy)
         : "memory");
+}
+// L2 policy for data that is read once (the score maps): evict first, so the stream does not push the
+// candidate lists and the previous call's outputs out of L2
+__device__ __forceinline__ uint64_t l2_evict_first_policy() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
 }
 __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* tmap) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(tmap)) : "memory");
@@ -318,6 +325,7 @@ __global__ void __launch_bounds__(NMS_WARPS * 32, 2) k_nms_tma(const __grid_cons
     unsigned char* my_smem = smem_raw + warp * NMS_STAGES * BOX_BYTES;
     uint64_t* bar = bars + warp * NMS_STAGES;
 
+    const uint64_t policy = l2_evict_first_policy();
     // issue side (every lane tracks the cursor, lane 0 issues): next box = chunk ic of unit iteration iit
     int iit = 0, ic = 0, issued = 0;
     UnitCoords iu = unit_coords(first, p);
@@ -326,7 +334,7 @@ __global__ void __launch_bounds__(NMS_WARPS * 32, 2) k_nms_tma(const __grid_cons
         const int s = issued % NMS_STAGES;
         if (lane == 0) {
             mbar_arrive_expect_tx(&bar[s], BOX_BYTES);
-            tma_load_tile(my_smem + s * BOX_BYTES, &tmap, &bar[s], iu.x0 - HALO_X, iu.y0 + R + TH * ic, iu.b);
+            tma_load_tile(my_smem + s * BOX_BYTES, &tmap, &bar[s], iu.x0 - HALO_X, iu.y0 + R + TH * ic, iu.b, policy);
         }
         ++issued;
         if (++ic == iu.nch) {
