@@ -743,11 +743,11 @@ __device__ __forceinline__ void sample_axis(int xi, float d, const SampleAxis a,
     i1 = i0 + 1 < a.n - 1 ? i0 + 1 : a.n - 1;
 }
 
-__device__ __forceinline__ uint4 ld_stream16(const void* p) {
+__device__ __forceinline__ uint4 ld_stream16(const void* p, uint64_t policy) {   // read-once data: no L1, L2 evict-first
     uint4 r;
-    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.u32 {%0, %1, %2, %3}, [%4], %5;"
                  : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
-                 : "l"(p));
+                 : "l"(p), "l"(policy));
     return r;
 }
 __device__ __forceinline__ float ex2_approx(float x) {      // 2^x, MUFU.EX2 (max 2 ulp)
@@ -888,14 +888,15 @@ __global__ void __launch_bounds__(RG_THREADS) k_refine_gather(const __grid_const
         const uint4* p10 = reinterpret_cast<const uint4*>(base + (static_cast<size_t>(y1) * Wd + x0) * rowb);
         const uint4* p11 = reinterpret_cast<const uint4*>(base + (static_cast<size_t>(y1) * Wd + x1) * rowb);
         constexpr int N = ChunkT<DT >= 0 ? DT : 0>::N;
+        const uint64_t policy = l2_evict_first_policy();
         float acc[ITERS][N];
         float ss = 0.0f;
 #pragma unroll
         for (int it = 0; it < ITERS; ++it) {
             const int ch = gl + G * it;
             if (ch < p.nchunk) {
-                const uint4 q00 = ld_stream16(p00 + ch), q01 = ld_stream16(p01 + ch);
-                const uint4 q10 = ld_stream16(p10 + ch), q11 = ld_stream16(p11 + ch);
+                const uint4 q00 = ld_stream16(p00 + ch, policy), q01 = ld_stream16(p01 + ch, policy);
+                const uint4 q10 = ld_stream16(p10 + ch, policy), q11 = ld_stream16(p11 + ch, policy);
                 float a[N], bq[N], cq[N], dq[N];
                 chunk_to_float<DT >= 0 ? DT : 0>(q00, a);
                 chunk_to_float<DT >= 0 ? DT : 0>(q01, bq);
