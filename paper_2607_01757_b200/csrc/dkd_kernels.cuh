@@ -812,7 +812,7 @@ struct RGParams {
 
 // DT: DKD_F32 / DKD_F16 descriptor maps, or -1 for keypoints only.  G: lanes per keypoint.
 template <int DT, int G>
-__global__ void __launch_bounds__(RG_THREADS) k_refine_gather(const __grid_constant__ RGParams p) {
+__global__ void __launch_bounds__(RG_THREADS, 6) k_refine_gather(const __grid_constant__ RGParams p) {
     constexpr int ITERS = (G == 32) ? DKD_MAX_ROW_BYTES / 16 / 32 : 1;   // chunks per lane
     const int gl = threadIdx.x & (G - 1);                   // lane within the group
     const unsigned gmask = (G == 32) ? 0xffffffffu : (((1u << G) - 1u) << ((threadIdx.x & 31) & ~(G - 1)));
