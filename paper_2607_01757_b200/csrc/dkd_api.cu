@@ -56,8 +56,8 @@ struct dkd_ctx {
     int nms_ctas_per_sm[MAX_R + 1];
     PFN_tensorMapEncodeTiled encode;
     // workspace (device)
-    uint64_t* cand;          // [max_tiles * SEG_CAP] candidate keys, one private segment per tile
-    int* tile_cnt;           // [max_tiles]
+    uint64_t* cand;          // [max_tiles * SEG_CAP] candidate keys, one private segment per NMS unit
+    int* tile_cnt;           // [max_tiles] keys in each segment
     int32_t* sel_idx;        // [max_batch * max_top_k]
     size_t max_tiles;
     size_t ws_bytes;
@@ -106,7 +106,7 @@ cudaError_t setup_nms(dkd_ctx* ctx) {
 
 // Strip-tiles per unit: as many as possible (the 2R rows above a unit are fetched once per unit) while
 // the units still fill the machine several times over.
-NmsPlan nms_plan(const dkd_ctx* ctx, const ExtractArgs& a) {
+NmsPlan nms_plan(const dkd_ctx* ctx, const ExtractArgs& a) {   // (a.use_tma == 0: the plain loader works per strip-tile)
     NmsPlan p;
     p.H = a.H; p.W = a.W;
     p.strips_x = (a.W + STRIP_W - 1) / STRIP_W;
@@ -120,6 +120,7 @@ NmsPlan nms_plan(const dkd_ctx* ctx, const ExtractArgs& a) {
         if (static_cast<long long>(p.strips_x) * segs * a.B >= 4 * slots) { best = cpu; break; }
     }
     if (ctx->nms_cpu > 0) best = ctx->nms_cpu < MAX_CPU ? ctx->nms_cpu : MAX_CPU;
+    if (!a.use_tma) best = 1;
     p.cpu = best;
     p.segs = (p.chunks_y + best - 1) / best;
     p.units = p.strips_x * p.segs * a.B;
@@ -127,8 +128,7 @@ NmsPlan nms_plan(const dkd_ctx* ctx, const ExtractArgs& a) {
 }
 
 template <int R>
-cudaError_t launch_nms(dkd_ctx* ctx, const ExtractArgs& a, cudaStream_t st) {
-    const NmsPlan p = nms_plan(ctx, a);
+cudaError_t launch_nms(dkd_ctx* ctx, const ExtractArgs& a, const NmsPlan& p, cudaStream_t st) {
     if (a.use_tma) {
         CUtensorMap tmap;
         const cuuint64_t dims[3] = {(cuuint64_t)a.W, (cuuint64_t)a.H, (cuuint64_t)a.B};
@@ -225,24 +225,24 @@ cudaError_t launch_rg(const ExtractArgs& a, const int32_t* sel, cudaStream_t st,
 // Enqueue the three kernels of one extract on `st`.  No sync, no allocation: capture-safe.
 // prof: measurement mode, an event on `st` before and after every kernel.
 cudaError_t enqueue(dkd_ctx* ctx, const ExtractArgs& a, cudaStream_t st, bool prof = false) {
-    const int tiles_x = (a.W + STRIP_W - 1) / STRIP_W, tiles_y = (a.H + TH - 1) / TH;
-    const int tpi = tiles_x * tiles_y;                      // strip-tiles (candidate segments) per image
+    const NmsPlan plan = nms_plan(ctx, a);
+    const int tpi = plan.strips_x * plan.segs;              // candidate segments (NMS units) per image
     cudaError_t e;
     int nk = 0;
     auto mark = [&]() { return prof ? cudaEventRecord(ctx->prof_ev[nk++], st) : cudaSuccess; };
     if ((e = mark()) != cudaSuccess) return e;
     switch (a.r) {
-        case 1: e = launch_nms<1>(ctx, a, st); break;
-        case 2: e = launch_nms<2>(ctx, a, st); break;
-        case 3: e = launch_nms<3>(ctx, a, st); break;
-        default: e = launch_nms<4>(ctx, a, st); break;
+        case 1: e = launch_nms<1>(ctx, a, plan, st); break;
+        case 2: e = launch_nms<2>(ctx, a, plan, st); break;
+        case 3: e = launch_nms<3>(ctx, a, plan, st); break;
+        default: e = launch_nms<4>(ctx, a, plan, st); break;
     }
     if (e != cudaSuccess) return e;
     if ((e = mark()) != cudaSuccess) return e;
     int32_t* sel = a.out_index ? a.out_index : ctx->sel_idx;
     const bool pdl = ctx->use_pdl && !prof;                  // (events between the kernels would serialise them anyway)
-    e = launch_pdl(k_select, dim3(a.B), dim3(SEL_THREADS), SEL_SMEM_BYTES, st, pdl, ctx->cand, ctx->tile_cnt, tpi, a.top_k,
-                   sel, a.out_count);
+    e = launch_pdl(k_select, dim3(a.B), dim3(SEL_THREADS), SEL_SMEM_BYTES, st, pdl, ctx->cand, ctx->tile_cnt, tpi,
+                   plan.cpu * SEG_CAP, a.top_k, sel, a.out_count);
     if (e != cudaSuccess) return e;
     if ((e = mark()) != cudaSuccess) return e;
     e = launch_rg(a, sel, st, pdl);
@@ -403,7 +403,7 @@ int dkd_create(const dkd_create_params* p, dkd_ctx** out) {
     CKC(setup_nms<4>(ctx));
     CKC(cudaFuncSetAttribute(k_select, cudaFuncAttributeMaxDynamicSharedMemorySize, SEL_SMEM_BYTES));
     const size_t tx = (p->max_w + STRIP_W - 1) / STRIP_W, ty = (p->max_h + TH - 1) / TH;
-    ctx->max_tiles = tx * ty * p->max_batch;
+    ctx->max_tiles = tx * (ty + MAX_CPU - 1) * p->max_batch;   // segments of whole units: up to MAX_CPU-1 spare strip-tiles per strip
     const size_t b_cand = align256(ctx->max_tiles * SEG_CAP * sizeof(uint64_t));
     const size_t b_cnt = align256(ctx->max_tiles * sizeof(int));
     const size_t b_sel = align256(static_cast<size_t>(p->max_batch) * p->max_top_k * sizeof(int32_t));

@@ -262,8 +262,8 @@ __device__ __forceinline__ unsigned strip_colmask(int X, int W, int R) {
 }
 
 // ---- work decomposition (host: nms_plan) -----------------------------------------------------------
-// strip-tile index t = (b * chunks_y + cy) * strips_x + sx  (segment t of `cand`, tile_cnt[t]).
-// unit u = (b * segs + sg) * strips_x + sx  covers strip-tiles cy = sg*cpu .. min(sg*cpu + cpu, chunks_y) - 1.
+// unit u = (b * segs + sg) * strips_x + sx  covers strip-tiles cy = sg*cpu .. min(sg*cpu + cpu, chunks_y) - 1 of
+// strip sx; its candidates go to segment u of `cand` (capacity cpu * SEG_CAP keys), their number to seg_cnt[u].
 struct NmsPlan {
     int H, W;
     int strips_x, chunks_y;  // strip-tiles per image row / column
@@ -272,7 +272,7 @@ struct NmsPlan {
     float thr_up;            // nextafter(thresh, +inf)
 };
 struct UnitCoords {
-    int b, x0, y0, nch, t0;  // image, first output column / row, strip-tiles in the unit, first strip-tile index
+    int b, x0, y0, nch;      // image, first output column / row, strip-tiles in the unit
 };
 __device__ __forceinline__ UnitCoords unit_coords(int u, const NmsPlan& p) {
     const int upi = p.strips_x * p.segs;
@@ -283,7 +283,6 @@ __device__ __forceinline__ UnitCoords unit_coords(int u, const NmsPlan& p) {
     c.x0 = sx * STRIP_W;
     c.y0 = sg * p.cpu * TH;
     c.nch = p.chunks_y - sg * p.cpu < p.cpu ? p.chunks_y - sg * p.cpu : p.cpu;
-    c.t0 = (c.b * p.chunks_y + sg * p.cpu) * p.strips_x + sx;
     return c;
 }
 
@@ -314,7 +313,7 @@ __global__ void __launch_bounds__(NMS_WARPS * 32, 2) k_nms_tma(const __grid_cons
                                                                const __grid_constant__ NmsPlan p,
                                                                const float* __restrict__ score,
                                                                uint64_t* __restrict__ cand,
-                                                               int* __restrict__ tile_cnt) {
+                                                               int* __restrict__ seg_cnt) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t bars[NMS_WARPS * NMS_STAGES];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -360,6 +359,9 @@ __global__ void __launch_bounds__(NMS_WARPS * 32, 2) k_nms_tma(const __grid_cons
         float4 cat[TH + 2 * R];                              // rows yc-R .. yc+R+TH-1 of the current strip-tile
         load_head<R>(cat, score + static_cast<size_t>(cu.b) * p.H * p.W, X, cu.y0, p.H, p.W);
         const unsigned colmask = strip_colmask(X, p.W, R);
+        const int u = first + it * step;                     // the unit's candidate segment: p.cpu * SEG_CAP keys
+        uint64_t* useg = cand + static_cast<size_t>(u) * (p.cpu * SEG_CAP);
+        int ucnt = 0;                                        // warp-uniform running count of the segment
         for (int c = 0; c < cu.nch; ++c) {
             const int s = consumed % NMS_STAGES;
             mbar_wait(&bar[s], (consumed / NMS_STAGES) & 1);
@@ -371,16 +373,14 @@ __global__ void __launch_bounds__(NMS_WARPS * 32, 2) k_nms_tma(const __grid_cons
             }
             unsigned neg[4];
             nms_rows<R, NEGT>(cat, p.thr_up, neg);
-            const int t = cu.t0 + c * p.strips_x;
-            const int cnt = nms_emit<R>(neg, colmask, X, cu.y0 + TH * c, p.H, p.W, cat, rows,
-                                        cand + static_cast<size_t>(t) * SEG_CAP);
+            ucnt += nms_emit<R>(neg, colmask, X, cu.y0 + TH * c, p.H, p.W, cat, rows, useg + ucnt);
             __syncwarp();                                    // every lane is done with stage s
             issue_box();                                     // (the other NMS_STAGES-1 boxes stay in flight meanwhile)
             ++consumed;
-            if (lane == 0) tile_cnt[t] = cnt;
 #pragma unroll
             for (int q = 0; q < 2 * R; ++q) cat[q] = cat[TH + q];   // the 2R rows above the next strip-tile
         }
+        if (lane == 0) seg_cnt[u] = ucnt;
         if (it + 1 < n_my) cu = unit_coords(first + (it + 1) * step, p);
     }
 }
@@ -392,9 +392,9 @@ template <int R>
 __global__ void __launch_bounds__(PLAIN_WARPS * 32) k_nms_plain(const float* __restrict__ score,
                                                                 const __grid_constant__ NmsPlan p, int total,
                                                                 uint64_t* __restrict__ cand,
-                                                                int* __restrict__ tile_cnt) {
+                                                                int* __restrict__ seg_cnt) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int t = blockIdx.x * PLAIN_WARPS + warp;
+    const int t = blockIdx.x * PLAIN_WARPS + warp;          // unit == strip-tile (nms_plan: cpu = 1 on this path)
     if (t >= total) return;
     const int tpi = p.strips_x * p.chunks_y;
     const int b = t / tpi, rem = t - b * tpi;
@@ -420,7 +420,7 @@ __global__ void __launch_bounds__(PLAIN_WARPS * 32) k_nms_plain(const float* __r
     nms_rows<R, true>(cat, p.thr_up, neg);
     const int cnt = nms_emit<R>(neg, strip_colmask(X, p.W, R), X, y0, p.H, p.W, cat, boxes[warp],
                                 cand + static_cast<size_t>(t) * SEG_CAP);
-    if (lane == 0) tile_cnt[t] = cnt;
+    if (lane == 0) seg_cnt[t] = cnt;
 }
 
 // ---- k_select: per-image top-k select + order ---------------------------------------------------
@@ -455,7 +455,8 @@ __device__ __forceinline__ int block_sum_1024(int v, int* s_red) {
 }
 
 __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __restrict__ cand,
-                                                           const int* __restrict__ tile_cnt, int tpi, int top_k,
+                                                           const int* __restrict__ seg_cnt, int tpi, int seg_cap,
+                                                           int top_k,
                                                            int32_t* __restrict__ sel_idx,
                                                            int32_t* __restrict__ out_count) {
     extern __shared__ __align__(16) unsigned char sel_smem[];
@@ -472,8 +473,8 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
     constexpr int NW = SEL_THREADS / 32;
     constexpr unsigned FULL = 0xffffffffu;
     const int b = blockIdx.x;
-    const int* cnt = tile_cnt + static_cast<size_t>(b) * tpi;
-    const uint64_t* seg0 = cand + static_cast<size_t>(b) * tpi * SEG_CAP;
+    const int* cnt = seg_cnt + static_cast<size_t>(b) * tpi;             // tpi segments of seg_cap keys per image
+    const uint64_t* seg0 = cand + static_cast<size_t>(b) * tpi * seg_cap;
 
     pdl_launch_dependents();
     if (tid == 0) { s_n = 0; s_hi = 0u; s_lo = 0xffffffffu; s_maxb = 0; }
@@ -481,14 +482,16 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
     pdl_wait();                                              // the candidates of k_nms_* are complete and visible
     __syncthreads();
 
+    // segments per warp iteration: all 32 warps busy with as few dependent rounds as possible
+    const int gt = tpi >= 32 * NW ? 32 : (tpi + NW - 1) / NW;
     uint64_t lo = 0;                                        // gather keys >= lo (0: all of them)
     for (int pass = 0; pass < 2; ++pass) {                  // second pass only if the first found n > SORT_CAP
-        // ---- gather: 32 strip-tiles per warp iteration; lane l reads tile l's count, the warp copies the
-        // concatenation of the 32 segments with every lane busy (a 5-step search finds an item's tile)
+        // ---- gather: gt <= 32 segments per warp iteration; lane l reads segment l's count, the warp copies
+        // the concatenation of the segments with every lane busy (a 5-step search finds an item's segment)
         unsigned khi = 0u, klo = 0xffffffffu;                   // range of the gathered score words
-        for (int t0 = warp * 32; t0 < tpi; t0 += NW * 32) {
+        for (int t0 = warp * gt; t0 < tpi; t0 += NW * gt) {
             const int t = t0 + lane;
-            const int c = t < tpi ? cnt[t] : 0;
+            const int c = (lane < gt && t < tpi) ? cnt[t] : 0;
             int incl = c;
     #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
@@ -513,7 +516,7 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
                 }
                 const int excl = __shfl_sync(FULL, incl - c, tl);
                 uint64_t k = 0ull;
-                if (e < total) k = seg0[static_cast<size_t>(t0 + tl) * SEG_CAP + (e - excl)];
+                if (e < total) k = seg0[static_cast<size_t>(t0 + tl) * seg_cap + (e - excl)];
                 if (lo == 0) {
                     if (e < total) keys[gbase + e] = k;
                 } else {
@@ -548,7 +551,7 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
                 __syncthreads();
                 for (int t = warp; t < tpi; t += NW) {
                     const int c = cnt[t];
-                    const uint64_t* seg = seg0 + static_cast<size_t>(t) * SEG_CAP;
+                    const uint64_t* seg = seg0 + static_cast<size_t>(t) * seg_cap;
                     for (int e0 = 0; e0 < c; e0 += 32) {
                         const int e = e0 + lane;
                         int digit = 256;                        // dummy bin: past the end / outside the prefix
