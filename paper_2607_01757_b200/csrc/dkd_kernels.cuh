@@ -506,34 +506,44 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
                 gbase = __shfl_sync(FULL, gbase, 0);
                 if (gbase + total > SORT_CAP) continue;         // too many candidates (rare): counted, radix select below
             }
-            for (int e0 = 0; e0 < total; e0 += 32) {
-                const int e = e0 + lane;
-                int tl = 0;                                     // first lane whose inclusive count exceeds e
-    #pragma unroll
-                for (int step = 16; step > 0; step >>= 1) {
-                    const int v = __shfl_sync(FULL, incl, tl + step - 1);
-                    if (v <= e) tl += step;
-                }
-                const int excl = __shfl_sync(FULL, incl - c, tl);
-                uint64_t k = 0ull;
-                if (e < total) k = seg0[static_cast<size_t>(t0 + tl) * seg_cap + (e - excl)];
-                if (lo == 0) {
-                    if (e < total) keys[gbase + e] = k;
-                } else {
-                    const bool take = (e < total) && (k >= lo);
-                    const unsigned bal = __ballot_sync(FULL, take);
-                    if (bal) {
-                        int pb = 0;
-                        if (lane == 0) pb = atomicAdd(&s_n, __popc(bal));
-                        pb = __shfl_sync(FULL, pb, 0);
-                        if (take) keys[pb + __popc(bal & ((1u << lane) - 1u))] = k;
+            constexpr int GU = 4;                               // loads in flight per lane
+            for (int e0 = 0; e0 < total; e0 += 32 * GU) {
+                uint64_t kk[GU];
+#pragma unroll
+                for (int u = 0; u < GU; ++u) {                  // (warp-uniform trip count: shuffles inside)
+                    const int e = e0 + 32 * u + lane;
+                    int tl = 0;                                 // first lane whose inclusive count exceeds e
+#pragma unroll
+                    for (int step = 16; step > 0; step >>= 1) {
+                        const int v = __shfl_sync(FULL, incl, tl + step - 1);
+                        if (v <= e) tl += step;
                     }
-                    if (!take) k = 0ull;
+                    const int excl = __shfl_sync(FULL, incl - c, tl);
+                    kk[u] = 0ull;
+                    if (e < total) kk[u] = seg0[static_cast<size_t>(t0 + tl) * seg_cap + (e - excl)];
                 }
-                if (k != 0ull) {
-                    const unsigned kb = static_cast<unsigned>(k >> 32);
-                    khi = kb > khi ? kb : khi;
-                    klo = kb < klo ? kb : klo;
+#pragma unroll
+                for (int u = 0; u < GU; ++u) {
+                    const int e = e0 + 32 * u + lane;
+                    uint64_t k = kk[u];
+                    if (lo == 0) {
+                        if (e < total) keys[gbase + e] = k;
+                    } else {
+                        const bool take = (e < total) && (k >= lo);
+                        const unsigned bal = __ballot_sync(FULL, take);
+                        if (bal) {
+                            int pb = 0;
+                            if (lane == 0) pb = atomicAdd(&s_n, __popc(bal));
+                            pb = __shfl_sync(FULL, pb, 0);
+                            if (take) keys[pb + __popc(bal & ((1u << lane) - 1u))] = k;
+                        }
+                        if (!take) k = 0ull;
+                    }
+                    if (k != 0ull) {
+                        const unsigned kb = static_cast<unsigned>(k >> 32);
+                        khi = kb > khi ? kb : khi;
+                        klo = kb < klo ? kb : klo;
+                    }
                 }
             }
         }
