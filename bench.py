@@ -206,7 +206,7 @@ def run_ours(args):
     import torch.distributed as dist
     import synth
     import paper_2607_01757_b200 as dkd
-    from paper_2607_01757_b200.binding import OPT_PROFILE
+    from paper_2607_01757_b200.binding import OPT_PROFILE, OPT_USE_GRAPH
 
     rank, world, local = dist_env()
     if not torch.cuda.is_available():
@@ -288,6 +288,23 @@ def run_ours(args):
         torch.cuda.synchronize()
         lat.append((time.perf_counter() - t0) * 1e6)
     lat.sort()
+
+    # the same steps as plain stream launches (DKD_OPT_USE_GRAPH = 0: three PDL-linked launches per step)
+    stream_us = None
+    if args.leg != "c5":
+        ctx.set_option(OPT_USE_GRAPH, 0)
+        for i in range(Wm):
+            calls[i % R]()
+        barrier()
+        torch.cuda.synchronize()
+        ev0.record(stream)
+        for i in range(K):
+            calls[i % R]()
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        barrier()
+        stream_us = max_over_ranks(ev0.elapsed_time(ev1) / K) * 1e3 / world
+        ctx.set_option(OPT_USE_GRAPH, 1)
 
     # per-kernel device time at c2 (library measurement mode: plain launches + events)
     ctx.set_option(OPT_PROFILE, 1)
@@ -427,12 +444,14 @@ def run_ours(args):
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": workload_name(cfg), "l2": f"cold: steps rotate through {R} distinct seeded input sets "
                        f"({R * cb['total'] / 1e6:.0f} MB touched per rotation > 126 MB L2)",
-                       "launch": "one cached CUDA-graph launch per step (3 kernels)", "parallelism": f"batch-sharded x{world}, no collective"},
+                       "launch": "one cached CUDA-graph launch per step (3 kernels, programmatic dependent launch edges)", "parallelism": f"batch-sharded x{world}, no collective"},
             "frames_per_s": world * cfg.B / (ms_step * 1e-3), "keypoints_per_s": world * kept / (ms_step * 1e-3),
             "credited_bytes": cb, "credited_gbs": cb["total"] / (ms_step * 1e-3) / 1e9,
             "wall_ms_per_step": wall_ms_step,
             "latency_us": {"median": lat[len(lat) // 2], "min": lat[0], "p95": lat[int(len(lat) * 0.95)],
                            "what": "single shot: enqueue -> stream idle, host clock"},
+            "stream_launch": {"value": stream_us, "unit": UNIT,
+                              "what": "same steps with DKD_OPT_USE_GRAPH = 0: three PDL-linked launches per step instead of one graph launch"},
             "kernel_us_c2": kt2,
             "clocks": sampler.summary(),
             "e2e": {"value": e2e_us / world, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
