@@ -84,6 +84,37 @@ def test_temperature(ctx, T):
     compare(res, ref)
 
 
+# ---- seeded random sweep over shapes and parameters ---------------------------------------------
+@pytest.mark.parametrize("case", range(48))
+def test_random_shapes_and_parameters(ctx, case):
+    """Random small problems (ragged widths incl. W % 4 != 0 -> plain loader, images smaller than a
+    strip-tile, every radius / stride / descriptor type, top_k above and below the candidate count,
+    forced NMS unit lengths) against the oracle."""
+    from paper_2607_01757_b200.binding import OPT_NMS_UNIT
+    g = np.random.default_rng(1000 + case)
+    B = int(g.integers(1, 4))
+    H = int(g.integers(3, 140))
+    W = int(g.integers(3, 400))
+    if case % 3 == 0:
+        W = 4 * max(W // 4, 1)                                    # TMA path
+    r = int(g.integers(1, 5))
+    stride = int(g.choice([1, 1, 2, 4, 8]))
+    dtype, D = [(torch.float16, 64), (torch.float16, 8), (torch.float32, 32), (torch.float16, 264), (None, 0)][case % 5]
+    top_k = int(g.choice([1, 7, 64, 300, 2048]))
+    thresh = float(g.choice([0.0, 0.05, 0.2, 0.6]))
+    T = float(g.choice([0.05, 0.1, 0.5]))
+    score = synth.score_maps(B, H, W, 5000 + case, 0.1, int(g.integers(0, 200)))
+    desc = None
+    if D:
+        desc = synth.desc_maps(B, max(H // stride, 1), max(W // stride, 1), D, case, dtype, "cuda")
+    try:
+        ctx.set_option(OPT_NMS_UNIT, int(g.integers(0, 9)))
+        res, ref = run_both(ctx, score, desc, stride, r, thresh, top_k, T)
+        compare(res, ref, dtype)
+    finally:
+        ctx.set_option(OPT_NMS_UNIT, 0)
+
+
 # ---- full-size configs c1-c4 ---------------------------------------------------------------------
 @pytest.mark.parametrize("name", ["c1", "c2", "c3", "c4"])
 def test_config_full_size(name):
