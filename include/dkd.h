@@ -137,12 +137,17 @@ int dkd_extract_ex(dkd_ctx* ctx,
                    void* stream);
 
 /*
- * dkd_extract_host — the same call with HOST buffers (the end-to-end path): copies score (and desc)
- * host->device into context-owned staging buffers, runs dkd_extract_ex, copies every non-NULL
- * output device->host, and synchronises `stream` before returning.  Staging is (re)allocated on
- * first use / growth.  Pointers have the shapes above; pinned memory makes the copies asynchronous.
- * desc_resident != 0 reuses the descriptor map uploaded by the previous call with the same
- * desc pointer and shape (a dense network would leave it on the device).
+ * dkd_extract_host — the same call with HOST buffers (the end-to-end path): copies score host->device
+ * into a context-owned staging buffer, runs dkd_extract_ex, delivers every non-NULL output to the host
+ * buffers, and synchronises `stream` before returning.  Staging is (re)allocated on first use / growth.
+ * Pointers have the shapes above.  Pinned (page-locked, mapped: cudaHostAlloc / cudaHostRegister) buffers
+ * are used in place where that is cheaper:
+ *   - a pinned descriptor map of which the call can touch at most 1/8 (4 rows per output slot) is NOT
+ *     uploaded: the gather samples its corner rows directly over PCIe;
+ *   - when every output buffer is pinned the kernels store straight into them (no staging, no copies back).
+ * Pageable buffers go through staged cudaMemcpyAsync copies.
+ * desc_resident != 0 uploads the descriptor map once and reuses the device copy while the same desc pointer
+ * and shape are passed (a dense network would leave it on the device).
  */
 int dkd_extract_host(dkd_ctx* ctx,
                      const float* score, int B, int H, int W,

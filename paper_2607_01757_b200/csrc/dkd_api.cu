@@ -354,6 +354,17 @@ int grow(dkd_ctx* ctx, void** buf, size_t* have, size_t need) {
 
 size_t align256(size_t x) { return (x + 255) & ~static_cast<size_t>(255); }
 
+// device address of a pinned, mapped host buffer (cudaHostAlloc / cudaHostRegister); NULL for pageable memory
+void* mapped_device_pointer(const void* host) {
+    if (!host) return nullptr;
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, host) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return nullptr;
+    }
+    return at.type == cudaMemoryTypeHost ? at.devicePointer : nullptr;
+}
+
 }  // namespace
 
 extern "C" {
@@ -517,19 +528,48 @@ int dkd_extract_host(dkd_ctx* ctx, const float* score, int B, int H, int W, cons
     const size_t o_desc = align256(o_off + slots * 8), n_out = align256(o_desc + (desc ? slots * D * esz : 0));
     int rc;
     if ((rc = grow(ctx, &ctx->st_score, &ctx->st_score_bytes, n_score)) != DKD_OK) return rc;
-    if ((rc = grow(ctx, &ctx->st_out, &ctx->st_out_bytes, n_out)) != DKD_OK) return rc;
+    // Pinned (page-locked, mapped) host buffers are addressable from the device.  Two uses:
+    //  * descriptor map: only 4 rows per kept keypoint are ever read, so when that is a small part of the map
+    //    the gather samples it in place over PCIe instead of uploading all of it;
+    //  * outputs: when every output buffer is pinned the kernels store straight into them (no staging, no
+    //    device->host copies).
+    const void* desc_dev = nullptr;
     if (desc) {
+        const void* zc = mapped_device_pointer(desc);
+        const size_t touched = slots * 4 * static_cast<size_t>(D) * esz;
         const bool have = desc_resident && ctx->st_desc && ctx->st_desc_src == desc && ctx->st_desc_src_bytes == n_desc;
-        if (!have) {
+        if (have) {
+            desc_dev = ctx->st_desc;
+        } else if (zc && !desc_resident && touched * 8 <= n_desc) {
+            desc_dev = zc;
+        } else {
             if ((rc = grow(ctx, &ctx->st_desc, &ctx->st_desc_bytes, n_desc)) != DKD_OK) return rc;
             CK(ctx, cudaMemcpyAsync(ctx->st_desc, desc, n_desc, cudaMemcpyHostToDevice, st));
             ctx->st_desc_src = desc;
             ctx->st_desc_src_bytes = n_desc;
+            desc_dev = ctx->st_desc;
         }
     }
     CK(ctx, cudaMemcpyAsync(ctx->st_score, score, n_score, cudaMemcpyHostToDevice, st));
+    void* d_kpts = mapped_device_pointer(out_kpts);
+    void* d_scores = mapped_device_pointer(out_scores);
+    void* d_count = mapped_device_pointer(out_count);
+    void* d_desc = desc ? mapped_device_pointer(out_desc) : nullptr;
+    void* d_index = out_index ? mapped_device_pointer(out_index) : nullptr;
+    void* d_off = out_offset ? mapped_device_pointer(out_offset) : nullptr;
+    const bool direct = d_kpts && d_scores && d_count && (!desc || d_desc) && (!out_index || d_index) &&
+                        (!out_offset || d_off) && (!desc || (reinterpret_cast<uintptr_t>(d_desc) & 15) == 0);
+    if (direct) {
+        rc = dkd_extract_ex(ctx, static_cast<const float*>(ctx->st_score), B, H, W, desc_dev, desc_dtype, Hd, Wd, D, stride,
+                            r, thresh, top_k, T, static_cast<float*>(d_kpts), static_cast<float*>(d_scores), d_desc,
+                            static_cast<int32_t*>(d_count), static_cast<int32_t*>(d_index), static_cast<float*>(d_off), st);
+        if (rc != DKD_OK) return rc;
+        CK(ctx, cudaStreamSynchronize(st));
+        return DKD_OK;
+    }
+    if ((rc = grow(ctx, &ctx->st_out, &ctx->st_out_bytes, n_out)) != DKD_OK) return rc;
     char* so = static_cast<char*>(ctx->st_out);
-    rc = dkd_extract_ex(ctx, static_cast<const float*>(ctx->st_score), B, H, W, desc ? ctx->st_desc : nullptr,
+    rc = dkd_extract_ex(ctx, static_cast<const float*>(ctx->st_score), B, H, W, desc_dev,
                         desc_dtype, Hd, Wd, D, stride, r, thresh, top_k, T, reinterpret_cast<float*>(so + o_kpts),
                         reinterpret_cast<float*>(so + o_scores), desc ? so + o_desc : nullptr,
                         reinterpret_cast<int32_t*>(so + o_count),

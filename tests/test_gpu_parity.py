@@ -282,12 +282,19 @@ def test_host_path_matches_device_path(ctx):
     score, desc = small_inputs(2, 90, 200, seed=4, nblobs=100, D=128, dtype=torch.float16, stride=1)
     dev = ctx.extract(score.cuda(), desc, 1, 2, 0.2, 128, 0.1)
     torch.cuda.synchronize()
+    # pinned buffers: descriptor rows sampled in place over PCIe (the gather touches 128*4 of 18000 rows),
+    # outputs stored straight into the host tensors; pageable buffers: staged copies; resident: uploaded once
     sp, dp = score.pin_memory(), desc.cpu().pin_memory()
-    for resident in (False, True, True):
-        host = ctx.extract_host(sp, dp, 1, 2, 0.2, 128, 0.1, desc_resident=resident)
+    pageable_out = ctx.alloc_outputs(2, 128, desc, 128, device="cpu", pin=False)
+    for s_in, d_in, out, resident in ((sp, dp, None, False), (sp, dp, None, True), (sp, dp, None, True),
+                                      (score, desc.cpu(), pageable_out, False), (sp, dp, pageable_out, False),
+                                      (score, desc.cpu(), None, False)):
+        host = ctx.extract_host(s_in, d_in, 1, 2, 0.2, 128, 0.1, out=out, desc_resident=resident)
         for n in ("kpts", "scores", "desc", "count", "index", "offsets"):
             assert not getattr(host, n).is_cuda
             assert torch.equal(getattr(dev, n).cpu(), getattr(host, n)), n
+        for n in ("kpts", "scores", "desc", "count", "index", "offsets"):
+            getattr(host, n).zero_()
 
 
 def test_capture_safe_inside_a_user_graph(ctx):
