@@ -49,6 +49,8 @@ def lib():
         L.dkd_oracle_refine.argtypes = [vp, i, i, i, f, i, vp, vp, vp]
         L.dkd_oracle_gather.restype = None
         L.dkd_oracle_gather.argtypes = [vp, i, i, i, i, i, i, vp, vp, vp]
+        L.dkd_oracle_preprocess.restype = i
+        L.dkd_oracle_preprocess.argtypes = [vp, i, i, i, i, i, i, i, ctypes.c_double, vp, vp, ctypes.c_double, vp]
         L.dkd_oracle_extract.restype = i
         L.dkd_oracle_extract.argtypes = [vp, i, i, i, vp, i, i, i, i, i, i, f, i, f,
                                          vp, vp, vp, vp, vp, vp]
@@ -159,3 +161,27 @@ def extract(score, desc, stride, r, thresh, top_k, T) -> OracleResult:
     if rc != 0:
         raise ValueError("dkd_oracle_extract: invalid argument")
     return OracleResult(kp, off, sc, de, cnt, idx)
+
+
+# ---- fused input pre-processing ---------------------------
+def padded_size(H: int, W: int, grid: int):
+    """(Hp, Wp, oy, ox): padded size on the resolution grid and the centred letterbox offset (P1, P2)."""
+    Hp, Wp = (H + grid - 1) // grid * grid, (W + grid - 1) // grid * grid
+    return Hp, Wp, (Hp - H) // 2, (Wp - W) // 2
+
+
+def preprocess(src, out_channels, grid, bgr=False, scale=1.0 / 255.0, mean=(0.0, 0.0, 0.0),
+               inv_std=(1.0, 1.0, 1.0), pad_value=0.0) -> np.ndarray:
+    """src [B,H,W,Cin] u8 -> [B,Cout,Hp,Wp] f64 (letterbox, colour conversion, normalisation, NCHW)."""
+    src = _c(src, np.uint8)
+    B, H, W, Cin = src.shape
+    Hp, Wp, _, _ = padded_size(H, W, grid)
+    m = _c(np.asarray(mean, np.float64), np.float64)
+    s = _c(np.asarray(inv_std, np.float64), np.float64)
+    out = np.empty((B, int(out_channels), Hp, Wp), np.float64)
+    rc = lib().dkd_oracle_preprocess(_p(src), B, H, W, Cin, int(out_channels), int(grid), int(bool(bgr)),
+                                     float(scale), _p(m), _p(s), float(pad_value), _p(out))
+    if rc != 0:
+        raise ValueError("dkd_oracle_preprocess: invalid argument")
+    return out
+

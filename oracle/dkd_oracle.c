@@ -27,6 +27,9 @@
  *   O4: affine maps (bilinear exact); constant maps; torch grid_sample(border,
  *       align_corners=False); unit norm; zero-map guard.
  *   O5: direct equality.
+ *   pre-processing (dkd_oracle_preprocess, tests/test_preprocess_pins.py): hand-worked 2x3 fixture;
+ *       exact copy / pad-value / centred-offset invariants; BT.601 closed forms; an independent torch
+ *       pad + permute + matmul routine in float64; keypoint un-shift round trip.
  * Unpinned: agreement with the paper's own kernel / ALIKED's DKD (no worked example, no code,
  *   no printed number for this path exists in PAPER.md) — "parity unpinned" w.r.t. the paper's
  *   kernel; parity is against this definition only.
@@ -259,3 +262,48 @@ int dkd_oracle_extract(const float* score, int B, int H, int W,
     free(mask);
     return 0;
 }
+
+/* =============================================================================================
+ * Fused input pre-processing (Sec. III-B): letterbox padding to
+ * the resolution grid (multiples of 8 / 32), colour-format conversion (mono -> 3 channels by
+ * replication, colour -> one luminance channel), intensity normalisation, NCHW packing, stereo pair =
+ * batch.  The paper prints no constant; the readings (P1..P7):
+ *   P1 padded size Hp = ceil(H/g)*g, Wp = ceil(W/g)*g;
+ *   P2 letterbox is CENTRED: oy = (Hp-H)/2, ox = (Wp-W)/2 (integer division), source pixel (y,x) lands
+ *      at (y+oy, x+ox); keypoints are shifted back by subtracting (ox,oy);
+ *   P3 padding holds pad_value (a value in OUTPUT units, i.e. after normalisation);
+ *   P4 luminance = 0.299 R + 0.587 G + 0.114 B (ITU-R BT.601) on the 8-bit values; `bgr` says the
+ *      interleaved input is B,G,R; 3 -> 3 channels re-orders to R,G,B planes;
+ *   P5 normalisation: out = (value * scale - mean[c]) * inv_std[c]  (scale = 1/255 for [0,1]);
+ *   P6 mono -> 3 channels: the same 8-bit value in every plane, each with its own mean / inv_std;
+ *   P7 output planar [B,Cout,Hp,Wp].
+ * src [B,H,W,Cin] u8 interleaved; out [B,Cout,Hp,Wp] double.  Returns 0, -1 on a bad argument.
+ * ============================================================================================= */
+int dkd_oracle_preprocess(const uint8_t* src, int B, int H, int W, int Cin, int Cout, int grid, int bgr,
+                          double scale, const double* mean, const double* inv_std, double pad_value,
+                          double* out) {
+    if (!src || !out || B < 1 || H < 1 || W < 1 || grid < 1) return -1;
+    if (!((Cin == 1 || Cin == 3) && (Cout == 1 || Cout == 3))) return -1;
+    int Hp = (H + grid - 1) / grid * grid, Wp = (W + grid - 1) / grid * grid;
+    int oy = (Hp - H) / 2, ox = (Wp - W) / 2;
+    for (int b = 0; b < B; ++b)
+        for (int c = 0; c < Cout; ++c)
+            for (int yp = 0; yp < Hp; ++yp)
+                for (int xp = 0; xp < Wp; ++xp) {
+                    double* o = out + (((size_t)b * Cout + c) * Hp + yp) * Wp + xp;
+                    int y = yp - oy, x = xp - ox;
+                    if (y < 0 || y >= H || x < 0 || x >= W) { *o = pad_value; continue; }
+                    const uint8_t* px = src + (((size_t)b * H + y) * W + x) * Cin;
+                    double v;
+                    if (Cin == 1) {
+                        v = (double)px[0];                                   /* P6 (or 1 -> 1) */
+                    } else {
+                        double R = (double)px[bgr ? 2 : 0], G = (double)px[1], Bl = (double)px[bgr ? 0 : 2];
+                        if (Cout == 1) v = 0.299 * R + 0.587 * G + 0.114 * Bl;          /* P4 */
+                        else v = c == 0 ? R : (c == 1 ? G : Bl);
+                    }
+                    *o = (v * scale - mean[c]) * inv_std[c];                 /* P5 */
+                }
+    return 0;
+}
+
