@@ -58,6 +58,9 @@ enum {
     DKD_OPT_USE_PDL   = 3,   /* [1] the select and refine/gather kernels are launched with programmatic
                                 stream serialization (they start while their predecessor drains and wait
                                 on-device for its results): hides the launch latency between the kernels. */
+    DKD_OPT_ORIGIN_X  = 5,   /* [0] letterbox offset (ox, oy) of the score map inside the padded network input: it is */
+    DKD_OPT_ORIGIN_Y  = 6,   /* [0] subtracted from every keypoint coordinate ("shifted back to native coordinates by
+                                subtracting the offset"); out_index / out_offset are unaffected. */
     DKD_OPT_NMS_UNIT  = 4    /* [0] strip-tiles (8 output rows each) a warp of the NMS kernel walks down before it
                                 moves to another strip: 0 = chosen per call from the problem size, 1..8 = forced
                                 (tuning / test knob; results do not depend on it). */
@@ -156,6 +159,37 @@ int dkd_extract_host(dkd_ctx* ctx,
                      float* out_kpts, float* out_scores, void* out_desc, int32_t* out_count,
                      int32_t* out_index, float* out_offset,
                      int desc_resident, void* stream);
+
+/*
+ * Fused input pre-processing (Sec. III-B: "letterbox padding, color-format conversion,
+ * intensity normalization, and NCHW layout packing in a single pass, with stereo pairs processed as one
+ * batch"; frames padded to multiples of 8 (SuperPoint, XFeat) or 32 (ALIKED, RaCo); mono replicated to three
+ * channels, colour reduced to one luminance channel).  The paper prints no constant; P1..P7:
+ *   padded size Hp = ceil(H/grid)*grid, Wp likewise; the image is CENTRED: oy = (Hp-H)/2, ox = (Wp-W)/2;
+ *   padding holds pad_value (output units); luminance = 0.299 R + 0.587 G + 0.114 B (BT.601);
+ *   out = (value * scale - mean[c]) * inv_std[c]; 3 -> 3 channels are written as R,G,B planes.
+ */
+typedef struct {
+    int in_channels;     /* 1 (mono) or 3 (interleaved colour) */
+    int out_channels;    /* 1 or 3 */
+    int grid;            /* >= 1; H and W are padded up to multiples of it */
+    int bgr;             /* != 0: colour input is stored B,G,R */
+    int out_dtype;       /* DKD_F32 or DKD_F16 */
+    float scale;         /* 1/255 maps 8-bit values to [0,1] */
+    float mean[3];
+    float inv_std[3];
+    float pad_value;
+} dkd_pre_params;
+
+/* Padded size and letterbox offset for (H, W, grid); any output pointer may be NULL.  DKD_ERR_INVALID_ARG if
+ * H, W or grid < 1. */
+int dkd_pre_padded_size(int H, int W, int grid, int* Hp, int* Wp, int* oy, int* ox);
+
+/*   src  device [B,H,W,in_channels] u8, interleaved, contiguous                       (read only)
+ *   dst  device [B,out_channels,Hp,Wp] f32|f16 planar, contiguous, 16-byte aligned
+ * Asynchronous on `stream`; one kernel launch; every element of dst is written. */
+int dkd_preprocess(dkd_ctx* ctx, const uint8_t* src, int B, int H, int W, const dkd_pre_params* p, void* dst,
+                   void* stream);
 
 /* Measurement mode (DKD_OPT_PROFILE = 1): waits for the events of the most recent dkd_extract* call
  * on this context and writes the device time of each of its kernels, in launch order, to

@@ -10,13 +10,13 @@ import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 F32, F16 = 0, 1
-OPT_USE_GRAPH, OPT_USE_TMA, OPT_PROFILE, OPT_USE_PDL, OPT_NMS_UNIT = 0, 1, 2, 3, 4
+OPT_USE_GRAPH, OPT_USE_TMA, OPT_PROFILE, OPT_USE_PDL, OPT_NMS_UNIT, OPT_ORIGIN_X, OPT_ORIGIN_Y = 0, 1, 2, 3, 4, 5, 6
 MAX_RADIUS, MAX_TOP_K, MAX_ROW_BYTES = 4, 8192, 2048
 
 EXPORTED_SYMBOLS = (
     "dkd_create", "dkd_destroy", "dkd_last_error", "dkd_workspace_bytes", "dkd_set_option",
     "dkd_extract", "dkd_extract_ex", "dkd_extract_host", "dkd_launches_per_extract", "dkd_version",
-    "dkd_profile_read", "dkd_kernel_name",
+    "dkd_profile_read", "dkd_kernel_name", "dkd_pre_padded_size", "dkd_preprocess",
 )
 
 
@@ -29,6 +29,12 @@ class DKDError(RuntimeError):
 class _CreateParams(ctypes.Structure):
     _fields_ = [("device", ctypes.c_int), ("max_batch", ctypes.c_int), ("max_h", ctypes.c_int),
                 ("max_w", ctypes.c_int), ("max_top_k", ctypes.c_int), ("max_dim", ctypes.c_int)]
+
+
+class _PreParams(ctypes.Structure):
+    _fields_ = [("in_channels", ctypes.c_int), ("out_channels", ctypes.c_int), ("grid", ctypes.c_int),
+                ("bgr", ctypes.c_int), ("out_dtype", ctypes.c_int), ("scale", ctypes.c_float),
+                ("mean", ctypes.c_float * 3), ("inv_std", ctypes.c_float * 3), ("pad_value", ctypes.c_float)]
 
 
 def lib_path() -> str:
@@ -66,6 +72,11 @@ def load_library():
     L.dkd_profile_read.argtypes = [vp, ctypes.POINTER(ctypes.c_float), i]
     L.dkd_kernel_name.restype = ctypes.c_char_p
     L.dkd_kernel_name.argtypes = [i]
+    ip = ctypes.POINTER(ctypes.c_int)
+    L.dkd_pre_padded_size.restype = i
+    L.dkd_pre_padded_size.argtypes = [i, i, i, ip, ip, ip, ip]
+    L.dkd_preprocess.restype = i
+    L.dkd_preprocess.argtypes = [vp, vp, i, i, i, ctypes.POINTER(_PreParams), vp, vp]
     common = [vp, vp, i, i, i, vp, i, i, i, i, i, i, f, i, f, vp, vp, vp, vp]
     L.dkd_extract.restype = i
     L.dkd_extract.argtypes = common + [vp]
@@ -150,6 +161,33 @@ class DKD:
         if n < 0:
             self._check(n)
         return {self._L.dkd_kernel_name(j).decode(): float(buf[j]) for j in range(n)}
+
+    # -- fused input pre-processing (dkd_pre_padded_size / dkd_preprocess) ---------------------
+    @staticmethod
+    def padded_size(H: int, W: int, grid: int):
+        """(Hp, Wp, oy, ox) of dkd_pre_padded_size."""
+        v = [ctypes.c_int() for _ in range(4)]
+        rc = load_library().dkd_pre_padded_size(H, W, grid, *[ctypes.byref(x) for x in v])
+        if rc != 0:
+            raise DKDError(rc, "dkd_pre_padded_size: H, W, grid must be >= 1")
+        return tuple(x.value for x in v)
+
+    def preprocess(self, src: torch.Tensor, out_channels: int, grid: int, bgr=False, scale=1.0 / 255.0,
+                   mean=(0.0, 0.0, 0.0), inv_std=(1.0, 1.0, 1.0), pad_value=0.0, out_dtype=torch.float32,
+                   out: Optional[torch.Tensor] = None, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+        """src [B,H,W,Cin] u8 cuda contiguous -> [B,out_channels,Hp,Wp] f32|f16 (dkd_preprocess)."""
+        if not (src.is_cuda and src.is_contiguous() and src.dtype == torch.uint8 and src.dim() == 4):
+            raise DKDError(-1, "src must be a contiguous CUDA uint8 [B,H,W,C] tensor")
+        B, H, W, Cin = src.shape
+        Hp, Wp, _, _ = self.padded_size(H, W, grid)
+        if out is None:
+            out = torch.empty((B, out_channels, Hp, Wp), dtype=out_dtype, device=src.device)
+        p = _PreParams(Cin, int(out_channels), int(grid), int(bool(bgr)), _dt(out), float(scale),
+                       (ctypes.c_float * 3)(*mean), (ctypes.c_float * 3)(*inv_std), float(pad_value))
+        st = torch.cuda.current_stream(self.device) if stream is None else stream
+        self._check(self._L.dkd_preprocess(self._h, _ptr(src), B, H, W, ctypes.byref(p), _ptr(out),
+                                           ctypes.c_void_p(st.cuda_stream)))
+        return out
 
     # -- device buffers ---------------------------------------------------------------------
     def alloc_outputs(self, B: int, top_k: int, desc: Optional[torch.Tensor], D: int = 0,

@@ -36,6 +36,7 @@ struct ExtractArgs {                       // everything that determines the enq
     int32_t* out_index;
     float* out_offset;
     int use_tma;
+    int origin_x, origin_y;                // letterbox offset subtracted from the keypoint coordinates
 };
 
 struct GraphEntry {
@@ -67,7 +68,7 @@ struct dkd_ctx {
     void* st_out;   size_t st_out_bytes;
     const void* st_desc_src; size_t st_desc_src_bytes;      // what st_desc currently holds
     // options
-    int use_graph, use_tma, use_pdl, profile, nms_cpu;
+    int use_graph, use_tma, use_pdl, profile, nms_cpu, origin_x, origin_y;
     cudaEvent_t prof_ev[MAX_KERNELS + 1];                   // measurement mode: event before/after every kernel
     int prof_n;                                             // kernels of the last profiled call (0: none)
     std::vector<GraphEntry> graphs;
@@ -211,6 +212,7 @@ cudaError_t launch_rg(const ExtractArgs& a, const int32_t* sel, cudaStream_t st,
     p.sel_idx = sel; p.top_k = a.top_k; p.r = a.r;
     p.kscale = static_cast<float>(1.4426950408889634 / static_cast<double>(a.T));
     p.out_kpts = a.out_kpts; p.out_scores = a.out_scores; p.out_off = a.out_offset;
+    p.origin_x = a.origin_x; p.origin_y = a.origin_y;
     if (a.desc == nullptr) return launch_rg_g<-1, 8>(p, a.B, st, pdl);
     const size_t esz = a.desc_dtype == DKD_F16 ? 2 : 4;
     p.desc = static_cast<const unsigned char*>(a.desc);
@@ -290,6 +292,7 @@ bool same_key(const ExtractArgs& x, const ExtractArgs& y) { return memcmp(&x, &y
 int run(dkd_ctx* ctx, ExtractArgs a, cudaStream_t st) {
     int rc = validate(ctx, a);
     if (rc != DKD_OK) return rc;
+    a.origin_x = ctx->origin_x; a.origin_y = ctx->origin_y;
     a.use_tma = ctx->use_tma && ctx->encode && (a.W % 4 == 0) && ((reinterpret_cast<uintptr_t>(a.score) & 15) == 0);
 
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
@@ -352,6 +355,17 @@ int grow(dkd_ctx* ctx, void** buf, size_t* have, size_t need) {
     return DKD_OK;
 }
 
+template <int CIN, int COUT, int DT>
+cudaError_t launch_pre(PreParams& q, cudaStream_t st) {
+    const bool vec = q.Wp % 8 == 0;
+    const int V = vec ? 8 : 1;
+    q.groups = static_cast<long long>(q.B) * q.Hp * ((q.Wp + V - 1) / V);
+    const unsigned grid = static_cast<unsigned>((q.groups + 255) / 256);
+    if (vec) k_preprocess<CIN, COUT, DT, 8><<<grid, 256, 0, st>>>(q);
+    else k_preprocess<CIN, COUT, DT, 1><<<grid, 256, 0, st>>>(q);
+    return cudaGetLastError();
+}
+
 size_t align256(size_t x) { return (x + 255) & ~static_cast<size_t>(255); }
 
 // device address of a pinned, mapped host buffer (cudaHostAlloc / cudaHostRegister); NULL for pageable memory
@@ -389,6 +403,7 @@ int dkd_create(const dkd_create_params* p, dkd_ctx** out) {
     ctx->use_tma = 1;
     ctx->use_pdl = 1;
     ctx->nms_cpu = 0;
+    ctx->origin_x = ctx->origin_y = 0;
     ctx->err[0] = 0;
     ctx->tick = 0;
 #define CKC(call)                                                                                        \
@@ -464,6 +479,8 @@ int dkd_set_option(dkd_ctx* ctx, int option, int value) {
             if (option == DKD_OPT_USE_PDL) ctx->use_pdl = value != 0;
             else ctx->nms_cpu = value > 0 ? value : 0;
             return DKD_OK;
+        case DKD_OPT_ORIGIN_X: ctx->origin_x = value; return DKD_OK;   // (part of the graph-cache key)
+        case DKD_OPT_ORIGIN_Y: ctx->origin_y = value; return DKD_OK;
         default: return fail(ctx, DKD_ERR_INVALID_ARG, "unknown option");
     }
 }
@@ -482,6 +499,54 @@ int dkd_profile_read(dkd_ctx* ctx, float* ms, int n) {
     CK(ctx, cudaEventSynchronize(ctx->prof_ev[ctx->prof_n]));
     for (int i = 0; i < ctx->prof_n && i < n; ++i) CK(ctx, cudaEventElapsedTime(&ms[i], ctx->prof_ev[i], ctx->prof_ev[i + 1]));
     return ctx->prof_n;
+}
+
+int dkd_pre_padded_size(int H, int W, int grid, int* Hp, int* Wp, int* oy, int* ox) {
+    if (H < 1 || W < 1 || grid < 1) return DKD_ERR_INVALID_ARG;
+    const int hp = (H + grid - 1) / grid * grid, wp = (W + grid - 1) / grid * grid;
+    if (Hp) *Hp = hp;
+    if (Wp) *Wp = wp;
+    if (oy) *oy = (hp - H) / 2;
+    if (ox) *ox = (wp - W) / 2;
+    return DKD_OK;
+}
+
+int dkd_preprocess(dkd_ctx* ctx, const uint8_t* src, int B, int H, int W, const dkd_pre_params* p, void* dst,
+                   void* stream) {
+    if (!ctx) return DKD_ERR_INVALID_ARG;
+    if (!src || !dst || !p || B < 1 || H < 1 || W < 1) return fail(ctx, DKD_ERR_INVALID_ARG, "NULL pointer or size < 1");
+    if (p->grid < 1) return fail(ctx, DKD_ERR_INVALID_ARG, "grid must be >= 1");
+    if ((p->in_channels != 1 && p->in_channels != 3) || (p->out_channels != 1 && p->out_channels != 3))
+        return fail(ctx, DKD_ERR_UNSUPPORTED, "in_channels and out_channels must be 1 or 3");
+    if (p->out_dtype != DKD_F32 && p->out_dtype != DKD_F16) return fail(ctx, DKD_ERR_UNSUPPORTED, "out_dtype must be DKD_F32 or DKD_F16");
+    if (reinterpret_cast<uintptr_t>(dst) & 15) return fail(ctx, DKD_ERR_UNSUPPORTED, "dst not 16-byte aligned");
+    PreParams q;
+    memset(&q, 0, sizeof(q));
+    q.src = src; q.dst = static_cast<unsigned char*>(dst);
+    q.B = B; q.H = H; q.W = W;
+    dkd_pre_padded_size(H, W, p->grid, &q.Hp, &q.Wp, &q.oy, &q.ox);
+    if (static_cast<long long>(B) * q.Hp * q.Wp > (1ll << 40)) return fail(ctx, DKD_ERR_UNSUPPORTED, "output too large");
+    q.bgr = p->bgr != 0;
+    for (int c = 0; c < 3; ++c) {
+        q.a[c] = static_cast<float>(static_cast<double>(p->scale) * static_cast<double>(p->inv_std[c]));
+        q.b[c] = static_cast<float>(-static_cast<double>(p->mean[c]) * static_cast<double>(p->inv_std[c]));
+    }
+    q.pad = p->pad_value;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    cudaError_t e;
+    const int key = (p->in_channels == 3) * 4 + (p->out_channels == 3) * 2 + (p->out_dtype == DKD_F16);
+    switch (key) {
+        case 0: e = launch_pre<1, 1, DKD_F32>(q, st); break;
+        case 1: e = launch_pre<1, 1, DKD_F16>(q, st); break;
+        case 2: e = launch_pre<1, 3, DKD_F32>(q, st); break;
+        case 3: e = launch_pre<1, 3, DKD_F16>(q, st); break;
+        case 4: e = launch_pre<3, 1, DKD_F32>(q, st); break;
+        case 5: e = launch_pre<3, 1, DKD_F16>(q, st); break;
+        case 6: e = launch_pre<3, 3, DKD_F32>(q, st); break;
+        default: e = launch_pre<3, 3, DKD_F16>(q, st); break;
+    }
+    if (e != cudaSuccess) return fail_cuda(ctx, "k_preprocess launch", e);
+    return DKD_OK;
 }
 
 int dkd_extract_ex(dkd_ctx* ctx, const float* score, int B, int H, int W, const void* desc, int desc_dtype, int Hd,

@@ -821,6 +821,7 @@ struct RGParams {
     float* out_scores;
     float* out_off;
     unsigned char* out_desc;
+    int origin_x, origin_y;             // letterbox offset subtracted from the stored coordinates
 };
 
 // DT: DKD_F32 / DKD_F16 descriptor maps, or -1 for keypoints only.  G: lanes per keypoint.
@@ -880,7 +881,7 @@ __global__ void __launch_bounds__(RG_THREADS, 6) k_refine_gather(const __grid_co
     const float inv_z = __frcp_rn(z);                        // z >= 1 (the centre weight is exactly 1)
     const float dx = sx * inv_z, dy = sy * inv_z;
     if (gl == 0) {
-        *reinterpret_cast<float2*>(p.out_kpts + 2 * slot) = make_float2(static_cast<float>(x) + dx, static_cast<float>(y) + dy);
+        *reinterpret_cast<float2*>(p.out_kpts + 2 * slot) = make_float2(static_cast<float>(x - p.origin_x) + dx, static_cast<float>(y - p.origin_y) + dy);
         p.out_scores[slot] = c;                              // raw S at the integer peak (G7)
         if (p.out_off != nullptr) *reinterpret_cast<float2*>(p.out_off + 2 * slot) = make_float2(dx, dy);
     }
@@ -936,6 +937,82 @@ __global__ void __launch_bounds__(RG_THREADS, 6) k_refine_gather(const __grid_co
                 for (int e = 0; e < N; ++e) f[e] = acc[it][e] * inv;
                 o[ch] = float_to_chunk<DT >= 0 ? DT : 0>(f);
             }
+        }
+    }
+}
+
+// ---- k_preprocess: fused letterbox + colour conversion + normalisation + NCHW packing -------------------
+// (P1..P7.)  HBM-bound, write-dominated: one thread produces VEC consecutive
+// output columns of one padded row for EVERY output channel, so each source pixel is read once;
+// VEC = 8 -> 32-byte (f32) / 16-byte (f16) stores per plane.  Padding pixels get pad_value.
+struct PreParams {
+    const uint8_t* src;
+    unsigned char* dst;
+    int B, H, W, Hp, Wp, oy, ox;
+    int bgr;
+    float a[3], b[3];        // out = value * a[c] + b[c],  a = scale * inv_std, b = -mean * inv_std
+    float pad;
+    long long groups;        // B * Hp * ceil(Wp / VEC)
+};
+
+template <int CIN, int COUT, int DT, int VEC>
+__global__ void __launch_bounds__(256) k_preprocess(const __grid_constant__ PreParams p) {
+    const long long g = blockIdx.x * 256ll + threadIdx.x;
+    if (g >= p.groups) return;
+    const int gpr = (p.Wp + VEC - 1) / VEC;                  // groups per padded row
+    const int xg = static_cast<int>(g % gpr);
+    const long long row = g / gpr;
+    const int yp = static_cast<int>(row % p.Hp), b = static_cast<int>(row / p.Hp);
+    const int xp0 = xg * VEC, y = yp - p.oy;
+    float v[COUT][VEC];
+#pragma unroll
+    for (int i = 0; i < VEC; ++i) {
+        const int x = xp0 + i - p.ox;
+        const bool in = y >= 0 && y < p.H && x >= 0 && x < p.W;
+        float val[COUT];
+        if (in) {
+            const uint8_t* px = p.src + ((static_cast<size_t>(b) * p.H + y) * p.W + x) * CIN;
+            if constexpr (CIN == 1) {
+                const float m = static_cast<float>(__ldg(px));
+#pragma unroll
+                for (int c = 0; c < COUT; ++c) val[c] = fmaf(m, p.a[c], p.b[c]);
+            } else {
+                const float c0 = static_cast<float>(__ldg(px)), c1 = static_cast<float>(__ldg(px + 1));
+                const float c2 = static_cast<float>(__ldg(px + 2));
+                const float R = p.bgr ? c2 : c0, Bl = p.bgr ? c0 : c2;
+                if constexpr (COUT == 1) {
+                    val[0] = fmaf(fmaf(0.299f, R, fmaf(0.587f, c1, 0.114f * Bl)), p.a[0], p.b[0]);
+                } else {
+                    val[0] = fmaf(R, p.a[0], p.b[0]);
+                    val[1] = fmaf(c1, p.a[1], p.b[1]);
+                    val[2] = fmaf(Bl, p.a[2], p.b[2]);
+                }
+            }
+        } else {
+#pragma unroll
+            for (int c = 0; c < COUT; ++c) val[c] = p.pad;
+        }
+#pragma unroll
+        for (int c = 0; c < COUT; ++c) v[c][i] = val[c];
+    }
+    constexpr int ESZ = DT == DKD_F16 ? 2 : 4;
+#pragma unroll
+    for (int c = 0; c < COUT; ++c) {
+        unsigned char* o = p.dst + (((static_cast<size_t>(b) * COUT + c) * p.Hp + yp) * p.Wp + xp0) * ESZ;
+        if constexpr (VEC == 8) {                            // Wp % 8 == 0: aligned vector stores
+            if constexpr (DT == DKD_F16) {
+                uint4 q;
+                __half2* h = reinterpret_cast<__half2*>(&q);
+#pragma unroll
+                for (int i = 0; i < 4; ++i) h[i] = __floats2half2_rn(v[c][2 * i], v[c][2 * i + 1]);
+                *reinterpret_cast<uint4*>(o) = q;
+            } else {
+                reinterpret_cast<float4*>(o)[0] = make_float4(v[c][0], v[c][1], v[c][2], v[c][3]);
+                reinterpret_cast<float4*>(o)[1] = make_float4(v[c][4], v[c][5], v[c][6], v[c][7]);
+            }
+        } else {
+            if constexpr (DT == DKD_F16) *reinterpret_cast<__half*>(o) = __float2half_rn(v[c][0]);
+            else *reinterpret_cast<float*>(o) = v[c][0];
         }
     }
 }
