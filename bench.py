@@ -53,9 +53,10 @@ def parse_args():
     ap.add_argument("--batch64-steps", type=int, default=30)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=0, help="0 = min(steps, 100)")
-    ap.add_argument("--leg", default="all", choices=["all", "c2", "c5"],
+    ap.add_argument("--leg", default="all", choices=["all", "c2", "c5", "pre"],
                     help="profiling aid: c5 = shortest possible c2 legs (13 c2 launches) then the batch-64 leg; "
-                         "c2 = no batch-64 leg.  The driver's bench line is --leg all.")
+                         "c2 = no batch-64 leg; pre = shortest c2 legs, then only the pre-processing kernel.  "
+                         "The driver's bench line is --leg all.")
     return ap.parse_args()
 
 
@@ -238,8 +239,10 @@ def run_ours(args):
     sampler = ClockSampler(local)
     cfg = synth.CONFIGS["c2"]
     esz = 2 if cfg.desc_dtype == "f16" else 4
-    if args.leg == "c5":
+    if args.leg in ("c5", "pre"):
         args.sets, args.steps, args.warmup, args.e2e_steps, args.no_cpu_baseline = 1, 1, 3, 1, True
+    if args.leg == "pre":
+        args.no_batch64 = True
     if args.leg == "c2":
         args.no_batch64 = True
     R = max(1, args.sets)
@@ -281,7 +284,7 @@ def run_ours(args):
 
     # single-shot latency (enqueue -> outputs complete), one pair at a time
     lat = []
-    for i in range(min(200, max(K, 20)) if args.leg != "c5" else 1):
+    for i in range(min(200, max(K, 20)) if args.leg not in ("c5", "pre") else 1):
         torch.cuda.synchronize()
         t0 = time.perf_counter()
         calls[i % R]()
@@ -291,7 +294,7 @@ def run_ours(args):
 
     # the same steps as plain stream launches (DKD_OPT_USE_GRAPH = 0: three PDL-linked launches per step)
     stream_us = None
-    if args.leg != "c5":
+    if args.leg not in ("c5", "pre"):
         ctx.set_option(OPT_USE_GRAPH, 0)
         for i in range(Wm):
             calls[i % R]()
@@ -309,7 +312,7 @@ def run_ours(args):
     # per-kernel device time at c2 (library measurement mode: plain launches + events)
     ctx.set_option(OPT_PROFILE, 1)
     kt2 = {}
-    nprof = 50 if args.leg != "c5" else 0
+    nprof = 50 if args.leg not in ("c5", "pre") else 0
     for i in range(nprof + 5 if nprof else 0):
         calls[i % R]()
         d = ctx.profile_read()
@@ -420,6 +423,50 @@ def run_ours(args):
             ctx5.close()
             torch.cuda.empty_cache()
 
+    # ---- fused input pre-processing kernel: stereo pair + batch 64 ----
+    pre = None
+    if args.leg in ("all", "pre"):
+        pre = {}
+        ctxp = dkd.DKD(2, 64, 64, 16, 0, device=local)
+        for name, (Bp, Hq, Wq, dt, n_it) in {"stereo_752x480_mono_to_3ch_f32_grid32": (2, 480, 752, torch.float32, 200),
+                                               "batch64_1920x1080_mono_to_3ch_f16_grid32": (64, 1080, 1920, torch.float16, 20)}.items():
+            srcs = [torch.randint(0, 256, (Bp, Hq, Wq, 1), dtype=torch.uint8, device=dev) for _ in range(2 if Bp > 2 else 32)]
+            Hp, Wp, _, _ = ctxp.padded_size(Hq, Wq, 32)
+            outs = [torch.empty((Bp, 3, Hp, Wp), dtype=dt, device=dev) for _ in range(len(srcs))]
+            kw = dict(mean=(0.485, 0.456, 0.406), inv_std=(4.367, 4.464, 4.444))
+            for j in range(len(srcs)):
+                ctxp.preprocess(srcs[j], 3, 32, out=outs[j], **kw)
+            torch.cuda.synchronize()
+            if Bp <= 2:                                          # launch-bound size: replay the launches from one
+                gph = torch.cuda.CUDAGraph()                     # captured graph so that Python is not what is timed
+                cs = torch.cuda.Stream(device=dev)
+                with torch.cuda.stream(cs), torch.cuda.graph(gph, stream=cs):
+                    for j in range(len(srcs)):
+                        ctxp.preprocess(srcs[j], 3, 32, out=outs[j], stream=cs, **kw)
+                gph.replay()
+                torch.cuda.synchronize()
+                reps = max(n_it // len(srcs), 1)
+                ev0.record(stream)
+                for _ in range(reps):
+                    gph.replay()
+                ev1.record(stream)
+                torch.cuda.synchronize()
+                us = ev0.elapsed_time(ev1) * 1e3 / (reps * len(srcs))
+            else:
+                ev0.record(stream)
+                for i in range(n_it):
+                    j = i % len(srcs)
+                    ctxp.preprocess(srcs[j], 3, 32, out=outs[j], **kw)
+                ev1.record(stream)
+                torch.cuda.synchronize()
+                us = ev0.elapsed_time(ev1) * 1e3 / n_it
+            nbytes = Bp * Hq * Wq + Bp * 3 * Hp * Wp * outs[0].element_size()
+            pre[name] = {"us": us, "algorithmic_bytes": nbytes, "gbs": nbytes / us / 1e3, "frac_of_hbm_peak": nbytes / us / 1e3 / hbm_peak,
+                         "l2": f"rotates through {len(srcs)} buffer sets ({len(srcs) * nbytes / 1e6:.0f} MB)"}
+            del srcs, outs
+        ctxp.close()
+        torch.cuda.empty_cache()
+
     # ---- CPU baseline: the oracle as it stands, on this box's host cores (rank 0, N = 1) -----------
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -466,7 +513,7 @@ def run_ours(args):
                                   "d2h_bytes_per_step": d2h,
                                   "what": "same, descriptor map left on the device by the previous call (network output)"},
             "gpu_launches": K * 3,
-            "batch64": b64, "roofline": roof, "cpu_baseline": cpu,
+            "batch64": b64, "roofline": roof, "cpu_baseline": cpu, "preprocess": pre,
             "context": "paper: whole pipeline 29-47 FPS mono / 18-33 FPS stereo on Jetson AGX Orin (PAPER.md:5) — other hardware, whole system",
         }
         print(json.dumps(line), flush=True)

@@ -359,8 +359,8 @@ template <int CIN, int COUT, int DT>
 cudaError_t launch_pre(PreParams& q, cudaStream_t st) {
     const bool vec = q.Wp % 8 == 0;
     const int V = vec ? 8 : 1;
-    q.groups = static_cast<long long>(q.B) * q.Hp * ((q.Wp + V - 1) / V);
-    const unsigned grid = static_cast<unsigned>((q.groups + 255) / 256);
+    q.gpr = (q.Wp + V - 1) / V;
+    const dim3 grid((q.gpr + 255) / 256, q.Hp, q.B);
     if (vec) k_preprocess<CIN, COUT, DT, 8><<<grid, 256, 0, st>>>(q);
     else k_preprocess<CIN, COUT, DT, 1><<<grid, 256, 0, st>>>(q);
     return cudaGetLastError();
@@ -525,7 +525,7 @@ int dkd_preprocess(dkd_ctx* ctx, const uint8_t* src, int B, int H, int W, const 
     q.src = src; q.dst = static_cast<unsigned char*>(dst);
     q.B = B; q.H = H; q.W = W;
     dkd_pre_padded_size(H, W, p->grid, &q.Hp, &q.Wp, &q.oy, &q.ox);
-    if (static_cast<long long>(B) * q.Hp * q.Wp > (1ll << 40)) return fail(ctx, DKD_ERR_UNSUPPORTED, "output too large");
+    if (B > 65535 || q.Hp > 65535) return fail(ctx, DKD_ERR_UNSUPPORTED, "B and the padded height must be <= 65535");
     q.bgr = p->bgr != 0;
     for (int c = 0; c < 3; ++c) {
         q.a[c] = static_cast<float>(static_cast<double>(p->scale) * static_cast<double>(p->inv_std[c]));

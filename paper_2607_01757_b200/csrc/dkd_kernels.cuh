@@ -952,48 +952,66 @@ struct PreParams {
     int bgr;
     float a[3], b[3];        // out = value * a[c] + b[c],  a = scale * inv_std, b = -mean * inv_std
     float pad;
-    long long groups;        // B * Hp * ceil(Wp / VEC)
+    int gpr;                 // groups per padded row = ceil(Wp / VEC)
 };
 
 template <int CIN, int COUT, int DT, int VEC>
 __global__ void __launch_bounds__(256) k_preprocess(const __grid_constant__ PreParams p) {
-    const long long g = blockIdx.x * 256ll + threadIdx.x;
-    if (g >= p.groups) return;
-    const int gpr = (p.Wp + VEC - 1) / VEC;                  // groups per padded row
-    const int xg = static_cast<int>(g % gpr);
-    const long long row = g / gpr;
-    const int yp = static_cast<int>(row % p.Hp), b = static_cast<int>(row / p.Hp);
+    // grid = (ceil(groups per row / 256), Hp, B): no index division
+    const int xg = blockIdx.x * 256 + threadIdx.x;
+    if (xg >= p.gpr) return;
+    const int yp = blockIdx.y, b = blockIdx.z;
     const int xp0 = xg * VEC, y = yp - p.oy;
     float v[COUT][VEC];
+    const bool row_in = y >= 0 && y < p.H;
+    const int x0 = xp0 - p.ox;                               // source column of the group's first pixel
+    // one pixel: 8-bit channel values -> COUT normalised outputs
+    auto convert = [&](float c0, float c1, float c2, int i) {
+        if constexpr (CIN == 1) {
 #pragma unroll
-    for (int i = 0; i < VEC; ++i) {
-        const int x = xp0 + i - p.ox;
-        const bool in = y >= 0 && y < p.H && x >= 0 && x < p.W;
-        float val[COUT];
-        if (in) {
-            const uint8_t* px = p.src + ((static_cast<size_t>(b) * p.H + y) * p.W + x) * CIN;
-            if constexpr (CIN == 1) {
-                const float m = static_cast<float>(__ldg(px));
-#pragma unroll
-                for (int c = 0; c < COUT; ++c) val[c] = fmaf(m, p.a[c], p.b[c]);
+            for (int c = 0; c < COUT; ++c) v[c][i] = fmaf(c0, p.a[c], p.b[c]);
+        } else {
+            const float R = p.bgr ? c2 : c0, Bl = p.bgr ? c0 : c2;
+            if constexpr (COUT == 1) {
+                v[0][i] = fmaf(fmaf(0.299f, R, fmaf(0.587f, c1, 0.114f * Bl)), p.a[0], p.b[0]);
             } else {
-                const float c0 = static_cast<float>(__ldg(px)), c1 = static_cast<float>(__ldg(px + 1));
-                const float c2 = static_cast<float>(__ldg(px + 2));
-                const float R = p.bgr ? c2 : c0, Bl = p.bgr ? c0 : c2;
-                if constexpr (COUT == 1) {
-                    val[0] = fmaf(fmaf(0.299f, R, fmaf(0.587f, c1, 0.114f * Bl)), p.a[0], p.b[0]);
-                } else {
-                    val[0] = fmaf(R, p.a[0], p.b[0]);
-                    val[1] = fmaf(c1, p.a[1], p.b[1]);
-                    val[2] = fmaf(Bl, p.a[2], p.b[2]);
-                }
+                v[0][i] = fmaf(R, p.a[0], p.b[0]);
+                v[1][i] = fmaf(c1, p.a[1], p.b[1]);
+                v[2][i] = fmaf(Bl, p.a[2], p.b[2]);
+            }
+        }
+    };
+    if (row_in && x0 >= 0 && x0 + VEC <= p.W) {              // interior group: no per-pixel test, one row pointer
+        const uint8_t* q = p.src + ((static_cast<size_t>(b) * p.H + y) * p.W + x0) * CIN;
+        constexpr int NB = VEC * CIN;
+        uint8_t raw[NB];
+        if (NB % 4 == 0 && (reinterpret_cast<uintptr_t>(q) & 3) == 0) {      // (uniform along a row)
+#pragma unroll
+            for (int w = 0; w < NB / 4; ++w) {
+                const uint32_t u = __ldg(reinterpret_cast<const uint32_t*>(q) + w);
+                raw[4 * w] = u & 0xff; raw[4 * w + 1] = (u >> 8) & 0xff; raw[4 * w + 2] = (u >> 16) & 0xff; raw[4 * w + 3] = u >> 24;
             }
         } else {
 #pragma unroll
-            for (int c = 0; c < COUT; ++c) val[c] = p.pad;
+            for (int k = 0; k < NB; ++k) raw[k] = __ldg(q + k);
         }
 #pragma unroll
-        for (int c = 0; c < COUT; ++c) v[c][i] = val[c];
+        for (int i = 0; i < VEC; ++i)
+            convert(static_cast<float>(raw[i * CIN]), CIN == 3 ? static_cast<float>(raw[i * CIN + (CIN == 3 ? 1 : 0)]) : 0.0f,
+                    CIN == 3 ? static_cast<float>(raw[i * CIN + (CIN == 3 ? 2 : 0)]) : 0.0f, i);
+    } else {                                                 // padding rows / groups straddling the image edge
+#pragma unroll
+        for (int i = 0; i < VEC; ++i) {
+            const int x = x0 + i;
+            if (row_in && x >= 0 && x < p.W) {
+                const uint8_t* px = p.src + ((static_cast<size_t>(b) * p.H + y) * p.W + x) * CIN;
+                convert(static_cast<float>(__ldg(px)), CIN == 3 ? static_cast<float>(__ldg(px + (CIN == 3 ? 1 : 0))) : 0.0f,
+                        CIN == 3 ? static_cast<float>(__ldg(px + (CIN == 3 ? 2 : 0))) : 0.0f, i);
+            } else {
+#pragma unroll
+                for (int c = 0; c < COUT; ++c) v[c][i] = p.pad;
+            }
+        }
     }
     constexpr int ESZ = DT == DKD_F16 ? 2 : 4;
 #pragma unroll
@@ -1005,10 +1023,10 @@ __global__ void __launch_bounds__(256) k_preprocess(const __grid_constant__ PreP
                 __half2* h = reinterpret_cast<__half2*>(&q);
 #pragma unroll
                 for (int i = 0; i < 4; ++i) h[i] = __floats2half2_rn(v[c][2 * i], v[c][2 * i + 1]);
-                *reinterpret_cast<uint4*>(o) = q;
+                __stcs(reinterpret_cast<uint4*>(o), q);      // streaming stores: written once, read by the network later
             } else {
-                reinterpret_cast<float4*>(o)[0] = make_float4(v[c][0], v[c][1], v[c][2], v[c][3]);
-                reinterpret_cast<float4*>(o)[1] = make_float4(v[c][4], v[c][5], v[c][6], v[c][7]);
+                __stcs(reinterpret_cast<float4*>(o), make_float4(v[c][0], v[c][1], v[c][2], v[c][3]));
+                __stcs(reinterpret_cast<float4*>(o) + 1, make_float4(v[c][4], v[c][5], v[c][6], v[c][7]));
             }
         } else {
             if constexpr (DT == DKD_F16) *reinterpret_cast<__half*>(o) = __float2half_rn(v[c][0]);
