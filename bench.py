@@ -292,6 +292,26 @@ def run_ours(args):
         lat.append((time.perf_counter() - t0) * 1e6)
     lat.sort()
 
+    # the paper's keypoint-cap sweep (caps 160 / 192 / 256 / 384, DKD runtime minimum at
+    # 256 with its fixed 64-thread blocks): same c2 stereo pair, one graph launch per step, cap = top_k
+    cap_sweep = None
+    if args.leg == "all":
+        cap_sweep = {}
+        sd0, desc0 = sets[0][0], sets[0][1]
+        for cap in (160, 192, 256, 384):
+            outc = ctx.alloc_outputs(cfg.B, cap, desc0, cfg.D, want_index=False, want_offsets=False)
+            fc = ctx.bind(sd0, desc0, cfg.stride, cfg.r, cfg.thresh, cap, cfg.T, outc, stream)
+            for _ in range(20):
+                fc()
+            torch.cuda.synchronize()
+            ev0.record(stream)
+            for _ in range(500):
+                fc()
+            ev1.record(stream)
+            torch.cuda.synchronize()
+            cap_sweep[str(cap)] = ev0.elapsed_time(ev1) * 1e3 / 500
+        cap_sweep["what"] = "us per 752x480 stereo pair vs keypoint cap (warm inputs: one input set)"
+
     # the same steps as plain stream launches (DKD_OPT_USE_GRAPH = 0: three PDL-linked launches per step)
     stream_us = None
     if args.leg not in ("c5", "pre"):
@@ -513,7 +533,7 @@ def run_ours(args):
                                   "d2h_bytes_per_step": d2h,
                                   "what": "same, descriptor map left on the device by the previous call (network output)"},
             "gpu_launches": K * 3,
-            "batch64": b64, "roofline": roof, "cpu_baseline": cpu, "preprocess": pre,
+            "batch64": b64, "roofline": roof, "cpu_baseline": cpu, "preprocess": pre, "cap_sweep": cap_sweep,
             "context": "paper: whole pipeline 29-47 FPS mono / 18-33 FPS stereo on Jetson AGX Orin (PAPER.md:5) — other hardware, whole system",
         }
         print(json.dumps(line), flush=True)
