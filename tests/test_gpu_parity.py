@@ -168,6 +168,27 @@ def test_config_c5_full_size_sampled():
         c.close()
 
 
+# ---- larger shapes than the configs: 4K frames, the plain loader at scale, the largest cap -------------
+@pytest.mark.parametrize("case", ["4k_r4_k8192_d256_s8", "plain_1081x1923", "tall_narrow", "d1024_f16"])
+def test_large_and_odd_shapes(case):
+    import paper_2607_01757_b200 as dkd
+    B, H, W, r, thresh, k, T, D, dtype, stride, base, blobs = {
+        "4k_r4_k8192_d256_s8": (2, 2160, 3840, 4, 0.05, 8192, 0.1, 256, torch.float16, 8, 0.05, 20000),
+        "plain_1081x1923": (2, 1081, 1923, 2, 0.2, 2048, 0.1, 64, torch.float32, 1, 0.1, 4000),
+        "tall_narrow": (3, 4000, 132, 3, 0.2, 1024, 0.05, 128, torch.float16, 2, 0.1, 3000),
+        "d1024_f16": (1, 300, 500, 2, 0.2, 512, 0.1, 1024, torch.float16, 4, 0.1, 800),
+    }[case]
+    c = dkd.DKD(B, H, W, k, D)
+    try:
+        score = synth.score_maps(B, H, W, 99, base, blobs)
+        desc = synth.desc_maps(B, H // stride, W // stride, D, 99, dtype, "cuda")
+        res, ref = run_both(c, score, desc, stride, r, thresh, k, T)
+        st = compare(res, ref, dtype)
+        assert ref.count.min() > 500 and st["max_offset_err"] <= 1e-5
+    finally:
+        c.close()
+
+
 # ---- degenerate and adversarial inputs -----------------------------------------------------------
 def test_no_candidates_and_tiny_images(ctx):
     score = torch.full((2, 40, 140), 0.1)
