@@ -242,9 +242,11 @@ cudaError_t enqueue(dkd_ctx* ctx, const ExtractArgs& a, cudaStream_t st, bool pr
     if (e != cudaSuccess) return e;
     if ((e = mark()) != cudaSuccess) return e;
     int32_t* sel = a.out_index ? a.out_index : ctx->sel_idx;
+    int idx_shift = 0;                                       // (H*W - 1) >> idx_shift < NBT: index buckets of the top ties
+    while (((static_cast<long long>(a.H) * a.W - 1) >> idx_shift) >= NBT) ++idx_shift;
     const bool pdl = ctx->use_pdl && !prof;                  // (events between the kernels would serialise them anyway)
     e = launch_pdl(k_select, dim3(a.B), dim3(SEL_THREADS), SEL_SMEM_BYTES, st, pdl, ctx->cand, ctx->tile_cnt, tpi,
-                   plan.cpu * SEG_CAP, a.top_k, sel, a.out_count);
+                   plan.cpu * SEG_CAP, a.top_k, idx_shift, sel, a.out_count);
     if (e != cudaSuccess) return e;
     if ((e = mark()) != cudaSuccess) return e;
     e = launch_rg(a, sel, st, pdl);

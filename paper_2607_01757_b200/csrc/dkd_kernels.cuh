@@ -430,16 +430,19 @@ __global__ void __launch_bounds__(PLAIN_WARPS * 32) k_nms_plain(const float* __r
 //                   narrows to a lower bound `lo` with  top_k <= #{key >= lo} <= SORT_CAP; gather again,
 //                   keys >= lo only.
 //   order         : bucket rank (the common case) — one pass of a monotone bucket function over the
-//                   score bits (NB buckets spanning [min, max] of the gathered scores), an exclusive
+//                   score bits (NB buckets spanning [min, max] of the gathered scores; the keys tied at the
+//                   maximum score get NBT buckets over their pixel index instead), an exclusive
 //                   scan of the bucket counts, a scatter into bucket order, and an exact rank
 //                   = keys in better buckets + keys of the own bucket with a larger key.  ~100
 //                   lane-instructions per key instead of the ~550 of a 64-bit bitonic network.
 //                   Falls back to the in-smem bitonic sort when one bucket holds more than
 //                   BUCKET_LIMIT keys (near-constant maps).
 // Keys are unique (they embed the pixel index) so the result is the unique (score desc, idx asc) order.
-constexpr int NB = 4096;                 // buckets of the rank pass
+constexpr int NB = 4096;                 // score buckets of the rank pass
+constexpr int NBT = 1024;                // index buckets for the keys tied at the maximum score (see k_select)
+constexpr int NBK = NBT + NB;
 constexpr int BUCKET_LIMIT = 1024;       // largest bucket the rank pass accepts
-constexpr int SEL_SMEM_BYTES = 2 * SORT_CAP * 8 + 2 * NB * 4;     // keys | sorted | base | cur = 160 KB
+constexpr int SEL_SMEM_BYTES = 2 * SORT_CAP * 8 + 2 * NBK * 4;    // keys | sorted | base | cur = 168 KB
 
 __device__ __forceinline__ int block_sum_1024(int v, int* s_red) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -456,14 +459,14 @@ __device__ __forceinline__ int block_sum_1024(int v, int* s_red) {
 
 __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __restrict__ cand,
                                                            const int* __restrict__ seg_cnt, int tpi, int seg_cap,
-                                                           int top_k,
+                                                           int top_k, int idx_shift,
                                                            int32_t* __restrict__ sel_idx,
                                                            int32_t* __restrict__ out_count) {
     extern __shared__ __align__(16) unsigned char sel_smem[];
     uint64_t* keys = reinterpret_cast<uint64_t*>(sel_smem);            // SORT_CAP entries (gathered, unordered)
     uint64_t* sorted = keys + SORT_CAP;                                // SORT_CAP entries (bucket order)
-    int* base = reinterpret_cast<int*>(sorted + SORT_CAP);             // NB
-    int* cur = base + NB;                                              // NB
+    int* base = reinterpret_cast<int*>(sorted + SORT_CAP);             // NBK
+    int* cur = base + NBK;                                             // NBK
     __shared__ int s_hist[257];
     __shared__ int s_red[32];
     __shared__ int s_n, s_digit, s_cum, s_h, s_maxb;
@@ -478,7 +481,7 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
 
     pdl_launch_dependents();
     if (tid == 0) { s_n = 0; s_hi = 0u; s_lo = 0xffffffffu; s_maxb = 0; }
-    for (int i = tid; i < NB; i += SEL_THREADS) cur[i] = 0;
+    for (int i = tid; i < NBK; i += SEL_THREADS) cur[i] = 0;
     pdl_wait();                                              // the candidates of k_nms_* are complete and visible
     __syncthreads();
 
@@ -624,14 +627,21 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
     const unsigned hi = s_hi;
     const unsigned range = hi - s_lo;
     const int shift = range >= static_cast<unsigned>(NB) ? (32 - __clz(range)) - 12 : 0;   // (range >> shift) < NB
-    for (int i = tid; i < m; i += SEL_THREADS) atomicAdd(&cur[(hi - static_cast<unsigned>(keys[i] >> 32)) >> shift], 1);
+    // Monotone bucket function (a better key never gets a larger bucket).  Keys TIED at the maximum score
+    // (score maps saturate: the clamp at 1.0 ties hundreds of peaks) differ only in their index, so they
+    // are spread over NBT buckets by index; every other key goes by its score word.
+    auto bucket_of = [&](uint64_t k) -> int {
+        const unsigned kb = static_cast<unsigned>(k >> 32);
+        return kb == hi ? key_index(k) >> idx_shift : NBT + static_cast<int>((hi - kb) >> shift);
+    };
+    for (int i = tid; i < m; i += SEL_THREADS) atomicAdd(&cur[bucket_of(keys[i])], 1);
     __syncthreads();
-    {   // exclusive scan of the NB bucket counts (4 consecutive buckets per thread), largest bucket
-        int c4[NB / SEL_THREADS];
+    {   // exclusive scan of the NBK bucket counts (5 consecutive buckets per thread), largest bucket
+        int c4[NBK / SEL_THREADS];
         int sum = 0, mx = 0;
 #pragma unroll
-        for (int q = 0; q < NB / SEL_THREADS; ++q) {
-            c4[q] = cur[tid * (NB / SEL_THREADS) + q];
+        for (int q = 0; q < NBK / SEL_THREADS; ++q) {
+            c4[q] = cur[tid * (NBK / SEL_THREADS) + q];
             sum += c4[q];
             mx = c4[q] > mx ? c4[q] : mx;
         }
@@ -655,9 +665,9 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
         woff = __shfl_sync(FULL, wincl - woff, warp);
         int run = woff + incl - sum;
 #pragma unroll
-        for (int q = 0; q < NB / SEL_THREADS; ++q) {
-            base[tid * (NB / SEL_THREADS) + q] = run;
-            cur[tid * (NB / SEL_THREADS) + q] = 0;
+        for (int q = 0; q < NBK / SEL_THREADS; ++q) {
+            base[tid * (NBK / SEL_THREADS) + q] = run;
+            cur[tid * (NBK / SEL_THREADS) + q] = 0;
             run += c4[q];
         }
         __syncthreads();
@@ -665,13 +675,13 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
     if (s_maxb <= BUCKET_LIMIT) {                           // block-uniform
         for (int i = tid; i < m; i += SEL_THREADS) {        // scatter into bucket order
             const uint64_t k = keys[i];
-            const int d = (hi - static_cast<unsigned>(k >> 32)) >> shift;
+            const int d = bucket_of(k);
             sorted[base[d] + atomicAdd(&cur[d], 1)] = k;
         }
         __syncthreads();
         for (int i = tid; i < m; i += SEL_THREADS) {        // exact rank inside the own bucket
             const uint64_t k = sorted[i];
-            const int d = (hi - static_cast<unsigned>(k >> 32)) >> shift;
+            const int d = bucket_of(k);
             const int s0 = base[d], s1 = s0 + cur[d];
             int rank = s0;
             int j = s0;
