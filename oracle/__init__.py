@@ -4,9 +4,10 @@ Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline``
 ``--impl reference`` legs may import this package.  The product
 (``paper_2607_01757_b200``) never does, and this package never imports the product.
 
-The arithmetic lives in ``dkd_oracle.c`` (plain C99, fp64, naive loops; see its header for the
-passages of /root/reference/PAPER.md and the DESIGN.md readings it follows).  This file only
-compiles it with gcc and marshals numpy arrays through ctypes.
+The arithmetic lives in ``dkd_oracle.c`` (the hot path), ``dkd_variants.c`` (the DKD variants, SURVEY.md
+8(f) f2) and ``match_oracle.c`` (descriptor matching, retrieval scan, stereo validation, covariance weighting:
+f3, f4) — plain C99, fp64, naive loops; see their headers for the passages of /root/reference/PAPER.md and the
+DESIGN.md readings they follow.  This file only compiles them with gcc and marshals numpy arrays through ctypes.
 """
 from __future__ import annotations
 
@@ -18,7 +19,7 @@ from dataclasses import dataclass
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SRC = os.path.join(_HERE, "dkd_oracle.c")
+_SRCS = [os.path.join(_HERE, f) for f in ("dkd_oracle.c", "dkd_variants.c", "match_oracle.c")]
 _LIB = os.path.join(_HERE, "libdkd_oracle.so")
 
 F32, F16 = 0, 1
@@ -27,10 +28,10 @@ _lib = None
 
 def build(force: bool = False) -> str:
     """gcc -O2 -fopenmp (no -ffast-math) -> oracle/libdkd_oracle.so."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(f) for f in _SRCS):
         tmp = _LIB + f".tmp{os.getpid()}"
         subprocess.check_call(["gcc", "-O2", "-std=c99", "-fopenmp", "-shared", "-fPIC",
-                               _SRC, "-o", tmp, "-lm"])
+                               *_SRCS, "-o", tmp, "-lm"])
         os.replace(tmp, _LIB)
     return _LIB
 
@@ -54,6 +55,22 @@ def lib():
         L.dkd_oracle_extract.restype = i
         L.dkd_oracle_extract.argtypes = [vp, i, i, i, vp, i, i, i, i, i, i, f, i, f,
                                          vp, vp, vp, vp, vp, vp]
+        d = ctypes.c_double
+        L.dkd_oracle_nms_iter.restype = ctypes.c_long
+        L.dkd_oracle_nms_iter.argtypes = [vp, i, i, i, f, i, vp]
+        L.dkd_oracle_bilinear_score.restype = d
+        L.dkd_oracle_bilinear_score.argtypes = [vp, i, i, d, d]
+        L.dkd_oracle_extract_var.restype = i
+        L.dkd_oracle_extract_var.argtypes = [vp, vp, vp, i, i, i, vp, i, i, i, i, i, i, f, i, f, i, i,
+                                             vp, vp, vp, vp, vp, vp, vp]
+        L.match_oracle_nn.restype = i
+        L.match_oracle_nn.argtypes = [vp, vp, i, i, i, i, i, i, d, i, vp, vp, vp, vp]
+        L.retrieval_oracle_scan.restype = i
+        L.retrieval_oracle_scan.argtypes = [vp, vp, i, i, i, i, d, i, vp, vp]
+        L.stereo_oracle_validate.restype = i
+        L.stereo_oracle_validate.argtypes = [vp, vp, i, d, d, d, d, d, d, d, d, d, vp, vp, vp, vp]
+        L.cov_oracle_sqrt_info.restype = i
+        L.cov_oracle_sqrt_info.argtypes = [vp, i, d, d, d, d, d, d, d, vp, vp]
         _lib = L
     return _lib
 
@@ -185,3 +202,126 @@ def preprocess(src, out_channels, grid, bgr=False, scale=1.0 / 255.0, mean=(0.0,
         raise ValueError("dkd_oracle_preprocess: invalid argument")
     return out
 
+
+
+# ---- DKD variants (dkd_variants.c) ------------------------------------------------
+def nms_mask_iter(S, r, thresh, iters):
+    """V1 -> uint8 mask [H,W] of the iterated suppress-and-recover NMS (iters = 0: the single pass)."""
+    S = _c(S, np.float32)
+    H, W = S.shape
+    mask = np.zeros((H, W), np.uint8)
+    n = lib().dkd_oracle_nms_iter(_p(S), H, W, int(r), float(thresh), int(iters), _p(mask))
+    assert n == int(mask.sum())
+    return mask
+
+
+def bilinear_score(S, px, py):
+    """V2 -> S interpolated bilinearly at (px, py) (fp64)."""
+    S = _c(S, np.float32)
+    H, W = S.shape
+    return float(lib().dkd_oracle_bilinear_score(_p(S), H, W, float(px), float(py)))
+
+
+@dataclass
+class OracleVarResult(OracleResult):
+    total: np.ndarray = None   # [B] i32: candidates before the cap (V3)
+
+
+def extract_var(score, desc, stride, r, thresh, top_k, T, reliability=None, valid_mask=None, nms_iters=0,
+                score_mode=0) -> OracleVarResult:
+    """The whole path with the variants V1..V5.  `scores` is float64 (exactly the fp32 score in raw mode)."""
+    score = _c(score, np.float32)
+    B, H, W = score.shape
+    rel = None if reliability is None else _c(reliability, np.float32)
+    vm = None if valid_mask is None else _c(valid_mask, np.uint8)
+    assert rel is None or rel.shape == score.shape
+    assert vm is None or vm.shape == score.shape
+    desc, dt = _desc_arg(desc)
+    if desc is not None:
+        _, Hd, Wd, D = desc.shape
+    else:
+        Hd = Wd = D = 0
+    k = int(top_k)
+    kp = np.empty((B, k, 2), np.float64)
+    off = np.empty((B, k, 2), np.float64)
+    sc = np.empty((B, k), np.float64)
+    de = np.empty((B, k, D), np.float64) if desc is not None else None
+    cnt = np.empty(B, np.int32)
+    idx = np.empty((B, k), np.int32)
+    tot = np.empty(B, np.int32)
+    rc = lib().dkd_oracle_extract_var(_p(score), _p(rel), _p(vm), B, H, W, _p(desc), dt, Hd, Wd, D, int(stride),
+                                      int(r), float(thresh), k, float(T), int(nms_iters), int(score_mode),
+                                      _p(kp), _p(off), _p(sc), _p(de), _p(cnt), _p(idx), _p(tot))
+    if rc != 0:
+        raise ValueError("dkd_oracle_extract_var: invalid argument")
+    return OracleVarResult(kp, off, sc, de, cnt, idx, tot)
+
+
+# ---- descriptor matching / retrieval / stereo validation / covariance (f3, f4; match_oracle.c) -----------
+def _mdt(a):
+    if a.dtype == np.float16:
+        return F16
+    if a.dtype == np.float32:
+        return F32
+    raise TypeError("descriptors must be float16 or float32")
+
+
+def match_nn(A, Bm, na=None, nb=None, ratio=0.8, mutual=False, want_sim=False):
+    """M1..M5.  A [Na,D], Bm [Nb,D] (f16|f32, same dtype) -> (idx [Na] i32, s1 [Na] f64, s2 [Na] f64[, S [na,nb]])."""
+    A = np.ascontiguousarray(A)
+    Bm = np.ascontiguousarray(Bm)
+    assert A.dtype == Bm.dtype and A.shape[1] == Bm.shape[1]
+    Na, D = A.shape
+    Nb = Bm.shape[0]
+    na = Na if na is None else int(na)
+    nb = Nb if nb is None else int(nb)
+    idx = np.empty(Na, np.int32)
+    s1 = np.empty(Na, np.float64)
+    s2 = np.empty(Na, np.float64)
+    S = np.empty((na, nb), np.float64) if want_sim else None
+    rc = lib().match_oracle_nn(_p(A), _p(Bm), _mdt(A), Na, Nb, D, na, nb, float(ratio), int(bool(mutual)),
+                               _p(idx), _p(s1), _p(s2), _p(S))
+    if rc < 0:
+        raise ValueError("match_oracle_nn: invalid argument")
+    return (idx, s1, s2, S) if want_sim else (idx, s1, s2)
+
+
+def retrieval_scan(db, q, n_exclude=50, tau=0.60, max_cand=16):
+    """M6..M8.  db [n,D], q [D] (f16|f32) -> (sim [n] f64, cand [max_cand] i32 (-1 padded), count)."""
+    db = np.ascontiguousarray(db)
+    q = np.ascontiguousarray(q)
+    assert db.dtype == q.dtype and db.shape[1] == q.shape[0]
+    n, D = db.shape
+    sim = np.empty(n, np.float64)
+    cand = np.empty(max_cand, np.int32)
+    K = lib().retrieval_oracle_scan(_p(db), _p(q), _mdt(db), n, D, int(n_exclude), float(tau), int(max_cand),
+                                    _p(sim), _p(cand))
+    if K < 0:
+        raise ValueError("retrieval_oracle_scan: invalid argument")
+    return sim, cand, int(K)
+
+
+def stereo_validate(pl, pr, fx, fy, cx, cy, baseline, d_min, z_min, z_max, max_reproj=1.5):
+    """S1..S4 -> (valid [n] u8, xyz [n,3], disparity [n], reproj_err [n])."""
+    pl = _c(pl, np.float64)
+    pr = _c(pr, np.float64)
+    n = pl.shape[0]
+    xyz = np.empty((n, 3), np.float64)
+    disp = np.empty(n, np.float64)
+    err = np.empty(n, np.float64)
+    valid = np.empty(n, np.uint8)
+    lib().stereo_oracle_validate(_p(pl), _p(pr), n, float(fx), float(fy), float(cx), float(cy), float(baseline),
+                                 float(d_min), float(z_min), float(z_max), float(max_reproj),
+                                 _p(xyz), _p(disp), _p(err), _p(valid))
+    return valid, xyz, disp, err
+
+
+def cov_sqrt_info(Lf, scale, floor_px, fx, fy, lam, lam_min, sigma0):
+    """C1..C4.  Lf [n,3] = (l11, l21, l22) -> (omega [n,2,2] f64, ok [n] u8)."""
+    Lf = _c(Lf, np.float64)
+    n = Lf.shape[0]
+    om = np.empty((n, 2, 2), np.float64)
+    ok = np.empty(n, np.uint8)
+    lib().cov_oracle_sqrt_info(_p(Lf), n, float(scale), float(floor_px), float(fx), float(fy), float(lam),
+                               float(lam_min), float(sigma0), _p(om), _p(ok))
+    return om, ok
