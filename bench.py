@@ -422,6 +422,12 @@ def run_ours(args):
             b64 = {"skipped": f"needs {need >> 30} GiB of device memory, {free >> 30} GiB free"}
         else:
             ctx5 = dkd.DKD(c5.B, c5.H, c5.W, c5.top_k, c5.D, device=local)
+            if os.environ.get("DKD_BENCH_NMS_UNIT"):             # tuning aid (not used by the driver's line)
+                from paper_2607_01757_b200.binding import OPT_NMS_UNIT
+                ctx5.set_option(OPT_NMS_UNIT, int(os.environ["DKD_BENCH_NMS_UNIT"]))
+            if os.environ.get("DKD_BENCH_SEL_PREFETCH"):
+                from paper_2607_01757_b200.binding import OPT_SEL_PREFETCH
+                ctx5.set_option(OPT_SEL_PREFETCH, int(os.environ["DKD_BENCH_SEL_PREFETCH"]))
             score5 = synth.score_maps(c5.B, c5.H, c5.W, c5.seed, c5.base, c5.nblobs).to(dev)
             desc5 = synth.desc_maps(c5.B, c5.Hd, c5.Wd, c5.D, c5.seed, torch.float16, dev)
             out5 = ctx5.alloc_outputs(c5.B, c5.top_k, desc5, c5.D, want_index=False, want_offsets=False)

@@ -35,12 +35,15 @@ enum {
     DKD_OK = 0,
     DKD_ERR_INVALID_ARG = -1,   /* NULL required pointer, size < 1, r < 1, T <= 0 or non-finite, ... */
     DKD_ERR_UNSUPPORTED = -2,   /* r > DKD_MAX_RADIUS; D*elemsize not a multiple of 16 B or > DKD_MAX_ROW_BYTES;
-                                   desc/out_desc not 16-byte aligned; score not 4-byte aligned; unknown dtype */
+                                   desc/out_desc not 16-byte aligned; out_kpts/out_offset not 8-byte aligned; any
+                                   other f32/i32 buffer not 4-byte aligned; unknown dtype */
     DKD_ERR_CAPACITY = -3,      /* B, H, W, top_k or D above the dkd_create maxima */
     DKD_ERR_CUDA = -4           /* CUDA runtime/driver failure; text in dkd_last_error() */
 };
 
 enum { DKD_F32 = 0, DKD_F16 = 1 };          /* descriptor-map element type */
+
+enum { DKD_SCORE_RAW = 0, DKD_SCORE_BILINEAR = 1 };   /* reported score, see dkd_variant_params */
 
 #define DKD_MAX_RADIUS    4                 /* (2r+1)^2 window, r in [1,4] (paper's extractors use 2..4) */
 #define DKD_MAX_TOP_K     8192              /* per-image cap (paper: 160..384) */
@@ -50,7 +53,11 @@ enum { DKD_F32 = 0, DKD_F16 = 1 };          /* descriptor-map element type */
 enum {
     DKD_OPT_USE_GRAPH = 0,   /* [1] run each dkd_extract as ONE cached CUDA-graph launch (north_star:
                                 "the whole stereo pair in one CUDA-graph launch"); 0 = plain launches.
-                                Ignored (plain launches) while `stream` is being captured by the caller. */
+                                Ignored (plain launches) while `stream` is being captured by the caller.
+                                The cache is keyed on SHAPES (B, H, W, r, top_k, D, dtype, stride, which optional
+                                buffers are present, options): a call that differs only in buffer addresses, thresh
+                                or T re-uses the instantiated graph and updates its kernel nodes' parameters in
+                                place — nothing is captured or instantiated again (dkd_graph_stats). */
     DKD_OPT_USE_TMA   = 1,   /* [1] NMS tiles staged by TMA (cp.async.bulk.tensor) when W % 4 == 0 and
                                 score is 16-byte aligned; 0 = always the plain-load tile loader. */
     DKD_OPT_PROFILE   = 2,   /* [0] 1 = measurement mode: plain launches (no graph) with a CUDA event recorded
@@ -61,6 +68,9 @@ enum {
     DKD_OPT_ORIGIN_X  = 5,   /* [0] letterbox offset (ox, oy) of the score map inside the padded network input: it is */
     DKD_OPT_ORIGIN_Y  = 6,   /* [0] subtracted from every keypoint coordinate ("shifted back to native coordinates by
                                 subtracting the offset"); out_index / out_offset are unaffected. */
+    DKD_OPT_SEL_PREFETCH = 7, /* [0] the select kernel asks L2 for the refinement-window rows of every kept keypoint, so
+                                that the refinement's dependent loads hit L2 (tuning knob; results do not depend on it;
+                                measured a net loss at batch 64: DESIGN.md 7.3). */
     DKD_OPT_NMS_UNIT  = 4    /* [0] strip-tiles (8 output rows each) a warp of the NMS kernel walks down before it
                                 moves to another strip: 0 = chosen per call from the problem size, 1..8 = forced
                                 (tuning / test knob; results do not depend on it). */
@@ -108,7 +118,7 @@ int dkd_set_option(dkd_ctx* ctx, int option, int value);
  *   desc       device [B,Hd,Wd,D] channel-last, DKD_F16 or DKD_F32, contiguous, 16-byte aligned,
  *              or NULL to skip step (4) (then out_desc must be NULL).  Hd*stride, Wd*stride need
  *              not equal H, W: sampling positions are clamped to the map.           (read only)
- *   out_kpts   device [B,top_k,2] f32 (x,y)
+ *   out_kpts   device [B,top_k,2] f32 (x,y), 8-byte aligned
  *   out_scores device [B,top_k]   f32, raw S at the integer peak (bit-identical to the input)
  *   out_desc   device [B,top_k,D] same element type as desc, 16-byte aligned
  *   out_count  device [B] i32 = K_b
@@ -129,8 +139,8 @@ int dkd_extract(dkd_ctx* ctx,
 /* dkd_extract plus two optional outputs (either may be NULL):
  *   out_index  device [B,top_k] i32: linear index y*W+x of the integer peak, -1 in padding
  *              (integer positions cannot be recovered from the refined coordinates);
- *   out_offset device [B,top_k,2] f32: the sub-pixel offset (dx,dy) before it is added to (x,y)
- *              (the 1e-5 px parity bound applies to this; G11). */
+ *   out_offset device [B,top_k,2] f32, 8-byte aligned: the sub-pixel offset (dx,dy) before it is added to
+ *              (x,y) (the 1e-5 px parity bound applies to this; G11). */
 int dkd_extract_ex(dkd_ctx* ctx,
                    const float* score, int B, int H, int W,
                    const void* desc, int desc_dtype, int Hd, int Wd, int D, int stride,
@@ -138,6 +148,50 @@ int dkd_extract_ex(dkd_ctx* ctx,
                    float* out_kpts, float* out_scores, void* out_desc, int32_t* out_count,
                    int32_t* out_index, float* out_offset,
                    void* stream);
+
+/*
+ * Variants of the path on the same kernels (readings V1..V5 in DESIGN.md).  Every field may be
+ * left 0 / NULL, which is the base path.
+ *   reliability  device [B,H,W] f32: the score the whole path works on is heat x reliability, each product rounded
+ *                once to fp32 and formed BEFORE the window maximum (XFeat: keypoint heat "filtered using an additional
+ *                reliability heatmap").  `score` is the heat map.  The product is never written to
+ *                memory: the NMS kernel streams both maps (second TMA stream).  Threshold, order, reported score and
+ *                refinement all use the product.
+ *   valid_mask   device [B,H,W] u8: a pixel can be a keypoint only where the mask is non-zero ("a fisheye validity
+ *                mask that culls features near the image periphery").  Masked pixels still take part
+ *                in every window maximum and in the refinement windows.
+ *   nms_iters    0 = one (2r+1)^2 max-pool pass (north_star).  n > 0 = the iterated suppress-and-recover NMS of "the
+ *                original PyTorch NMS" with n recovery rounds (the published procedure uses 2).
+ *   score_mode   DKD_SCORE_RAW: out_scores = S at the integer peak (bit-exact).  DKD_SCORE_BILINEAR: out_scores = S
+ *                interpolated bilinearly at the refined position (x+dx, y+dy).  Selection and order always use the
+ *                raw score.
+ *   out_total    device [B] i32 or NULL: C_b, the number of candidates of image b BEFORE the cap.  Threshold-only
+ *                mode (no cap) = top_k set to the capacity of the output buffers: out_count = min(C_b, top_k) and
+ *                out_total tells whether the buffers were large enough (if not, the best top_k are returned).
+ */
+typedef struct {
+    const float* reliability;
+    const uint8_t* valid_mask;
+    int nms_iters;
+    int score_mode;
+    int32_t* out_total;
+} dkd_variant_params;
+
+/* dkd_extract_ex with the variants above (v == NULL: identical to dkd_extract_ex). */
+int dkd_extract_var(dkd_ctx* ctx,
+                    const float* score, int B, int H, int W,
+                    const void* desc, int desc_dtype, int Hd, int Wd, int D, int stride,
+                    int r, float thresh, int top_k, float T,
+                    float* out_kpts, float* out_scores, void* out_desc, int32_t* out_count,
+                    int32_t* out_index, float* out_offset,
+                    const dkd_variant_params* v,
+                    void* stream);
+
+/* Graph-cache statistics since dkd_create (any pointer may be NULL): graphs instantiated, calls served by updating
+ * the kernel-node parameters of a cached graph, calls that replayed a cached graph unchanged, calls enqueued as plain
+ * launches. */
+int dkd_graph_stats(const dkd_ctx* ctx, uint64_t* instantiated, uint64_t* updated, uint64_t* replayed,
+                    uint64_t* stream_launched);
 
 /*
  * dkd_extract_host — the same call with HOST buffers (the end-to-end path): copies score host->device
@@ -149,8 +203,12 @@ int dkd_extract_ex(dkd_ctx* ctx,
  *     uploaded: the gather samples its corner rows directly over PCIe;
  *   - when every output buffer is pinned the kernels store straight into them (no staging, no copies back).
  * Pageable buffers go through staged cudaMemcpyAsync copies.
- * desc_resident != 0 uploads the descriptor map once and reuses the device copy while the same desc pointer
- * and shape are passed (a dense network would leave it on the device).
+ * desc_resident: 0 = the map is uploaded (or sampled in place) on every call; 1 = upload once and re-use the device
+ * copy while the same desc pointer and shape are passed — the caller must NOT modify the host map while it is resident
+ * (a copy uploaded by a desc_resident = 0 call is never re-used); 2 = upload now (the host map changed) and keep the
+ * copy resident for later desc_resident = 1 calls.  (A dense network would leave the map on the device.)
+ * Every shape / scalar argument is checked before anything is allocated or enqueued; if an error occurs after work
+ * was enqueued the stream is synchronised before the call returns.
  */
 int dkd_extract_host(dkd_ctx* ctx,
                      const float* score, int B, int H, int W,

@@ -10,13 +10,15 @@ import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 F32, F16 = 0, 1
-OPT_USE_GRAPH, OPT_USE_TMA, OPT_PROFILE, OPT_USE_PDL, OPT_NMS_UNIT, OPT_ORIGIN_X, OPT_ORIGIN_Y = 0, 1, 2, 3, 4, 5, 6
+OPT_USE_GRAPH, OPT_USE_TMA, OPT_PROFILE, OPT_USE_PDL, OPT_NMS_UNIT, OPT_ORIGIN_X, OPT_ORIGIN_Y, OPT_SEL_PREFETCH = 0, 1, 2, 3, 4, 5, 6, 7
 MAX_RADIUS, MAX_TOP_K, MAX_ROW_BYTES = 4, 8192, 2048
+
+SCORE_RAW, SCORE_BILINEAR = 0, 1
 
 EXPORTED_SYMBOLS = (
     "dkd_create", "dkd_destroy", "dkd_last_error", "dkd_workspace_bytes", "dkd_set_option",
-    "dkd_extract", "dkd_extract_ex", "dkd_extract_host", "dkd_launches_per_extract", "dkd_version",
-    "dkd_profile_read", "dkd_kernel_name", "dkd_pre_padded_size", "dkd_preprocess",
+    "dkd_extract", "dkd_extract_ex", "dkd_extract_var", "dkd_extract_host", "dkd_launches_per_extract", "dkd_version",
+    "dkd_profile_read", "dkd_kernel_name", "dkd_pre_padded_size", "dkd_preprocess", "dkd_graph_stats",
 )
 
 
@@ -37,8 +39,15 @@ class _PreParams(ctypes.Structure):
                 ("mean", ctypes.c_float * 3), ("inv_std", ctypes.c_float * 3), ("pad_value", ctypes.c_float)]
 
 
+class _VariantParams(ctypes.Structure):
+    _fields_ = [("reliability", ctypes.c_void_p), ("valid_mask", ctypes.c_void_p), ("nms_iters", ctypes.c_int),
+                ("score_mode", ctypes.c_int), ("out_total", ctypes.c_void_p)]
+
+
 def lib_path() -> str:
-    return os.path.join(_HERE, "libdkd.so")
+    """The in-tree library.  DKD_LIBRARY selects another build of it by file name (libdkd_debug.so: the
+    -DDKD_DEBUG build with device-side bounds checks)."""
+    return os.path.join(_HERE, os.environ.get("DKD_LIBRARY", "libdkd.so"))
 
 
 _lib = None
@@ -82,6 +91,11 @@ def load_library():
     L.dkd_extract.argtypes = common + [vp]
     L.dkd_extract_ex.restype = i
     L.dkd_extract_ex.argtypes = common + [vp, vp, vp]
+    L.dkd_extract_var.restype = i
+    L.dkd_extract_var.argtypes = common + [vp, vp, ctypes.POINTER(_VariantParams), vp]
+    u64p = ctypes.POINTER(ctypes.c_uint64)
+    L.dkd_graph_stats.restype = i
+    L.dkd_graph_stats.argtypes = [vp, u64p, u64p, u64p, u64p]
     L.dkd_extract_host.restype = i
     L.dkd_extract_host.argtypes = common + [vp, vp, i, vp]
     _lib = L
@@ -96,6 +110,7 @@ class DKDResult:
     count: torch.Tensor                # [B]     i32
     index: Optional[torch.Tensor]      # [B,k]   i32 (-1 padding)
     offsets: Optional[torch.Tensor]    # [B,k,2] f32 (dx,dy)
+    total: Optional[torch.Tensor] = None   # [B] i32: candidates before the cap (variants only)
 
 
 def _dt(t: Optional[torch.Tensor]) -> int:
@@ -162,6 +177,12 @@ class DKD:
             self._check(n)
         return {self._L.dkd_kernel_name(j).decode(): float(buf[j]) for j in range(n)}
 
+    def graph_stats(self) -> dict:
+        """dkd_graph_stats: {instantiated, updated, replayed, stream} call counts since the context was created."""
+        v = [ctypes.c_uint64() for _ in range(4)]
+        self._check(self._L.dkd_graph_stats(self._h, *[ctypes.byref(x) for x in v]))
+        return dict(zip(("instantiated", "updated", "replayed", "stream"), (int(x.value) for x in v)))
+
     # -- fused input pre-processing (dkd_pre_padded_size / dkd_preprocess) ---------------------
     @staticmethod
     def padded_size(H: int, W: int, grid: int):
@@ -203,11 +224,34 @@ class DKD:
             offsets=torch.empty((B, top_k, 2), dtype=torch.float32, **kw) if want_offsets else None,
         )
 
+    def _check_out(self, out: DKDResult, B: int, top_k: int, desc, D: int, cuda: bool):
+        """A caller-supplied output set must have exactly the shapes / dtypes / placement the C call writes."""
+        want = [("kpts", (B, top_k, 2), torch.float32, True), ("scores", (B, top_k), torch.float32, True),
+                ("count", (B,), torch.int32, True), ("index", (B, top_k), torch.int32, False),
+                ("offsets", (B, top_k, 2), torch.float32, False), ("total", (B,), torch.int32, False)]
+        if desc is not None:
+            want.append(("desc", (B, top_k, D), desc.dtype, True))
+        elif out.desc is not None:
+            raise DKDError(-1, "out.desc given without a descriptor map")
+        for name, shape, dtype, required in want:
+            t = getattr(out, name)
+            if t is None:
+                if required:
+                    raise DKDError(-1, f"out.{name} is missing")
+                continue
+            if tuple(t.shape) != shape or t.dtype != dtype or not t.is_contiguous() or t.is_cuda != cuda:
+                raise DKDError(-1, f"out.{name} must be a contiguous {'CUDA' if cuda else 'CPU'} {dtype} tensor of shape {shape}")
+            if cuda and t.device != self.device:
+                raise DKDError(-1, f"out.{name} is on {t.device}, the context is on {self.device}")
+
     def extract(self, score: torch.Tensor, desc: Optional[torch.Tensor], stride: int, r: int,
                 thresh: float, top_k: int, T: float, out: Optional[DKDResult] = None,
-                stream: Optional[torch.cuda.Stream] = None, want_index=True, want_offsets=True) -> DKDResult:
+                stream: Optional[torch.cuda.Stream] = None, want_index=True, want_offsets=True,
+                reliability: Optional[torch.Tensor] = None, valid_mask: Optional[torch.Tensor] = None,
+                nms_iters: int = 0, score_mode: int = SCORE_RAW, want_total: bool = False) -> DKDResult:
         """score [B,H,W] f32 cuda contiguous; desc [B,Hd,Wd,D] f16|f32 cuda contiguous or None.
-        Asynchronous on `stream` (default: the current torch stream)."""
+        Asynchronous on `stream` (default: the current torch stream).  The keyword arguments after
+        `want_offsets` are the variants of dkd_extract_var (dkd.h)."""
         if not (score.is_cuda and score.is_contiguous() and score.dtype == torch.float32 and score.dim() == 3):
             raise DKDError(-1, "score must be a contiguous CUDA float32 [B,H,W] tensor")
         B, H, W = score.shape
@@ -216,13 +260,25 @@ class DKD:
             if not (desc.is_cuda and desc.is_contiguous() and desc.dim() == 4 and desc.shape[0] == B):
                 raise DKDError(-1, "desc must be a contiguous CUDA [B,Hd,Wd,D] tensor")
             _, Hd, Wd, D = desc.shape
+        if reliability is not None and not (reliability.is_cuda and reliability.is_contiguous() and
+                                            reliability.dtype == torch.float32 and reliability.shape == score.shape):
+            raise DKDError(-1, "reliability must be a contiguous CUDA float32 tensor shaped like score")
+        if valid_mask is not None and not (valid_mask.is_cuda and valid_mask.is_contiguous() and
+                                           valid_mask.dtype == torch.uint8 and valid_mask.shape == score.shape):
+            raise DKDError(-1, "valid_mask must be a contiguous CUDA uint8 tensor shaped like score")
         if out is None:
             out = self.alloc_outputs(B, top_k, desc, D, want_index, want_offsets)
+        else:
+            self._check_out(out, B, top_k, desc, D, cuda=True)
+        if want_total and out.total is None:
+            out.total = torch.empty((B,), dtype=torch.int32, device=score.device)
         st = torch.cuda.current_stream(self.device) if stream is None else stream
-        rc = self._L.dkd_extract_ex(self._h, _ptr(score), B, H, W, _ptr(desc), _dt(desc), Hd, Wd, D,
-                                    int(stride), int(r), float(thresh), int(top_k), float(T),
-                                    _ptr(out.kpts), _ptr(out.scores), _ptr(out.desc), _ptr(out.count),
-                                    _ptr(out.index), _ptr(out.offsets), ctypes.c_void_p(st.cuda_stream))
+        v = _VariantParams(_ptr(reliability), _ptr(valid_mask), int(nms_iters), int(score_mode), _ptr(out.total))
+        rc = self._L.dkd_extract_var(self._h, _ptr(score), B, H, W, _ptr(desc), _dt(desc), Hd, Wd, D,
+                                     int(stride), int(r), float(thresh), int(top_k), float(T),
+                                     _ptr(out.kpts), _ptr(out.scores), _ptr(out.desc), _ptr(out.count),
+                                     _ptr(out.index), _ptr(out.offsets), ctypes.byref(v),
+                                     ctypes.c_void_p(st.cuda_stream))
         self._check(rc)
         return out
 
@@ -265,7 +321,9 @@ class DKD:
     def extract_host(self, score: torch.Tensor, desc: Optional[torch.Tensor], stride: int, r: int,
                      thresh: float, top_k: int, T: float, out: Optional[DKDResult] = None,
                      desc_resident: bool = False, stream: Optional[torch.cuda.Stream] = None) -> DKDResult:
-        """HOST tensors in, HOST tensors out (copies inside the call, synchronous on return)."""
+        """HOST tensors in, HOST tensors out (copies inside the call, synchronous on return).
+        desc_resident: False/0, True/1 (re-use the uploaded map; do not modify it meanwhile) or 2 (upload again
+        and keep resident) — see dkd.h."""
         if score.is_cuda or not score.is_contiguous() or score.dtype != torch.float32 or score.dim() != 3:
             raise DKDError(-1, "score must be a contiguous CPU float32 [B,H,W] tensor")
         B, H, W = score.shape
@@ -276,6 +334,8 @@ class DKD:
             _, Hd, Wd, D = desc.shape
         if out is None:
             out = self.alloc_outputs(B, top_k, desc, D, device="cpu", pin=True)
+        else:
+            self._check_out(out, B, top_k, desc, D, cuda=False)
         st = torch.cuda.current_stream(self.device) if stream is None else stream
         rc = self._L.dkd_extract_host(self._h, _ptr(score), B, H, W, _ptr(desc), _dt(desc), Hd, Wd, D,
                                       int(stride), int(r), float(thresh), int(top_k), float(T),

@@ -9,8 +9,9 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libdkd.so")
-SOURCES = [os.path.join(CSRC, "dkd_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "dkd_kernels.cuh"), os.path.join(ROOT, "include", "dkd.h")]
+SOURCES = [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith(".cu")]
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith((".cuh", ".h"))] + [
+    os.path.join(ROOT, "include", "dkd.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

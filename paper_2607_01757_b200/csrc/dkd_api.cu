@@ -1,5 +1,5 @@
 // dkd_api.cu — host side of libdkd: the C-ABI of include/dkd.h (argument validation, workspace,
-// TMA descriptor, launches, CUDA-graph cache, host-buffer path).  See DESIGN.md.
+// TMA descriptors, launch plans, the shape-keyed CUDA-graph cache, the host-buffer path).  See DESIGN.md.
 #include "dkd.h"
 
 #include <math.h>
@@ -9,6 +9,7 @@
 #include <vector>
 
 #include "dkd_kernels.cuh"
+#include "dkd_host.h"
 
 using namespace dkd;
 
@@ -19,9 +20,9 @@ typedef CUresult (*PFN_tensorMapEncodeTiled)(CUtensorMap*, CUtensorMapDataType, 
                                              CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
                                              CUtensorMapFloatOOBfill);
 
-char g_create_error[512] = "";
+thread_local char g_create_error[512] = "";
 
-struct ExtractArgs {                       // everything that determines the enqueued work
+struct ExtractArgs {                       // one dkd_extract* call
     const float* score;
     int B, H, W;
     const void* desc;
@@ -35,19 +36,58 @@ struct ExtractArgs {                       // everything that determines the enq
     int32_t* out_count;
     int32_t* out_index;
     float* out_offset;
+    // variants (dkd_extract_var)
+    const float* score2;                   // reliability map: score = heat x reliability
+    const uint8_t* mask;                   // validity mask
+    int nms_iters, score_mode;
+    int32_t* out_total;
+    // derived
     int use_tma;
     int origin_x, origin_y;                // letterbox offset subtracted from the keypoint coordinates
 };
 
+// What a cached graph's TOPOLOGY and launch geometry depend on.  Addresses and the scalars thresh / T are
+// kernel arguments: a call that differs only in those re-uses the instantiated graph and updates the
+// kernel nodes' parameters (cudaGraphExecKernelNodeSetParams) — no capture, no instantiation.
+struct ShapeKey {
+    int B, H, W, has_desc, desc_dtype, Hd, Wd, D, stride, r, top_k;
+    int has_index, has_offset, has_score2, has_mask, has_total, nms_iters, score_mode;
+    int use_tma, negt, use_pdl, nms_cpu, split;
+    bool operator==(const ShapeKey& o) const {
+        return B == o.B && H == o.H && W == o.W && has_desc == o.has_desc && desc_dtype == o.desc_dtype && Hd == o.Hd &&
+               Wd == o.Wd && D == o.D && stride == o.stride && r == o.r && top_k == o.top_k && has_index == o.has_index &&
+               has_offset == o.has_offset && has_score2 == o.has_score2 && has_mask == o.has_mask &&
+               has_total == o.has_total && nms_iters == o.nms_iters && score_mode == o.score_mode && use_tma == o.use_tma &&
+               negt == o.negt && use_pdl == o.use_pdl && nms_cpu == o.nms_cpu && split == o.split;
+    }
+};
+
+bool same_values(const ExtractArgs& x, const ExtractArgs& y) {   // the arguments a graph's kernel nodes embed
+    return x.score == y.score && x.desc == y.desc && x.thresh == y.thresh && x.T == y.T && x.out_kpts == y.out_kpts &&
+           x.out_scores == y.out_scores && x.out_desc == y.out_desc && x.out_count == y.out_count &&
+           x.out_index == y.out_index && x.out_offset == y.out_offset && x.score2 == y.score2 && x.mask == y.mask &&
+           x.out_total == y.out_total && x.origin_x == y.origin_x && x.origin_y == y.origin_y;
+}
+
+constexpr int MAX_KERNELS = 3;                              // kernels per extract, in launch order:
+const char* const KERNEL_NAMES[MAX_KERNELS] = {"nms", "select", "refine_gather"};
+
+struct Plan {                                               // the launches of one extract
+    KLaunch k[MAX_KERNELS];
+    int n;
+};
+
 struct GraphEntry {
-    ExtractArgs key;
+    ShapeKey key;
+    ExtractArgs last;                                       // the argument values the exec currently embeds
+    cudaGraph_t graph;                                      // kept: its kernel nodes address the exec's nodes
     cudaGraphExec_t exec;
+    cudaGraphNode_t node[MAX_KERNELS];
+    int n_nodes;                                            // 0: node handles unknown, parameters cannot be updated
     unsigned long long last_use;
 };
 
-constexpr size_t GRAPH_CACHE_CAP = 256;
-constexpr int MAX_KERNELS = 3;                              // kernels per extract, in launch order:
-const char* const KERNEL_NAMES[MAX_KERNELS] = {"nms", "select", "refine_gather"};
+constexpr size_t GRAPH_CACHE_CAP = 64;
 
 }  // namespace
 
@@ -55,6 +95,7 @@ struct dkd_ctx {
     dkd_create_params p;
     int num_sms;
     int nms_ctas_per_sm[MAX_R + 1];
+    int nms_ctas_per_sm_prod[MAX_R + 1];
     PFN_tensorMapEncodeTiled encode;
     // workspace (device)
     uint64_t* cand;          // [max_tiles * SEG_CAP] candidate keys, one private segment per NMS unit
@@ -66,14 +107,15 @@ struct dkd_ctx {
     void* st_score; size_t st_score_bytes;
     void* st_desc;  size_t st_desc_bytes;
     void* st_out;   size_t st_out_bytes;
-    const void* st_desc_src; size_t st_desc_src_bytes;      // what st_desc currently holds
+    const void* st_desc_src; size_t st_desc_src_bytes;      // the host map st_desc holds as a RESIDENT copy (else NULL)
     // options
-    int use_graph, use_tma, use_pdl, profile, nms_cpu, origin_x, origin_y;
+    int use_graph, use_tma, use_pdl, profile, nms_cpu, origin_x, origin_y, sel_prefetch;
     cudaEvent_t prof_ev[MAX_KERNELS + 1];                   // measurement mode: event before/after every kernel
     int prof_n;                                             // kernels of the last profiled call (0: none)
     std::vector<GraphEntry> graphs;
     cudaStream_t cap_stream;  // capture-only stream for building the cached graphs
     unsigned long long tick;
+    unsigned long long n_instantiated, n_updated, n_replayed, n_stream;   // graph-cache statistics (dkd_graph_stats)
     char err[512];
 };
 
@@ -93,15 +135,21 @@ int fail_cuda(dkd_ctx* ctx, const char* what, cudaError_t e) {
         if (e_ != cudaSuccess) return fail_cuda((ctx), #call, e_);     \
     } while (0)
 
+bool misaligned(const void* p, uintptr_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) != 0; }
+
 template <int R>
 cudaError_t setup_nms(dkd_ctx* ctx) {
-    cudaError_t e = cudaFuncSetAttribute(k_nms_tma<R, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, NMS_SMEM_BYTES);
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(k_nms_tma<R, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, NMS_SMEM_BYTES);
-    if (e != cudaSuccess) return e;
+    cudaError_t e;
+    if ((e = cudaFuncSetAttribute(k_nms_tma<R, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, NMS_SMEM_BYTES)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_nms_tma<R, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, NMS_SMEM_BYTES)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_nms_tma<R, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * NMS_SMEM_BYTES)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_nms_tma<R, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * NMS_SMEM_BYTES)) != cudaSuccess) return e;
     int n = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_nms_tma<R, true>, NMS_WARPS * 32, NMS_SMEM_BYTES);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_nms_tma<R, true, false>, NMS_WARPS * 32, NMS_SMEM_BYTES);
     ctx->nms_ctas_per_sm[R] = n > 0 ? n : 1;
+    if (e != cudaSuccess) return e;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_nms_tma<R, true, true>, NMS_WARPS * 32, 2 * NMS_SMEM_BYTES);
+    ctx->nms_ctas_per_sm_prod[R] = n > 0 ? n : 1;
     return e;
 }
 
@@ -128,30 +176,41 @@ NmsPlan nms_plan(const dkd_ctx* ctx, const ExtractArgs& a) {   // (a.use_tma == 
     return p;
 }
 
+bool encode_map(dkd_ctx* ctx, CUtensorMap* tmap, const float* base, const ExtractArgs& a) {
+    const cuuint64_t dims[3] = {(cuuint64_t)a.W, (cuuint64_t)a.H, (cuuint64_t)a.B};
+    const cuuint64_t strides[2] = {(cuuint64_t)a.W * 4, (cuuint64_t)a.W * a.H * 4};
+    const cuuint32_t box[3] = {(cuuint32_t)BOX_W, (cuuint32_t)TH, 1};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    return ctx->encode(tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(base), dims, strides, box, estr,
+                       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                       CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 template <int R>
-cudaError_t launch_nms(dkd_ctx* ctx, const ExtractArgs& a, const NmsPlan& p, cudaStream_t st) {
+cudaError_t plan_nms(dkd_ctx* ctx, const ExtractArgs& a, const NmsPlan& p, KLaunch& k) {
+    const bool prod = a.score2 != nullptr;
     if (a.use_tma) {
-        CUtensorMap tmap;
-        const cuuint64_t dims[3] = {(cuuint64_t)a.W, (cuuint64_t)a.H, (cuuint64_t)a.B};
-        const cuuint64_t strides[2] = {(cuuint64_t)a.W * 4, (cuuint64_t)a.W * a.H * 4};
-        const cuuint32_t box[3] = {(cuuint32_t)BOX_W, (cuuint32_t)TH, 1};
-        const cuuint32_t estr[3] = {1, 1, 1};
-        if (ctx->encode(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(a.score), dims, strides, box, estr,
-                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-            return cudaErrorInvalidValue;
-        int grid = ctx->num_sms * ctx->nms_ctas_per_sm[R];
+        CUtensorMap tmap, tmap2;
+        if (!encode_map(ctx, &tmap, a.score, a)) return cudaErrorInvalidValue;
+        tmap2 = tmap;
+        if (prod && !encode_map(ctx, &tmap2, a.score2, a)) return cudaErrorInvalidValue;
+        int grid = ctx->num_sms * (prod ? ctx->nms_ctas_per_sm_prod[R] : ctx->nms_ctas_per_sm[R]);
         if (grid > (p.units + NMS_WARPS - 1) / NMS_WARPS) grid = (p.units + NMS_WARPS - 1) / NMS_WARPS;
-        if (p.thr_up > 0.0f)
-            k_nms_tma<R, false><<<grid, NMS_WARPS * 32, NMS_SMEM_BYTES, st>>>(tmap, p, a.score, ctx->cand, ctx->tile_cnt);
-        else                                                 // a -0.0 score may be a candidate: fold it onto +0
-            k_nms_tma<R, true><<<grid, NMS_WARPS * 32, NMS_SMEM_BYTES, st>>>(tmap, p, a.score, ctx->cand, ctx->tile_cnt);
+        const size_t smem = prod ? 2 * NMS_SMEM_BYTES : NMS_SMEM_BYTES;
+        const bool negt = !(p.thr_up > 0.0f);                // a -0.0 score may be a candidate: fold it onto +0
+#define DKD_PREP_TMA(NEGT, PROD)                                                                                         \
+    prep(k, k_nms_tma<R, NEGT, PROD>, dim3(grid), dim3(NMS_WARPS * 32), smem, false, tmap, tmap2, p, a.score, a.score2, \
+         a.mask, ctx->cand, ctx->tile_cnt)
+        if (prod) { if (negt) DKD_PREP_TMA(true, true); else DKD_PREP_TMA(false, true); }
+        else { if (negt) DKD_PREP_TMA(true, false); else DKD_PREP_TMA(false, false); }
+#undef DKD_PREP_TMA
     } else {
         const int total = p.strips_x * p.chunks_y * a.B;
-        k_nms_plain<R><<<(total + PLAIN_WARPS - 1) / PLAIN_WARPS, PLAIN_WARPS * 32, 0, st>>>(a.score, p, total, ctx->cand,
-                                                                                             ctx->tile_cnt);
+        const dim3 grid((total + PLAIN_WARPS - 1) / PLAIN_WARPS);
+        if (prod) prep(k, k_nms_plain<R, true>, grid, dim3(PLAIN_WARPS * 32), 0, false, a.score, a.score2, a.mask, p, total, ctx->cand, ctx->tile_cnt);
+        else prep(k, k_nms_plain<R, false>, grid, dim3(PLAIN_WARPS * 32), 0, false, a.score, a.score2, a.mask, p, total, ctx->cand, ctx->tile_cnt);
     }
-    return cudaGetLastError();
+    return cudaSuccess;
 }
 
 FastDiv make_fastdiv(uint32_t d) {                          // exact n / d for every 32-bit n (d >= 1)
@@ -174,46 +233,34 @@ SampleAxis make_axis(int stride, int n) {
     return a;
 }
 
-// Launch with (pdl) or without the programmatic-stream-serialization attribute: with it the kernel may be
-// scheduled while its predecessor in the stream still runs (it calls griddepcontrol.wait before it reads
-// the predecessor's results), which hides the launch latency between the three kernels of an extract.
-template <typename... KArgs, typename... Args>
-cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, bool pdl,
-                       Args... args) {
-    cudaLaunchConfig_t cfg;
-    memset(&cfg, 0, sizeof(cfg));
-    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
-    cudaLaunchAttribute attr;
-    attr.id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr.val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = &attr;
-    cfg.numAttrs = pdl ? 1 : 0;
-    return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
-}
-
 template <int DT, int G>
-cudaError_t launch_rg_g(const RGParams& p, int B, cudaStream_t st, bool pdl) {
-    const dim3 grid((p.top_k + RG_THREADS / G - 1) / (RG_THREADS / G), B);
-    return launch_pdl(k_refine_gather<DT, G>, grid, dim3(RG_THREADS), 0, st, pdl, p);
+void plan_rg_g(const RGParams& p, int B, bool prod, bool pdl, KLaunch& k) {
+    const dim3 grid((p.top_k + RG_SLOTS - 1) / RG_SLOTS, B);
+    const dim3 block(DT < 0 ? 32 : RG_THREADS);
+    if (prod) prep(k, k_refine_gather<DT, G, true>, grid, block, 0, pdl, p);
+    else prep(k, k_refine_gather<DT, G, false>, grid, block, 0, pdl, p);
 }
 
 template <int DT>
-cudaError_t launch_rg_dt(const RGParams& p, int B, cudaStream_t st, bool pdl) {
-    if (p.nchunk <= 8) return launch_rg_g<DT, 8>(p, B, st, pdl);
-    if (p.nchunk <= 16) return launch_rg_g<DT, 16>(p, B, st, pdl);
-    return launch_rg_g<DT, 32>(p, B, st, pdl);
+void plan_rg_dt(const RGParams& p, int B, bool prod, bool pdl, KLaunch& k) {
+    if (p.nchunk <= 8) plan_rg_g<DT, 8>(p, B, prod, pdl, k);
+    else if (p.nchunk <= 16) plan_rg_g<DT, 16>(p, B, prod, pdl, k);
+    else plan_rg_g<DT, 32>(p, B, prod, pdl, k);
 }
 
-cudaError_t launch_rg(const ExtractArgs& a, const int32_t* sel, cudaStream_t st, bool pdl) {
+void plan_rg(const ExtractArgs& a, const int32_t* sel, bool pdl, KLaunch& k) {
     RGParams p;
     memset(&p, 0, sizeof(p));
-    p.score = a.score; p.H = a.H; p.W = a.W;
+    p.score = a.score; p.score2 = a.score2; p.H = a.H; p.W = a.W;
     p.divW = make_fastdiv(static_cast<uint32_t>(a.W));
     p.sel_idx = sel; p.top_k = a.top_k; p.r = a.r;
     p.kscale = static_cast<float>(1.4426950408889634 / static_cast<double>(a.T));
     p.out_kpts = a.out_kpts; p.out_scores = a.out_scores; p.out_off = a.out_offset;
     p.origin_x = a.origin_x; p.origin_y = a.origin_y;
-    if (a.desc == nullptr) return launch_rg_g<-1, 8>(p, a.B, st, pdl);
+    p.score_mode = a.score_mode;
+    p.vec_window = (a.W % 4 == 0) && !misaligned(a.score, 16) && a.score2 == nullptr;
+    const bool prod = a.score2 != nullptr;
+    if (a.desc == nullptr) { plan_rg_g<-1, 8>(p, a.B, prod, pdl, k); return; }
     const size_t esz = a.desc_dtype == DKD_F16 ? 2 : 4;
     p.desc = static_cast<const unsigned char*>(a.desc);
     p.nchunk = static_cast<int>(a.D * esz / 16);
@@ -221,51 +268,68 @@ cudaError_t launch_rg(const ExtractArgs& a, const int32_t* sel, cudaStream_t st,
     p.ax = make_axis(a.stride, a.Wd);
     p.ay = make_axis(a.stride, a.Hd);
     p.out_desc = static_cast<unsigned char*>(a.out_desc);
-    return a.desc_dtype == DKD_F16 ? launch_rg_dt<DKD_F16>(p, a.B, st, pdl) : launch_rg_dt<DKD_F32>(p, a.B, st, pdl);
+    if (a.desc_dtype == DKD_F16) plan_rg_dt<DKD_F16>(p, a.B, prod, pdl, k);
+    else plan_rg_dt<DKD_F32>(p, a.B, prod, pdl, k);
 }
 
-// Enqueue the three kernels of one extract on `st`.  No sync, no allocation: capture-safe.
-// prof: measurement mode, an event on `st` before and after every kernel.
-cudaError_t enqueue(dkd_ctx* ctx, const ExtractArgs& a, cudaStream_t st, bool prof = false) {
+// The launches of one extract (launch geometry + argument values).  Pure host work: nothing touches a stream.
+cudaError_t build_plan(dkd_ctx* ctx, const ExtractArgs& a, Plan& pl) {
     const NmsPlan plan = nms_plan(ctx, a);
     const int tpi = plan.strips_x * plan.segs;              // candidate segments (NMS units) per image
     cudaError_t e;
-    int nk = 0;
-    auto mark = [&]() { return prof ? cudaEventRecord(ctx->prof_ev[nk++], st) : cudaSuccess; };
-    if ((e = mark()) != cudaSuccess) return e;
     switch (a.r) {
-        case 1: e = launch_nms<1>(ctx, a, plan, st); break;
-        case 2: e = launch_nms<2>(ctx, a, plan, st); break;
-        case 3: e = launch_nms<3>(ctx, a, plan, st); break;
-        default: e = launch_nms<4>(ctx, a, plan, st); break;
+        case 1: e = plan_nms<1>(ctx, a, plan, pl.k[0]); break;
+        case 2: e = plan_nms<2>(ctx, a, plan, pl.k[0]); break;
+        case 3: e = plan_nms<3>(ctx, a, plan, pl.k[0]); break;
+        default: e = plan_nms<4>(ctx, a, plan, pl.k[0]); break;
     }
     if (e != cudaSuccess) return e;
-    if ((e = mark()) != cudaSuccess) return e;
     int32_t* sel = a.out_index ? a.out_index : ctx->sel_idx;
     int idx_shift = 0;                                       // (H*W - 1) >> idx_shift < NBT: index buckets of the top ties
     while (((static_cast<long long>(a.H) * a.W - 1) >> idx_shift) >= NBT) ++idx_shift;
-    const bool pdl = ctx->use_pdl && !prof;                  // (events between the kernels would serialise them anyway)
-    e = launch_pdl(k_select, dim3(a.B), dim3(SEL_THREADS), SEL_SMEM_BYTES, st, pdl, ctx->cand, ctx->tile_cnt, tpi,
-                   plan.cpu * SEG_CAP, a.top_k, idx_shift, sel, a.out_count);
-    if (e != cudaSuccess) return e;
-    if ((e = mark()) != cudaSuccess) return e;
-    e = launch_rg(a, sel, st, pdl);
-    if (e != cudaSuccess) return e;
-    if ((e = mark()) != cudaSuccess) return e;
-    if (prof) ctx->prof_n = nk - 1;
+    const bool pdl = ctx->use_pdl != 0;
+    SelPrefetch pf;
+    memset(&pf, 0, sizeof(pf));
+    if (ctx->sel_prefetch) {
+        const FastDiv dw = make_fastdiv(static_cast<uint32_t>(a.W));
+        pf.score = a.score; pf.score2 = a.score2; pf.W = a.W; pf.r = a.r;
+        pf.div_m = dw.m; pf.div_s1 = dw.s1; pf.div_s2 = dw.s2;
+        pf.img_px = static_cast<size_t>(a.H) * a.W;
+    }
+    prep(pl.k[1], k_select, dim3(a.B), dim3(SEL_THREADS), SEL_SMEM_BYTES, pdl, ctx->cand, ctx->tile_cnt, tpi,
+         plan.cpu * SEG_CAP, a.top_k, idx_shift, pf, sel, a.out_count, a.out_total);
+    plan_rg(a, sel, pdl, pl.k[2]);
+    pl.n = 3;
     return cudaSuccess;
 }
 
-int validate(dkd_ctx* ctx, const ExtractArgs& a) {
-    if (!ctx) return DKD_ERR_INVALID_ARG;
-    if (!a.score || !a.out_kpts || !a.out_scores || !a.out_count)
-        return fail(ctx, DKD_ERR_INVALID_ARG, "NULL required pointer (score/out_kpts/out_scores/out_count)");
+// Enqueue the kernels of one extract on `st`.  No sync, no allocation: capture-safe.
+// prof: measurement mode, an event on `st` before and after every kernel (and no PDL: the events would
+// serialise the kernels anyway).
+cudaError_t enqueue(dkd_ctx* ctx, const Plan& pl, cudaStream_t st, bool prof = false) {
+    cudaError_t e;
+    for (int i = 0; i < pl.n; ++i) {
+        if (prof && (e = cudaEventRecord(ctx->prof_ev[i], st)) != cudaSuccess) return e;
+        if ((e = launch(pl.k[i], st, !prof)) != cudaSuccess) return e;
+    }
+    if (prof) {
+        if ((e = cudaEventRecord(ctx->prof_ev[pl.n], st)) != cudaSuccess) return e;
+        ctx->prof_n = pl.n;
+    }
+    return cudaSuccess;
+}
+
+// shape / scalar checks (no pointer is dereferenced, no alignment is looked at): shared by the device and host paths
+int validate_shapes(dkd_ctx* ctx, const ExtractArgs& a) {
     if (a.B < 1 || a.H < 1 || a.W < 1 || a.top_k < 1) return fail(ctx, DKD_ERR_INVALID_ARG, "B, H, W, top_k must be >= 1");
     if (a.r < 1) return fail(ctx, DKD_ERR_INVALID_ARG, "r must be >= 1");
     if (!(a.T > 0.0f) || !isfinite(a.T)) return fail(ctx, DKD_ERR_INVALID_ARG, "T must be finite and > 0");
     if (isnan(a.thresh)) return fail(ctx, DKD_ERR_INVALID_ARG, "thresh is NaN");
     if ((a.desc == nullptr) != (a.out_desc == nullptr))
         return fail(ctx, DKD_ERR_INVALID_ARG, "desc and out_desc must both be NULL or both be set");
+    if (a.nms_iters < 0) return fail(ctx, DKD_ERR_INVALID_ARG, "nms_iters must be >= 0");
+    if (a.score_mode != DKD_SCORE_RAW && a.score_mode != DKD_SCORE_BILINEAR)
+        return fail(ctx, DKD_ERR_INVALID_ARG, "score_mode must be DKD_SCORE_RAW or DKD_SCORE_BILINEAR");
     if (a.desc) {
         if (a.Hd < 1 || a.Wd < 1 || a.D < 1 || a.stride < 1)
             return fail(ctx, DKD_ERR_INVALID_ARG, "Hd, Wd, D, stride must be >= 1");
@@ -273,77 +337,175 @@ int validate(dkd_ctx* ctx, const ExtractArgs& a) {
             return fail(ctx, DKD_ERR_UNSUPPORTED, "desc_dtype must be DKD_F32 or DKD_F16");
     }
     if (a.r > DKD_MAX_RADIUS) return fail(ctx, DKD_ERR_UNSUPPORTED, "r > DKD_MAX_RADIUS");
+    if (a.nms_iters > 0) return fail(ctx, DKD_ERR_UNSUPPORTED, "iterated NMS (nms_iters > 0) is not built yet");
     if (a.B > 65535) return fail(ctx, DKD_ERR_UNSUPPORTED, "B > 65535");
-    if (reinterpret_cast<uintptr_t>(a.score) & 3) return fail(ctx, DKD_ERR_UNSUPPORTED, "score not 4-byte aligned");
     if (a.desc) {
         const size_t rowb = static_cast<size_t>(a.D) * (a.desc_dtype == DKD_F16 ? 2 : 4);
         if (rowb % 16 != 0 || rowb > DKD_MAX_ROW_BYTES)
             return fail(ctx, DKD_ERR_UNSUPPORTED, "D * elemsize must be a multiple of 16 and <= DKD_MAX_ROW_BYTES");
-        if ((reinterpret_cast<uintptr_t>(a.desc) & 15) || (reinterpret_cast<uintptr_t>(a.out_desc) & 15))
-            return fail(ctx, DKD_ERR_UNSUPPORTED, "desc / out_desc not 16-byte aligned");
         if (a.D > ctx->p.max_dim) return fail(ctx, DKD_ERR_CAPACITY, "D > max_dim");
         if (a.stride > (1 << 20)) return fail(ctx, DKD_ERR_UNSUPPORTED, "stride too large");
+        if (static_cast<long long>(a.Hd) * a.Wd > 0x7fffffffLL) return fail(ctx, DKD_ERR_UNSUPPORTED, "Hd * Wd >= 2^31");
     }
     if (a.B > ctx->p.max_batch || a.H > ctx->p.max_h || a.W > ctx->p.max_w || a.top_k > ctx->p.max_top_k)
         return fail(ctx, DKD_ERR_CAPACITY, "B, H, W or top_k above the dkd_create maxima");
     return DKD_OK;
 }
 
-bool same_key(const ExtractArgs& x, const ExtractArgs& y) { return memcmp(&x, &y, sizeof(ExtractArgs)) == 0; }
+int validate(dkd_ctx* ctx, const ExtractArgs& a) {
+    if (!a.score || !a.out_kpts || !a.out_scores || !a.out_count)
+        return fail(ctx, DKD_ERR_INVALID_ARG, "NULL required pointer (score/out_kpts/out_scores/out_count)");
+    const int rc = validate_shapes(ctx, a);
+    if (rc != DKD_OK) return rc;
+    if (misaligned(a.score, 4) || misaligned(a.score2, 4)) return fail(ctx, DKD_ERR_UNSUPPORTED, "score / reliability not 4-byte aligned");
+    if (misaligned(a.out_kpts, 8) || misaligned(a.out_offset, 8))
+        return fail(ctx, DKD_ERR_UNSUPPORTED, "out_kpts / out_offset not 8-byte aligned");
+    if (misaligned(a.out_scores, 4) || misaligned(a.out_count, 4) || misaligned(a.out_index, 4) || misaligned(a.out_total, 4))
+        return fail(ctx, DKD_ERR_UNSUPPORTED, "out_scores / out_count / out_index / out_total not 4-byte aligned");
+    if (a.desc && (misaligned(a.desc, 16) || misaligned(a.out_desc, 16)))
+        return fail(ctx, DKD_ERR_UNSUPPORTED, "desc / out_desc not 16-byte aligned");
+    return DKD_OK;
+}
+
+ShapeKey shape_key(const dkd_ctx* ctx, const ExtractArgs& a) {
+    ShapeKey k;
+    memset(&k, 0, sizeof(k));
+    k.B = a.B; k.H = a.H; k.W = a.W; k.has_desc = a.desc != nullptr; k.desc_dtype = a.desc_dtype; k.Hd = a.Hd; k.Wd = a.Wd;
+    k.D = a.D; k.stride = a.stride; k.r = a.r; k.top_k = a.top_k;
+    k.has_index = a.out_index != nullptr; k.has_offset = a.out_offset != nullptr; k.has_score2 = a.score2 != nullptr;
+    k.has_mask = a.mask != nullptr; k.has_total = a.out_total != nullptr; k.nms_iters = a.nms_iters; k.score_mode = a.score_mode;
+    k.use_tma = a.use_tma; k.negt = !(nextafterf(a.thresh, INFINITY) > 0.0f); k.use_pdl = ctx->use_pdl; k.nms_cpu = ctx->nms_cpu;
+    k.split = ctx->sel_prefetch;
+    return k;
+}
+
+void drop_graphs(dkd_ctx* ctx) {
+    for (auto& g : ctx->graphs) {
+        cudaGraphExecDestroy(g.exec);
+        cudaGraphDestroy(g.graph);
+    }
+    ctx->graphs.clear();
+}
+
+// Capture the launches of `pl` once on the context's capture stream and instantiate them as a graph.  The
+// node handle of every kernel is read back right after its launch (the capturing stream's dependency set
+// is then exactly that node), so that later calls can re-point the kernels at other buffers.
+int build_graph(dkd_ctx* ctx, const Plan& pl, GraphEntry& ge) {
+    // (captured on a context-owned stream: the caller's may be the legacy default stream, which
+    // cannot be captured; the instantiated graph is then launched on the caller's stream)
+    CK(ctx, cudaStreamBeginCapture(ctx->cap_stream, cudaStreamCaptureModeThreadLocal));
+    cudaError_t e = cudaSuccess;
+    ge.n_nodes = pl.n;
+    for (int i = 0; i < pl.n; ++i) {
+        e = launch(pl.k[i], ctx->cap_stream, true);
+        if (e != cudaSuccess) break;
+        cudaStreamCaptureStatus cs;
+        const cudaGraphNode_t* deps = nullptr;
+        const cudaGraphEdgeData* edges = nullptr;
+        size_t nd = 0;
+        if (cudaStreamGetCaptureInfo_v3(ctx->cap_stream, &cs, nullptr, nullptr, &deps, &edges, &nd) == cudaSuccess &&
+            cs == cudaStreamCaptureStatusActive && nd == 1)
+            ge.node[i] = deps[0];
+        else
+            ge.n_nodes = 0;                                  // handles unknown: this entry is replay-only
+    }
+    cudaGraph_t graph = nullptr;
+    const cudaError_t e2 = cudaStreamEndCapture(ctx->cap_stream, &graph);
+    if (e != cudaSuccess || e2 != cudaSuccess) {
+        if (graph) cudaGraphDestroy(graph);
+        (void)cudaGetLastError();
+        return fail_cuda(ctx, "graph capture", e != cudaSuccess ? e : e2);
+    }
+    cudaGraphExec_t exec = nullptr;
+    e = cudaGraphInstantiate(&exec, graph, 0);
+    if (e != cudaSuccess) {
+        cudaGraphDestroy(graph);
+        return fail_cuda(ctx, "cudaGraphInstantiate", e);
+    }
+    ge.graph = graph;
+    ge.exec = exec;
+    ++ctx->n_instantiated;
+    return DKD_OK;
+}
+
+// Re-point an instantiated graph at the argument values of `pl` (same launch geometry: same ShapeKey).
+cudaError_t update_graph(GraphEntry& ge, const Plan& pl) {
+    for (int i = 0; i < pl.n; ++i) {
+        void* argp[KLaunch::MAX_ARGS];
+        cudaKernelNodeParams np;
+        memset(&np, 0, sizeof(np));
+        np.func = const_cast<void*>(pl.k[i].func);
+        np.gridDim = pl.k[i].grid; np.blockDim = pl.k[i].block;
+        np.sharedMemBytes = static_cast<unsigned>(pl.k[i].smem);
+        pl.k[i].arg_pointers(argp);
+        np.kernelParams = argp;
+        const cudaError_t e = cudaGraphExecKernelNodeSetParams(ge.exec, ge.node[i], &np);
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
 
 int run(dkd_ctx* ctx, ExtractArgs a, cudaStream_t st) {
     int rc = validate(ctx, a);
     if (rc != DKD_OK) return rc;
     a.origin_x = ctx->origin_x; a.origin_y = ctx->origin_y;
-    a.use_tma = ctx->use_tma && ctx->encode && (a.W % 4 == 0) && ((reinterpret_cast<uintptr_t>(a.score) & 15) == 0);
+    a.use_tma = ctx->use_tma && ctx->encode && (a.W % 4 == 0) && !misaligned(a.score, 16) && !misaligned(a.score2, 16);
 
+    Plan pl;
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     CK(ctx, cudaStreamIsCapturing(st, &cap));
     if (ctx->profile && cap == cudaStreamCaptureStatusNone) {
         ctx->prof_n = 0;
-        CK(ctx, enqueue(ctx, a, st, true));
+        CK(ctx, build_plan(ctx, a, pl));
+        CK(ctx, enqueue(ctx, pl, st, true));
         return DKD_OK;
     }
     if (!ctx->use_graph || cap != cudaStreamCaptureStatusNone) {
-        CK(ctx, enqueue(ctx, a, st));
+        CK(ctx, build_plan(ctx, a, pl));
+        CK(ctx, enqueue(ctx, pl, st));
+        ++ctx->n_stream;
         return DKD_OK;
     }
     ++ctx->tick;
-    for (auto& g : ctx->graphs)
-        if (same_key(g.key, a)) {
-            g.last_use = ctx->tick;
-            CK(ctx, cudaGraphLaunch(g.exec, st));
-            return DKD_OK;
+    const ShapeKey key = shape_key(ctx, a);
+    for (auto& g : ctx->graphs) {
+        if (!(g.key == key)) continue;
+        g.last_use = ctx->tick;
+        if (!same_values(g.last, a)) {                      // other buffers / thresh / T: update the kernel nodes in place
+            CK(ctx, build_plan(ctx, a, pl));
+            if (g.n_nodes != pl.n || update_graph(g, pl) != cudaSuccess) {
+                (void)cudaGetLastError();                   // cannot update: plain PDL-linked launches, the graph stays as it is
+                CK(ctx, enqueue(ctx, pl, st));
+                ++ctx->n_stream;
+                return DKD_OK;
+            }
+            g.last = a;
+            ++ctx->n_updated;
+        } else {
+            ++ctx->n_replayed;
         }
-    // first call with these arguments: capture the launches once, then replay as one graph launch
-    cudaGraph_t graph = nullptr;
-    // (captured on a context-owned stream: the caller's may be the legacy default stream, which
-    // cannot be captured; the instantiated graph is then launched on the caller's stream)
-    CK(ctx, cudaStreamBeginCapture(ctx->cap_stream, cudaStreamCaptureModeThreadLocal));
-    cudaError_t e = enqueue(ctx, a, ctx->cap_stream);
-    cudaError_t e2 = cudaStreamEndCapture(ctx->cap_stream, &graph);
-    if (e != cudaSuccess || e2 != cudaSuccess) {
-        if (graph) cudaGraphDestroy(graph);
-        return fail_cuda(ctx, "graph capture", e != cudaSuccess ? e : e2);
+        CK(ctx, cudaGraphLaunch(g.exec, st));
+        return DKD_OK;
     }
-    cudaGraphExec_t exec = nullptr;
-    e = cudaGraphInstantiate(&exec, graph, 0);
-    cudaGraphDestroy(graph);
-    if (e != cudaSuccess) return fail_cuda(ctx, "cudaGraphInstantiate", e);
+    // first call with this shape: capture the launches once, then replay as one graph launch
+    CK(ctx, build_plan(ctx, a, pl));
+    GraphEntry ge;
+    memset(&ge, 0, sizeof(ge));
+    if ((rc = build_graph(ctx, pl, ge)) != DKD_OK) return rc;
     if (ctx->graphs.size() >= GRAPH_CACHE_CAP) {            // evict the least recently used entry
         size_t v = 0;
         for (size_t i = 1; i < ctx->graphs.size(); ++i)
             if (ctx->graphs[i].last_use < ctx->graphs[v].last_use) v = i;
         cudaGraphExecDestroy(ctx->graphs[v].exec);
+        cudaGraphDestroy(ctx->graphs[v].graph);
         ctx->graphs[v] = ctx->graphs.back();
         ctx->graphs.pop_back();
     }
-    GraphEntry ge;
-    ge.key = a;
-    ge.exec = exec;
+    ge.key = key;
+    ge.last = a;
     ge.last_use = ctx->tick;
     ctx->graphs.push_back(ge);
-    CK(ctx, cudaGraphLaunch(exec, st));
+    CK(ctx, cudaGraphLaunch(ge.exec, st));
     return DKD_OK;
 }
 
@@ -381,11 +543,42 @@ void* mapped_device_pointer(const void* host) {
     return at.type == cudaMemoryTypeHost ? at.devicePointer : nullptr;
 }
 
+ExtractArgs make_args(const float* score, int B, int H, int W, const void* desc, int desc_dtype, int Hd, int Wd, int D,
+                      int stride, int r, float thresh, int top_k, float T, float* out_kpts, float* out_scores,
+                      void* out_desc, int32_t* out_count, int32_t* out_index, float* out_offset,
+                      const dkd_variant_params* v) {
+    ExtractArgs a;
+    memset(&a, 0, sizeof(a));
+    a.score = score; a.B = B; a.H = H; a.W = W;
+    a.desc = desc; a.desc_dtype = desc ? desc_dtype : 0; a.Hd = desc ? Hd : 0; a.Wd = desc ? Wd : 0;
+    a.D = desc ? D : 0; a.stride = desc ? stride : 1; a.r = r; a.thresh = thresh; a.top_k = top_k; a.T = T;
+    a.out_kpts = out_kpts; a.out_scores = out_scores; a.out_desc = out_desc; a.out_count = out_count;
+    a.out_index = out_index; a.out_offset = out_offset;
+    if (v) {
+        a.score2 = v->reliability; a.mask = v->valid_mask; a.nms_iters = v->nms_iters; a.score_mode = v->score_mode;
+        a.out_total = v->out_total;
+    }
+    return a;
+}
+
 }  // namespace
+
+// ---- helpers the other translation-unit-less parts of the library use (dkd_host.h) ---------------------------
+int dkd_ctx_device(const dkd_ctx* ctx) { return ctx->p.device; }
+int dkd_ctx_num_sms(const dkd_ctx* ctx) { return ctx->num_sms; }
+int dkd_ctx_fail(dkd_ctx* ctx, int code, const char* msg, const char* detail) {
+    return fail(ctx, code, "%s%s", msg, detail ? detail : "");
+}
 
 extern "C" {
 
-const char* dkd_version(void) { return "dkd-b200 0.1 (sm_100a)"; }
+const char* dkd_version(void) {
+#ifdef DKD_DEBUG
+    return "dkd-b200 0.2 (sm_100a, DKD_DEBUG: device-side bounds checks)";
+#else
+    return "dkd-b200 0.2 (sm_100a)";
+#endif
+}
 
 int dkd_create(const dkd_create_params* p, dkd_ctx** out) {
     if (out) *out = nullptr;
@@ -399,12 +592,16 @@ int dkd_create(const dkd_create_params* p, dkd_ctx** out) {
         snprintf(g_create_error, sizeof(g_create_error), "max_top_k > DKD_MAX_TOP_K");
         return DKD_ERR_UNSUPPORTED;
     }
+    int prev_dev = -1;
+    const bool have_prev = cudaGetDevice(&prev_dev) == cudaSuccess;   // the caller's current device is left unchanged
+    (void)cudaGetLastError();
     dkd_ctx* ctx = new dkd_ctx();
     ctx->p = *p;
     ctx->use_graph = 1;
     ctx->use_tma = 1;
     ctx->use_pdl = 1;
     ctx->nms_cpu = 0;
+    ctx->sel_prefetch = 0;
     ctx->origin_x = ctx->origin_y = 0;
     ctx->err[0] = 0;
     ctx->tick = 0;
@@ -414,6 +611,7 @@ int dkd_create(const dkd_create_params* p, dkd_ctx** out) {
         if (e_ != cudaSuccess) {                                                                         \
             snprintf(g_create_error, sizeof(g_create_error), "%s: %s", #call, cudaGetErrorString(e_));   \
             dkd_destroy(ctx);                                                                            \
+            if (have_prev) cudaSetDevice(prev_dev);                                                      \
             return DKD_ERR_CUDA;                                                                         \
         }                                                                                                \
     } while (0)
@@ -442,13 +640,15 @@ int dkd_create(const dkd_create_params* p, dkd_ctx** out) {
     CKC(cudaMalloc(&ctx->sel_idx, b_sel));
     ctx->ws_bytes = b_cand + b_cnt + b_sel;
 #undef CKC
+    if (have_prev) cudaSetDevice(prev_dev);
     *out = ctx;
     return DKD_OK;
 }
 
 int dkd_destroy(dkd_ctx* ctx) {
     if (!ctx) return DKD_OK;
-    for (auto& g : ctx->graphs) cudaGraphExecDestroy(g.exec);
+    DeviceGuard dg(ctx->p.device);
+    drop_graphs(ctx);
     if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
     for (int i = 0; i <= MAX_KERNELS; ++i)
         if (ctx->prof_ev[i]) cudaEventDestroy(ctx->prof_ev[i]);
@@ -474,17 +674,23 @@ int dkd_set_option(dkd_ctx* ctx, int option, int value) {
         case DKD_OPT_USE_GRAPH: ctx->use_graph = value != 0; return DKD_OK;
         case DKD_OPT_USE_TMA: ctx->use_tma = value != 0; return DKD_OK;
         case DKD_OPT_PROFILE: ctx->profile = value != 0; ctx->prof_n = 0; return DKD_OK;
-        case DKD_OPT_USE_PDL:                               // part of what a cached graph contains: drop the cache
-        case DKD_OPT_NMS_UNIT:
-            for (auto& g : ctx->graphs) cudaGraphExecDestroy(g.exec);
-            ctx->graphs.clear();
-            if (option == DKD_OPT_USE_PDL) ctx->use_pdl = value != 0;
-            else ctx->nms_cpu = value > 0 ? value : 0;
-            return DKD_OK;
-        case DKD_OPT_ORIGIN_X: ctx->origin_x = value; return DKD_OK;   // (part of the graph-cache key)
+        case DKD_OPT_USE_PDL: ctx->use_pdl = value != 0; return DKD_OK;          // (part of the graph-cache key)
+        case DKD_OPT_NMS_UNIT: ctx->nms_cpu = value > 0 ? value : 0; return DKD_OK;
+        case DKD_OPT_SEL_PREFETCH: ctx->sel_prefetch = value != 0; return DKD_OK;   // (kernel argument only)
+        case DKD_OPT_ORIGIN_X: ctx->origin_x = value; return DKD_OK;   // (a kernel argument: cached graphs are updated)
         case DKD_OPT_ORIGIN_Y: ctx->origin_y = value; return DKD_OK;
         default: return fail(ctx, DKD_ERR_INVALID_ARG, "unknown option");
     }
+}
+
+int dkd_graph_stats(const dkd_ctx* ctx, uint64_t* instantiated, uint64_t* updated, uint64_t* replayed,
+                    uint64_t* stream_launched) {
+    if (!ctx) return DKD_ERR_INVALID_ARG;
+    if (instantiated) *instantiated = ctx->n_instantiated;
+    if (updated) *updated = ctx->n_updated;
+    if (replayed) *replayed = ctx->n_replayed;
+    if (stream_launched) *stream_launched = ctx->n_stream;
+    return DKD_OK;
 }
 
 int dkd_launches_per_extract(const dkd_ctx* ctx, int with_desc) {
@@ -497,6 +703,7 @@ const char* dkd_kernel_name(int i) { return (i >= 0 && i < MAX_KERNELS) ? KERNEL
 
 int dkd_profile_read(dkd_ctx* ctx, float* ms, int n) {
     if (!ctx || !ms || n < 0) return DKD_ERR_INVALID_ARG;
+    DeviceGuard dg(ctx->p.device);
     if (ctx->prof_n <= 0) return fail(ctx, DKD_ERR_INVALID_ARG, "no profiled dkd_extract call (set DKD_OPT_PROFILE)");
     CK(ctx, cudaEventSynchronize(ctx->prof_ev[ctx->prof_n]));
     for (int i = 0; i < ctx->prof_n && i < n; ++i) CK(ctx, cudaEventElapsedTime(&ms[i], ctx->prof_ev[i], ctx->prof_ev[i + 1]));
@@ -522,6 +729,7 @@ int dkd_preprocess(dkd_ctx* ctx, const uint8_t* src, int B, int H, int W, const 
         return fail(ctx, DKD_ERR_UNSUPPORTED, "in_channels and out_channels must be 1 or 3");
     if (p->out_dtype != DKD_F32 && p->out_dtype != DKD_F16) return fail(ctx, DKD_ERR_UNSUPPORTED, "out_dtype must be DKD_F32 or DKD_F16");
     if (reinterpret_cast<uintptr_t>(dst) & 15) return fail(ctx, DKD_ERR_UNSUPPORTED, "dst not 16-byte aligned");
+    DeviceGuard dg(ctx->p.device);
     PreParams q;
     memset(&q, 0, sizeof(q));
     q.src = src; q.dst = static_cast<unsigned char*>(dst);
@@ -551,25 +759,30 @@ int dkd_preprocess(dkd_ctx* ctx, const uint8_t* src, int B, int H, int W, const 
     return DKD_OK;
 }
 
+int dkd_extract_var(dkd_ctx* ctx, const float* score, int B, int H, int W, const void* desc, int desc_dtype, int Hd,
+                    int Wd, int D, int stride, int r, float thresh, int top_k, float T, float* out_kpts,
+                    float* out_scores, void* out_desc, int32_t* out_count, int32_t* out_index, float* out_offset,
+                    const dkd_variant_params* v, void* stream) {
+    if (!ctx) return DKD_ERR_INVALID_ARG;
+    DeviceGuard dg(ctx->p.device);
+    return run(ctx, make_args(score, B, H, W, desc, desc_dtype, Hd, Wd, D, stride, r, thresh, top_k, T, out_kpts, out_scores,
+                              out_desc, out_count, out_index, out_offset, v),
+               static_cast<cudaStream_t>(stream));
+}
+
 int dkd_extract_ex(dkd_ctx* ctx, const float* score, int B, int H, int W, const void* desc, int desc_dtype, int Hd,
                    int Wd, int D, int stride, int r, float thresh, int top_k, float T, float* out_kpts,
                    float* out_scores, void* out_desc, int32_t* out_count, int32_t* out_index, float* out_offset,
                    void* stream) {
-    ExtractArgs a;
-    memset(&a, 0, sizeof(a));                               // key is compared with memcmp: no stray padding
-    a.score = score; a.B = B; a.H = H; a.W = W;
-    a.desc = desc; a.desc_dtype = desc ? desc_dtype : 0; a.Hd = desc ? Hd : 0; a.Wd = desc ? Wd : 0;
-    a.D = desc ? D : 0; a.stride = desc ? stride : 1; a.r = r; a.thresh = thresh; a.top_k = top_k; a.T = T;
-    a.out_kpts = out_kpts; a.out_scores = out_scores; a.out_desc = out_desc; a.out_count = out_count;
-    a.out_index = out_index; a.out_offset = out_offset;
-    return run(ctx, a, static_cast<cudaStream_t>(stream));
+    return dkd_extract_var(ctx, score, B, H, W, desc, desc_dtype, Hd, Wd, D, stride, r, thresh, top_k, T, out_kpts,
+                           out_scores, out_desc, out_count, out_index, out_offset, nullptr, stream);
 }
 
 int dkd_extract(dkd_ctx* ctx, const float* score, int B, int H, int W, const void* desc, int desc_dtype, int Hd,
                 int Wd, int D, int stride, int r, float thresh, int top_k, float T, float* out_kpts, float* out_scores,
                 void* out_desc, int32_t* out_count, void* stream) {
-    return dkd_extract_ex(ctx, score, B, H, W, desc, desc_dtype, Hd, Wd, D, stride, r, thresh, top_k, T, out_kpts,
-                          out_scores, out_desc, out_count, nullptr, nullptr, stream);
+    return dkd_extract_var(ctx, score, B, H, W, desc, desc_dtype, Hd, Wd, D, stride, r, thresh, top_k, T, out_kpts,
+                           out_scores, out_desc, out_count, nullptr, nullptr, nullptr, stream);
 }
 
 int dkd_extract_host(dkd_ctx* ctx, const float* score, int B, int H, int W, const void* desc, int desc_dtype, int Hd,
@@ -577,14 +790,15 @@ int dkd_extract_host(dkd_ctx* ctx, const float* score, int B, int H, int W, cons
                      float* out_scores, void* out_desc, int32_t* out_count, int32_t* out_index, float* out_offset,
                      int desc_resident, void* stream) {
     if (!ctx) return DKD_ERR_INVALID_ARG;
-    if (!score || !out_kpts || !out_scores || !out_count || B < 1 || H < 1 || W < 1 || top_k < 1)
-        return fail(ctx, DKD_ERR_INVALID_ARG, "NULL required pointer or size < 1");
-    if ((desc == nullptr) != (out_desc == nullptr))
-        return fail(ctx, DKD_ERR_INVALID_ARG, "desc and out_desc must both be NULL or both be set");
-    if (desc && (Hd < 1 || Wd < 1 || D < 1 || (desc_dtype != DKD_F32 && desc_dtype != DKD_F16)))
-        return fail(ctx, DKD_ERR_INVALID_ARG, "bad descriptor-map shape or dtype");
-    if (B > ctx->p.max_batch || H > ctx->p.max_h || W > ctx->p.max_w || top_k > ctx->p.max_top_k)
-        return fail(ctx, DKD_ERR_CAPACITY, "B, H, W or top_k above the dkd_create maxima");
+    if (!score || !out_kpts || !out_scores || !out_count)
+        return fail(ctx, DKD_ERR_INVALID_ARG, "NULL required pointer (score/out_kpts/out_scores/out_count)");
+    // every argument check that does not need a device address happens BEFORE anything is allocated or enqueued
+    const ExtractArgs chk = make_args(score, B, H, W, desc, desc_dtype, Hd, Wd, D, stride, r, thresh, top_k, T, out_kpts,
+                                      out_scores, out_desc, out_count, out_index, out_offset, nullptr);
+    int rc = validate_shapes(ctx, chk);
+    if (rc != DKD_OK) return rc;
+    if (desc_resident < 0 || desc_resident > 2) return fail(ctx, DKD_ERR_INVALID_ARG, "desc_resident must be 0, 1 or 2");
+    DeviceGuard dg(ctx->p.device);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const size_t esz = desc_dtype == DKD_F16 ? 2 : 4;
     const size_t n_score = static_cast<size_t>(B) * H * W * 4;
@@ -593,48 +807,59 @@ int dkd_extract_host(dkd_ctx* ctx, const float* score, int B, int H, int W, cons
     const size_t o_kpts = 0, o_scores = align256(o_kpts + slots * 8), o_count = align256(o_scores + slots * 4);
     const size_t o_index = align256(o_count + static_cast<size_t>(B) * 4), o_off = align256(o_index + slots * 4);
     const size_t o_desc = align256(o_off + slots * 8), n_out = align256(o_desc + (desc ? slots * D * esz : 0));
-    int rc;
-    if ((rc = grow(ctx, &ctx->st_score, &ctx->st_score_bytes, n_score)) != DKD_OK) return rc;
-    // Pinned (page-locked, mapped) host buffers are addressable from the device.  Two uses:
-    //  * descriptor map: only 4 rows per kept keypoint are ever read, so when that is a small part of the map
-    //    the gather samples it in place over PCIe instead of uploading all of it;
-    //  * outputs: when every output buffer is pinned the kernels store straight into them (no staging, no
-    //    device->host copies).
-    const void* desc_dev = nullptr;
-    if (desc) {
-        const void* zc = mapped_device_pointer(desc);
-        const size_t touched = slots * 4 * static_cast<size_t>(D) * esz;
-        const bool have = desc_resident && ctx->st_desc && ctx->st_desc_src == desc && ctx->st_desc_src_bytes == n_desc;
-        if (have) {
-            desc_dev = ctx->st_desc;
-        } else if (zc && !desc_resident && touched * 8 <= n_desc) {
-            desc_dev = zc;
-        } else {
-            if ((rc = grow(ctx, &ctx->st_desc, &ctx->st_desc_bytes, n_desc)) != DKD_OK) return rc;
-            CK(ctx, cudaMemcpyAsync(ctx->st_desc, desc, n_desc, cudaMemcpyHostToDevice, st));
-            ctx->st_desc_src = desc;
-            ctx->st_desc_src_bytes = n_desc;
-            desc_dev = ctx->st_desc;
-        }
-    }
-    CK(ctx, cudaMemcpyAsync(ctx->st_score, score, n_score, cudaMemcpyHostToDevice, st));
     void* d_kpts = mapped_device_pointer(out_kpts);
     void* d_scores = mapped_device_pointer(out_scores);
     void* d_count = mapped_device_pointer(out_count);
     void* d_desc = desc ? mapped_device_pointer(out_desc) : nullptr;
     void* d_index = out_index ? mapped_device_pointer(out_index) : nullptr;
     void* d_off = out_offset ? mapped_device_pointer(out_offset) : nullptr;
+    // Pinned (page-locked, mapped) host buffers are addressable from the device.  Two uses:
+    //  * descriptor map: only 4 rows per kept keypoint are ever read, so when that is a small part of the map
+    //    the gather samples it in place over PCIe instead of uploading all of it;
+    //  * outputs: when every output buffer is pinned (and suitably aligned) the kernels store straight into
+    //    them (no staging, no device->host copies).
     const bool direct = d_kpts && d_scores && d_count && (!desc || d_desc) && (!out_index || d_index) &&
-                        (!out_offset || d_off) && (!desc || (reinterpret_cast<uintptr_t>(d_desc) & 15) == 0);
+                        (!out_offset || d_off) && !misaligned(d_desc, 16) && !misaligned(d_kpts, 8) && !misaligned(d_off, 8) &&
+                        !misaligned(d_scores, 4) && !misaligned(d_count, 4) && !misaligned(d_index, 4);
+    if ((rc = grow(ctx, &ctx->st_score, &ctx->st_score_bytes, n_score)) != DKD_OK) return rc;
+    if (!direct && (rc = grow(ctx, &ctx->st_out, &ctx->st_out_bytes, n_out)) != DKD_OK) return rc;
+    const void* desc_dev = nullptr;
+    bool upload_desc = false;
+    if (desc) {
+        const void* zc = mapped_device_pointer(desc);
+        const size_t touched = slots * 4 * static_cast<size_t>(D) * esz;
+        const bool have = desc_resident == 1 && ctx->st_desc && ctx->st_desc_src == desc && ctx->st_desc_src_bytes == n_desc;
+        if (have) {
+            desc_dev = ctx->st_desc;
+        } else if (zc && !desc_resident && touched * 8 <= n_desc && !misaligned(zc, 16)) {
+            desc_dev = zc;
+        } else {
+            if ((rc = grow(ctx, &ctx->st_desc, &ctx->st_desc_bytes, n_desc)) != DKD_OK) return rc;
+            upload_desc = true;
+            desc_dev = ctx->st_desc;
+        }
+    }
+    // ---- from here on work is enqueued: on any error the stream is drained before returning ----------------
+    cudaError_t e = cudaSuccess;
+    if (upload_desc) {
+        ctx->st_desc_src = nullptr;                         // only an upload made by a resident call may be re-used later
+        e = cudaMemcpyAsync(ctx->st_desc, desc, n_desc, cudaMemcpyHostToDevice, st);
+        if (e == cudaSuccess && desc_resident) { ctx->st_desc_src = desc; ctx->st_desc_src_bytes = n_desc; }
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->st_score, score, n_score, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) {
+        cudaStreamSynchronize(st);
+        return fail_cuda(ctx, "host -> device copy", e);
+    }
     if (direct) {
         rc = dkd_extract_ex(ctx, static_cast<const float*>(ctx->st_score), B, H, W, desc_dev, desc_dtype, Hd, Wd, D, stride,
                             r, thresh, top_k, T, static_cast<float*>(d_kpts), static_cast<float*>(d_scores), d_desc,
                             static_cast<int32_t*>(d_count), static_cast<int32_t*>(d_index), static_cast<float*>(d_off), st);
+        e = cudaStreamSynchronize(st);
         if (rc != DKD_OK) return rc;
-        CK(ctx, cudaStreamSynchronize(st));
+        if (e != cudaSuccess) return fail_cuda(ctx, "cudaStreamSynchronize", e);
         return DKD_OK;
     }
-    if ((rc = grow(ctx, &ctx->st_out, &ctx->st_out_bytes, n_out)) != DKD_OK) return rc;
     char* so = static_cast<char*>(ctx->st_out);
     rc = dkd_extract_ex(ctx, static_cast<const float*>(ctx->st_score), B, H, W, desc_dev,
                         desc_dtype, Hd, Wd, D, stride, r, thresh, top_k, T, reinterpret_cast<float*>(so + o_kpts),
@@ -642,14 +867,19 @@ int dkd_extract_host(dkd_ctx* ctx, const float* score, int B, int H, int W, cons
                         reinterpret_cast<int32_t*>(so + o_count),
                         out_index ? reinterpret_cast<int32_t*>(so + o_index) : nullptr,
                         out_offset ? reinterpret_cast<float*>(so + o_off) : nullptr, st);
-    if (rc != DKD_OK) return rc;
-    CK(ctx, cudaMemcpyAsync(out_kpts, so + o_kpts, slots * 8, cudaMemcpyDeviceToHost, st));
-    CK(ctx, cudaMemcpyAsync(out_scores, so + o_scores, slots * 4, cudaMemcpyDeviceToHost, st));
-    CK(ctx, cudaMemcpyAsync(out_count, so + o_count, static_cast<size_t>(B) * 4, cudaMemcpyDeviceToHost, st));
-    if (out_index) CK(ctx, cudaMemcpyAsync(out_index, so + o_index, slots * 4, cudaMemcpyDeviceToHost, st));
-    if (out_offset) CK(ctx, cudaMemcpyAsync(out_offset, so + o_off, slots * 8, cudaMemcpyDeviceToHost, st));
-    if (desc) CK(ctx, cudaMemcpyAsync(out_desc, so + o_desc, slots * D * esz, cudaMemcpyDeviceToHost, st));
-    CK(ctx, cudaStreamSynchronize(st));
+    if (rc != DKD_OK) {
+        cudaStreamSynchronize(st);
+        return rc;
+    }
+    e = cudaMemcpyAsync(out_kpts, so + o_kpts, slots * 8, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(out_scores, so + o_scores, slots * 4, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(out_count, so + o_count, static_cast<size_t>(B) * 4, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && out_index) e = cudaMemcpyAsync(out_index, so + o_index, slots * 4, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && out_offset) e = cudaMemcpyAsync(out_offset, so + o_off, slots * 8, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && desc) e = cudaMemcpyAsync(out_desc, so + o_desc, slots * D * esz, cudaMemcpyDeviceToHost, st);
+    const cudaError_t es = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return fail_cuda(ctx, "device -> host copy", e);
+    if (es != cudaSuccess) return fail_cuda(ctx, "cudaStreamSynchronize", es);
     return DKD_OK;
 }
 

@@ -17,6 +17,15 @@
 
 #include "dkd.h"
 
+// -DDKD_DEBUG (libdkd_debug.so): device-side bounds checks on every workspace / shared-memory index and on
+// the mbarrier ring arithmetic; compiled out of the product library.
+#ifdef DKD_DEBUG
+#include <assert.h>
+#define DKD_ASSERT(c) assert(c)
+#else
+#define DKD_ASSERT(c) ((void)0)
+#endif
+
 namespace dkd {
 
 // ---- geometry -------------------------------------------------------------------------------
@@ -208,10 +217,11 @@ __device__ __forceinline__ void nms_rows(const float4 (&cat)[TH + 2 * R], float 
 // (no atomics, no shared counter).  The score of a candidate is re-read from the box `rows` (output
 // row o >= R has its centre in box row o - R) or, for the first R rows, from the rows still in
 // registers.  Returns the segment's count.
-template <int R>
+template <int R, bool PROD>
 __device__ __forceinline__ int nms_emit(const unsigned (&neg)[4], unsigned colmask, int X, int yc, int H, int W,
                                         const float4 (&cat)[TH + 2 * R], const float* __restrict__ rows,
-                                        uint64_t* __restrict__ seg) {
+                                        const float* __restrict__ rows2, const uint8_t* __restrict__ mask_img,
+                                        uint64_t* __restrict__ seg, int seg_room) {
     constexpr unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     unsigned rowmask = 0xffu;                                // bit TH-1-o = output row o is valid
@@ -228,13 +238,21 @@ __device__ __forceinline__ int nms_emit(const unsigned (&neg)[4], unsigned colma
     int cnt = 0;
     unsigned bal = __ballot_sync(FULL, w != 0u);
     while (bal) {                                            // warp-uniform; usually one round
+        bool take = false;
+        uint64_t key = 0ull;
         if (w != 0u) {
             const int bit = __ffs(w) - 1;
             w &= w - 1u;
             const int k = bit >> 3, o = TH - 1 - (bit & 7);
+            const int idx = (yc + o) * W + X + k;
+            // validity-mask variant: keypoints only where the mask is non-zero; masked pixels
+            // still take part in every window maximum (V5)
+            take = mask_img == nullptr || __ldg(mask_img + idx) != 0;
             float v;
             if (o >= R) {
+                DKD_ASSERT((o - R) * BOX_W + 4 * lane + k < BOX_W * TH);
                 v = rows[(o - R) * BOX_W + 4 * lane + k];
+                if constexpr (PROD) v = __fmul_rn(v, rows2[(o - R) * BOX_W + 4 * lane + k]);
             } else {
                 float4 tr = cat[R];
 #pragma unroll
@@ -242,11 +260,17 @@ __device__ __forceinline__ int nms_emit(const unsigned (&neg)[4], unsigned colma
                     if (o == j) tr = cat[R + j];
                 v = k == 0 ? tr.x : (k == 1 ? tr.y : (k == 2 ? tr.z : tr.w));
             }
-            seg[cnt + __popc(bal & ((1u << lane) - 1u))] = make_key(v, (yc + o) * W + X + k);
+            key = make_key(v, idx);
         }
-        cnt += __popc(bal);
+        const unsigned tb = __ballot_sync(FULL, take);
+        if (take) {
+            DKD_ASSERT(cnt + __popc(tb & ((1u << lane) - 1u)) < seg_room);
+            seg[cnt + __popc(tb & ((1u << lane) - 1u))] = key;
+        }
+        cnt += __popc(tb);
         bal = __ballot_sync(FULL, w != 0u);
     }
+    (void)seg_room;
     return cnt;
 }
 
@@ -288,15 +312,21 @@ __device__ __forceinline__ UnitCoords unit_coords(int u, const NmsPlan& p) {
 
 // the 2R rows above a unit (image rows y0-R .. y0+R-1), one float4 per lane and row, straight from
 // global memory (once per unit; mostly L2 hits: the unit above has just streamed them); 0 outside the image
-template <int R>
-__device__ __forceinline__ void load_head(float4 (&cat)[TH + 2 * R], const float* __restrict__ img, int X, int y0,
-                                          int H, int W) {
+__device__ __forceinline__ float4 mul4_rn(const float4 a, const float4 b) {   // heat x reliability, one rounding each
+    return make_float4(__fmul_rn(a.x, b.x), __fmul_rn(a.y, b.y), __fmul_rn(a.z, b.z), __fmul_rn(a.w, b.w));
+}
+template <int R, bool PROD>
+__device__ __forceinline__ void load_head(float4 (&cat)[TH + 2 * R], const float* __restrict__ img,
+                                          const float* __restrict__ img2, int X, int y0, int H, int W) {
 #pragma unroll
     for (int q = 0; q < 2 * R; ++q) {
         const int y = y0 - R + q;
         cat[q] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-        if (y >= 0 && y < H && X >= 0 && X < W)              // W % 4 == 0 and X % 4 == 0: all four or none
+        if (y >= 0 && y < H && X >= 0 && X < W) {            // W % 4 == 0 and X % 4 == 0: all four or none
             cat[q] = __ldg(reinterpret_cast<const float4*>(img + static_cast<size_t>(y) * W + X));
+            if constexpr (PROD)
+                cat[q] = mul4_rn(cat[q], __ldg(reinterpret_cast<const float4*>(img2 + static_cast<size_t>(y) * W + X)));
+        }
     }
 }
 
@@ -308,20 +338,24 @@ __device__ __forceinline__ void load_head(float4 (&cat)[TH + 2 * R], const float
 // arithmetic, the candidate scores picked out of the box), its other NMS_STAGES-1 boxes stay in flight.
 // No CTA-wide barrier after set-up: a warp only ever waits for its own boxes.  Dynamic smem:
 // NMS_SMEM_BYTES, 128-byte aligned; warp w owns NMS_STAGES boxes.  NEGT: thr_up <= 0 (see nms_rows).
-template <int R, bool NEGT>
-__global__ void __launch_bounds__(NMS_WARPS * 32, 2) k_nms_tma(const __grid_constant__ CUtensorMap tmap,
-                                                               const __grid_constant__ NmsPlan p,
-                                                               const float* __restrict__ score,
-                                                               uint64_t* __restrict__ cand,
-                                                               int* __restrict__ seg_cnt) {
+template <int R, bool NEGT, bool PROD>
+__global__ void __launch_bounds__(NMS_WARPS * 32, PROD ? 1 : 2) k_nms_tma(const __grid_constant__ CUtensorMap tmap,
+                                                                          const __grid_constant__ CUtensorMap tmap2,
+                                                                          const __grid_constant__ NmsPlan p,
+                                                                          const float* __restrict__ score,
+                                                                          const float* __restrict__ score2,
+                                                                          const uint8_t* __restrict__ mask,
+                                                                          uint64_t* __restrict__ cand,
+                                                                          int* __restrict__ seg_cnt) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t bars[NMS_WARPS * NMS_STAGES];
+    constexpr int STAGE_BYTES = PROD ? 2 * BOX_BYTES : BOX_BYTES;      // PROD: heat box | reliability box
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int first = blockIdx.x * NMS_WARPS + warp, step = gridDim.x * NMS_WARPS;
     const int n_my = first < p.units ? (p.units - first + step - 1) / step : 0;
     pdl_launch_dependents();                                 // k_select may fill the SMs this grid leaves
     if (n_my == 0) return;
-    unsigned char* my_smem = smem_raw + warp * NMS_STAGES * BOX_BYTES;
+    unsigned char* my_smem = smem_raw + warp * NMS_STAGES * STAGE_BYTES;
     uint64_t* bar = bars + warp * NMS_STAGES;
 
     const uint64_t policy = l2_evict_first_policy();
@@ -332,8 +366,11 @@ __global__ void __launch_bounds__(NMS_WARPS * 32, 2) k_nms_tma(const __grid_cons
         if (iit >= n_my) return;
         const int s = issued % NMS_STAGES;
         if (lane == 0) {
-            mbar_arrive_expect_tx(&bar[s], BOX_BYTES);
-            tma_load_tile(my_smem + s * BOX_BYTES, &tmap, &bar[s], iu.x0 - HALO_X, iu.y0 + R + TH * ic, iu.b, policy);
+            mbar_arrive_expect_tx(&bar[s], STAGE_BYTES);
+            tma_load_tile(my_smem + s * STAGE_BYTES, &tmap, &bar[s], iu.x0 - HALO_X, iu.y0 + R + TH * ic, iu.b, policy);
+            if constexpr (PROD)
+                tma_load_tile(my_smem + s * STAGE_BYTES + BOX_BYTES, &tmap2, &bar[s], iu.x0 - HALO_X, iu.y0 + R + TH * ic,
+                              iu.b, policy);
         }
         ++issued;
         if (++ic == iu.nch) {
@@ -345,6 +382,7 @@ __global__ void __launch_bounds__(NMS_WARPS * 32, 2) k_nms_tma(const __grid_cons
     UnitCoords cu = iu;
     if (lane == 0) {
         tma_prefetch_desc(&tmap);
+        if constexpr (PROD) tma_prefetch_desc(&tmap2);
 #pragma unroll
         for (int s = 0; s < NMS_STAGES; ++s) mbar_init(&bar[s], 1);
         fence_mbar_init();
@@ -354,26 +392,35 @@ __global__ void __launch_bounds__(NMS_WARPS * 32, 2) k_nms_tma(const __grid_cons
     for (int s = 0; s < NMS_STAGES; ++s) issue_box();
 
     int consumed = 0;
+    const size_t img_px = static_cast<size_t>(p.H) * p.W;
     for (int it = 0; it < n_my; ++it) {
         const int X = cu.x0 - HALO_X + 4 * lane;             // image column of this lane's first pixel
         float4 cat[TH + 2 * R];                              // rows yc-R .. yc+R+TH-1 of the current strip-tile
-        load_head<R>(cat, score + static_cast<size_t>(cu.b) * p.H * p.W, X, cu.y0, p.H, p.W);
+        load_head<R, PROD>(cat, score + cu.b * img_px, PROD ? score2 + cu.b * img_px : nullptr, X, cu.y0, p.H, p.W);
         const unsigned colmask = strip_colmask(X, p.W, R);
         const int u = first + it * step;                     // the unit's candidate segment: p.cpu * SEG_CAP keys
+        DKD_ASSERT(u >= 0 && u < p.units);
         uint64_t* useg = cand + static_cast<size_t>(u) * (p.cpu * SEG_CAP);
+        const uint8_t* mask_img = mask ? mask + cu.b * img_px : nullptr;
         int ucnt = 0;                                        // warp-uniform running count of the segment
         for (int c = 0; c < cu.nch; ++c) {
             const int s = consumed % NMS_STAGES;
+            DKD_ASSERT(consumed < issued && issued - consumed <= NMS_STAGES);
             mbar_wait(&bar[s], (consumed / NMS_STAGES) & 1);
-            const float* rows = reinterpret_cast<const float*>(my_smem + s * BOX_BYTES);
+            const float* rows = reinterpret_cast<const float*>(my_smem + s * STAGE_BYTES);
+            const float* rows2 = PROD ? rows + BOX_W * TH : nullptr;
             {
                 const float4* src = reinterpret_cast<const float4*>(rows) + lane;
 #pragma unroll
-                for (int o = 0; o < TH; ++o) cat[2 * R + o] = src[o * 32];
+                for (int o = 0; o < TH; ++o) {
+                    cat[2 * R + o] = src[o * 32];
+                    if constexpr (PROD) cat[2 * R + o] = mul4_rn(cat[2 * R + o], src[BOX_W * TH / 4 + o * 32]);
+                }
             }
             unsigned neg[4];
             nms_rows<R, NEGT>(cat, p.thr_up, neg);
-            ucnt += nms_emit<R>(neg, colmask, X, cu.y0 + TH * c, p.H, p.W, cat, rows, useg + ucnt);
+            ucnt += nms_emit<R, PROD>(neg, colmask, X, cu.y0 + TH * c, p.H, p.W, cat, rows, rows2, mask_img, useg + ucnt,
+                                      p.cpu * SEG_CAP - ucnt);
             __syncwarp();                                    // every lane is done with stage s
             issue_box();                                     // (the other NMS_STAGES-1 boxes stay in flight meanwhile)
             ++consumed;
@@ -388,18 +435,24 @@ __global__ void __launch_bounds__(NMS_WARPS * 32, 2) k_nms_tma(const __grid_cons
 // ---- k_nms_plain: same strip math, one strip-tile per warp, rows fetched with ordinary loads ---------
 // (any W, any alignment: scalar loads, 0 outside the image)
 constexpr int PLAIN_WARPS = 4;
-template <int R>
+template <int R, bool PROD>
 __global__ void __launch_bounds__(PLAIN_WARPS * 32) k_nms_plain(const float* __restrict__ score,
+                                                                const float* __restrict__ score2,
+                                                                const uint8_t* __restrict__ mask,
                                                                 const __grid_constant__ NmsPlan p, int total,
                                                                 uint64_t* __restrict__ cand,
                                                                 int* __restrict__ seg_cnt) {
+    __shared__ __align__(16) float boxes[PLAIN_WARPS][BOX_W * TH];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int t = blockIdx.x * PLAIN_WARPS + warp;          // unit == strip-tile (nms_plan: cpu = 1 on this path)
+    pdl_launch_dependents();
     if (t >= total) return;
     const int tpi = p.strips_x * p.chunks_y;
     const int b = t / tpi, rem = t - b * tpi;
     const int cy = rem / p.strips_x, x0 = (rem - cy * p.strips_x) * STRIP_W, y0 = cy * TH;
-    const float* img = score + static_cast<size_t>(b) * p.H * p.W;
+    const size_t img_px = static_cast<size_t>(p.H) * p.W;
+    const float* img = score + b * img_px;
+    const float* img2 = PROD ? score2 + b * img_px : nullptr;
     const int X = x0 - HALO_X + 4 * lane;
     float4 cat[TH + 2 * R];
 #pragma unroll
@@ -407,19 +460,24 @@ __global__ void __launch_bounds__(PLAIN_WARPS * 32) k_nms_plain(const float* __r
         const int gy = y0 - R + q;
         float v[4];
 #pragma unroll
-        for (int k = 0; k < 4; ++k)
-            v[k] = (gy >= 0 && gy < p.H && X + k >= 0 && X + k < p.W) ? __ldg(img + static_cast<size_t>(gy) * p.W + X + k) : 0.0f;
+        for (int k = 0; k < 4; ++k) {
+            v[k] = 0.0f;
+            if (gy >= 0 && gy < p.H && X + k >= 0 && X + k < p.W) {
+                const size_t e = static_cast<size_t>(gy) * p.W + X + k;
+                v[k] = __ldg(img + e);
+                if constexpr (PROD) v[k] = __fmul_rn(v[k], __ldg(img2 + e));
+            }
+        }
         cat[q] = make_float4(v[0], v[1], v[2], v[3]);
     }
-    __shared__ __align__(16) float boxes[PLAIN_WARPS][BOX_W * TH];
-    float4* box = reinterpret_cast<float4*>(boxes[warp]) + lane;
+    float4* box = reinterpret_cast<float4*>(boxes[warp]) + lane;   // (already the product: emit reads it as is)
 #pragma unroll
     for (int o = 0; o < TH; ++o) box[o * 32] = cat[2 * R + o];
     __syncwarp();
     unsigned neg[4];
     nms_rows<R, true>(cat, p.thr_up, neg);
-    const int cnt = nms_emit<R>(neg, strip_colmask(X, p.W, R), X, y0, p.H, p.W, cat, boxes[warp],
-                                cand + static_cast<size_t>(t) * SEG_CAP);
+    const int cnt = nms_emit<R, false>(neg, strip_colmask(X, p.W, R), X, y0, p.H, p.W, cat, boxes[warp], nullptr,
+                                       mask ? mask + b * img_px : nullptr, cand + static_cast<size_t>(t) * SEG_CAP, SEG_CAP);
     if (lane == 0) seg_cnt[t] = cnt;
 }
 
@@ -457,11 +515,41 @@ __device__ __forceinline__ int block_sum_1024(int v, int* s_red) {
     return r;
 }
 
+// The refinement that follows reads the (2r+1)^2 window of every kept keypoint: k_select, which knows the kept
+// indices first and has bandwidth to spare, asks L2 for those rows (first and last element of each window row:
+// one or two sectors), so that k_refine_gather's dependent window loads hit L2 instead of paying a DRAM round trip.
+struct SelPrefetch {
+    const float* score;                 // NULL: no prefetch
+    const float* score2;                // reliability map (product variant) or NULL
+    int W, r;
+    uint32_t div_m, div_s1, div_s2;     // idx / W (FastDiv)
+    size_t img_px;
+};
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+__device__ __forceinline__ void prefetch_window(const SelPrefetch& pf, int b, int idx) {
+    if (pf.score == nullptr) return;
+    const uint32_t t = __umulhi(pf.div_m, static_cast<uint32_t>(idx));
+    const int y = static_cast<int>((t + ((static_cast<uint32_t>(idx) - t) >> pf.div_s1)) >> pf.div_s2), x = idx - y * pf.W;
+    const float* row = pf.score + b * pf.img_px + static_cast<size_t>(y - pf.r) * pf.W + (x - pf.r);
+    for (int j = 0; j <= 2 * pf.r; ++j, row += pf.W) {
+        prefetch_l2(row);
+        prefetch_l2(row + 2 * pf.r);
+    }
+    if (pf.score2 != nullptr) {
+        row = pf.score2 + b * pf.img_px + static_cast<size_t>(y - pf.r) * pf.W + (x - pf.r);
+        for (int j = 0; j <= 2 * pf.r; ++j, row += pf.W) {
+            prefetch_l2(row);
+            prefetch_l2(row + 2 * pf.r);
+        }
+    }
+}
+
 __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __restrict__ cand,
                                                            const int* __restrict__ seg_cnt, int tpi, int seg_cap,
-                                                           int top_k, int idx_shift,
+                                                           int top_k, int idx_shift, const SelPrefetch pf,
                                                            int32_t* __restrict__ sel_idx,
-                                                           int32_t* __restrict__ out_count) {
+                                                           int32_t* __restrict__ out_count,
+                                                           int32_t* __restrict__ out_total) {
     extern __shared__ __align__(16) unsigned char sel_smem[];
     uint64_t* keys = reinterpret_cast<uint64_t*>(sel_smem);            // SORT_CAP entries (gathered, unordered)
     uint64_t* sorted = keys + SORT_CAP;                                // SORT_CAP entries (bucket order)
@@ -554,6 +642,7 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
         klo = __reduce_min_sync(FULL, klo);
         if (lane == 0 && khi >= klo) { atomicMax(&s_hi, khi); atomicMin(&s_lo, klo); }
         __syncthreads();
+        if (pass == 0 && tid == 0 && out_total != nullptr) out_total[b] = s_n;   // C_b: every candidate, before the cap
         if (s_n <= SORT_CAP) break;                         // block-uniform; always true in the second pass
         {
             uint64_t prefix = 0;
@@ -692,7 +781,10 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
                 rank += r8;
             }
             for (; j < s1; ++j) rank += sorted[j] > k ? 1 : 0;
-            if (rank < K) out[rank] = key_index(k);
+            if (rank < K) {
+                out[rank] = key_index(k);
+                prefetch_window(pf, b, key_index(k));
+            }
         }
         return;
     }
@@ -718,14 +810,23 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
             __syncthreads();
         }
     }
-    for (int i = tid; i < K; i += SEL_THREADS) out[i] = key_index(keys[i]);
+    for (int i = tid; i < K; i += SEL_THREADS) {
+        out[i] = key_index(keys[i]);
+        prefetch_window(pf, b, key_index(keys[i]));
+    }
 }
 
-// ---- k_refine_gather: one G-lane group per output slot (b, i) ---------------------------------------
-// G = 8, 16 or 32 lanes = the number of 16-byte chunks of one descriptor row rounded up to a power of
-// two (D=128 f16 / D=64 f32: 16 lanes, two keypoints per warp; D=256 f16: 32; D=64 f16: 8), so every
-// lane issues exactly one 16-byte load per corner row and no lane idles in the gather.
-// grid = (ceil(top_k / (RG_THREADS / G)), B): the image index is blockIdx.y (no division by top_k).
+// ---- k_refine_gather: steps a3, a4, a5 for RG_SLOTS consecutive output slots of one image per CTA ------
+// Phase 1 (warp 0, ONE THREAD PER KEYPOINT): index -> (y, x), the (2r+1)^2 window with every load of a row
+//   batch in flight at once, soft-argmax offset, keypoint / score / offset stores (coalesced across the
+//   lanes), and the four bilinear corner rows + weights of the keypoint, left in shared memory.  The
+//   refinement is scalar work per keypoint: done this way it costs ~8 warp instructions per keypoint
+//   instead of the ~110 of a lane-group-per-keypoint layout whose lanes mostly idle.
+// Phase 2 (all warps, G lanes per keypoint): G = 8, 16 or 32 = the number of 16-byte chunks of one
+//   descriptor row rounded up to a power of two (D=128 f16 / D=64 f32: 16; D=256 f16: 32; D=64 f16: 8),
+//   so every lane issues exactly one 16-byte load per corner row; fp32 FMAs, shuffle L2 norm, 16-byte stores.
+// grid = (ceil(top_k / RG_SLOTS), B): the image index is blockIdx.y (no division by top_k).
+constexpr int RG_SLOTS = 32;             // output slots per CTA = lanes of the refining warp
 
 // exact unsigned division by a runtime constant (Granlund-Montgomery): q = (t + ((n - t) >> s1)) >> s2,
 // t = umulhi(m, n); host-computed by make_fastdiv; exact for every 32-bit n.
@@ -818,6 +919,7 @@ __device__ __forceinline__ uint4 float_to_chunk(const float* f) {
 
 struct RGParams {
     const float* score;
+    const float* score2;                // reliability map of the heat x reliability variant, else NULL
     int H, W;
     FastDiv divW;                       // idx -> (y, x)
     const int32_t* sel_idx;             // [B, top_k] linear index, -1 in padding
@@ -832,120 +934,298 @@ struct RGParams {
     float* out_off;
     unsigned char* out_desc;
     int origin_x, origin_y;             // letterbox offset subtracted from the stored coordinates
+    int score_mode;                     // DKD_SCORE_RAW: S at the integer peak; DKD_SCORE_BILINEAR: S at the refined point
+    int vec_window;                     // W % 4 == 0 and a 16-byte aligned map: window rows as aligned 16-byte chunks
 };
 
-// DT: DKD_F32 / DKD_F16 descriptor maps, or -1 for keypoints only.  G: lanes per keypoint.
-template <int DT, int G>
-__global__ void __launch_bounds__(RG_THREADS, 6) k_refine_gather(const __grid_constant__ RGParams p) {
-    constexpr int ITERS = (G == 32) ? DKD_MAX_ROW_BYTES / 16 / 32 : 1;   // chunks per lane
-    const int gl = threadIdx.x & (G - 1);                   // lane within the group
-    const unsigned gmask = (G == 32) ? 0xffffffffu : (((1u << G) - 1u) << ((threadIdx.x & 31) & ~(G - 1)));
-    const int i_img = blockIdx.x * (RG_THREADS / G) + threadIdx.x / G;
-    if (i_img >= p.top_k) return;                           // whole groups leave together
-    const int b = blockIdx.y;
-    const size_t slot = static_cast<size_t>(b) * p.top_k + i_img;
-    pdl_wait();                                              // the selection of k_select is complete and visible
-    const int idx = __ldg(p.sel_idx + slot);
+// score value at one pixel: S, or heat x reliability rounded once to fp32 (the product variant)
+template <bool PROD>
+__device__ __forceinline__ float score_at(const float* __restrict__ S, const float* __restrict__ S2, size_t e) {
+    if constexpr (PROD) return __fmul_rn(__ldg(S + e), __ldg(S2 + e));
+    else return __ldg(S + e);
+}
 
-    if (idx < 0) {                                          // step a5: zero padding
-        if (gl < 2) p.out_kpts[2 * slot + gl] = 0.0f;
-        if (gl == 2) p.out_scores[slot] = 0.0f;
-        if (p.out_off != nullptr && gl >= 4 && gl < 6) p.out_off[2 * slot + gl - 4] = 0.0f;
-        if constexpr (DT >= 0) {
-            uint4* o = reinterpret_cast<uint4*>(p.out_desc + slot * p.nchunk * 16);
-            for (int ch = gl; ch < p.nchunk; ch += G) o[ch] = make_uint4(0u, 0u, 0u, 0u);
-        }
-        return;
-    }
-
-    // ---- step a3: soft-argmax over the (2r+1)^2 window.  Orbit q < (r+1)^2 = the mirror images
-    // {(+-i, +-j)}, i, j >= 0, of one window element; differences of mirrored weights are formed
-    // first, so a window symmetric about an axis refines to exactly 0 along it.
-    const int W = p.W;
-    const int y = static_cast<int>(fast_div(static_cast<uint32_t>(idx), p.divW)), x = idx - y * W;
-    const float* S = p.score + static_cast<size_t>(b) * p.H * W;
-    const float c = __ldg(S + idx);
-    const int r1 = p.r + 1, norb = r1 * r1, inv_r1 = (256 + p.r) / r1;   // j = q / r1 for q < 25
-    float sx = 0.0f, sy = 0.0f, z = 0.0f;
-    for (int q = gl; q < norb; q += G) {
-        const int j = (q * inv_r1) >> 8, i = q - j * r1;
-        const float vpp = __ldg(S + (y + j) * W + (x + i));
-        const float vmp = __ldg(S + (y + j) * W + (x - i));
-        const float vpm = __ldg(S + (y - j) * W + (x + i));
-        const float vmm = __ldg(S + (y - j) * W + (x - i));
-        const float wpp = ex2_approx((vpp - c) * p.kscale);
-        const float wmp = ex2_approx((vmp - c) * p.kscale);
-        const float wpm = ex2_approx((vpm - c) * p.kscale);
-        const float wmm = ex2_approx((vmm - c) * p.kscale);
-        const float mi = i > 0 ? 1.0f : 0.0f, mj = j > 0 ? 1.0f : 0.0f;
-        sx += static_cast<float>(i) * ((wpp - wmp) + mj * (wpm - wmm));
-        sy += static_cast<float>(j) * ((wpp - wpm) + mi * (wmp - wmm));
-        z += wpp + mi * wmp + mj * (wpm + mi * wmm);
-    }
+// ---- step a3 for one keypoint, one thread: soft-argmax over the (2R+1)^2 window ----------------------
+// w(i,j) = 2^((S[y+j,x+i] - c) * kscale); column sums Wcol, row sums Wrow in a fixed order, then the
+// antisymmetric pairing of the definition (dx = sum_a a (Wcol[+a] - Wcol[-a]) / Z): a window symmetric about
+// an axis gives two bitwise-equal sums, i.e. an offset of exactly 0 along it.  RPB rows of loads are in
+// flight at once (9 / 25 / 21 / 27 loads for R = 1..4).
+template <int R, bool PROD, bool VEC>
+__device__ __forceinline__ void refine_window(const float* __restrict__ S, const float* __restrict__ S2, int W,
+                                              int y, int x, float c, float kscale, float& dx, float& dy) {
+    constexpr int N = 2 * R + 1;
+    constexpr int RPB = R <= 2 ? N : 3;
+    float col[N], row[N];
 #pragma unroll
-    for (int o = G / 2; o > 0; o >>= 1) {
-        sx += __shfl_xor_sync(gmask, sx, o);
-        sy += __shfl_xor_sync(gmask, sy, o);
-        z += __shfl_xor_sync(gmask, z, o);
-    }
-    const float inv_z = __frcp_rn(z);                        // z >= 1 (the centre weight is exactly 1)
-    const float dx = sx * inv_z, dy = sy * inv_z;
-    if (gl == 0) {
-        *reinterpret_cast<float2*>(p.out_kpts + 2 * slot) = make_float2(static_cast<float>(x - p.origin_x) + dx, static_cast<float>(y - p.origin_y) + dy);
-        p.out_scores[slot] = c;                              // raw S at the integer peak (G7)
-        if (p.out_off != nullptr) *reinterpret_cast<float2*>(p.out_off + 2 * slot) = make_float2(dx, dy);
-    }
-
-    // ---- step a4: bilinear gather of the four corner rows (16-byte loads), fp32 accumulate, L2 norm
-    if constexpr (DT >= 0) {
-        int x0, x1, y0, y1;
-        float fx, fy;
-        sample_axis(x, dx, p.ax, x0, x1, fx);
-        sample_axis(y, dy, p.ay, y0, y1, fy);
-        const float w00 = (1.0f - fy) * (1.0f - fx), w01 = (1.0f - fy) * fx;
-        const float w10 = fy * (1.0f - fx), w11 = fy * fx;
-        const size_t rowb = static_cast<size_t>(p.nchunk) * 16;
-        const int Wd = p.ax.n;
-        const unsigned char* base = p.desc + static_cast<size_t>(b) * p.img_bytes;
-        const uint4* p00 = reinterpret_cast<const uint4*>(base + (static_cast<size_t>(y0) * Wd + x0) * rowb);
-        const uint4* p01 = reinterpret_cast<const uint4*>(base + (static_cast<size_t>(y0) * Wd + x1) * rowb);
-        const uint4* p10 = reinterpret_cast<const uint4*>(base + (static_cast<size_t>(y1) * Wd + x0) * rowb);
-        const uint4* p11 = reinterpret_cast<const uint4*>(base + (static_cast<size_t>(y1) * Wd + x1) * rowb);
-        constexpr int N = ChunkT<DT >= 0 ? DT : 0>::N;
-        const uint64_t policy = l2_evict_first_policy();
-        float acc[ITERS][N];
-        float ss = 0.0f;
+    for (int i = 0; i < N; ++i) col[i] = 0.0f, row[i] = 0.0f;
 #pragma unroll
-        for (int it = 0; it < ITERS; ++it) {
-            const int ch = gl + G * it;
-            if (ch < p.nchunk) {
-                const uint4 q00 = ld_stream16(p00 + ch, policy), q01 = ld_stream16(p01 + ch, policy);
-                const uint4 q10 = ld_stream16(p10 + ch, policy), q11 = ld_stream16(p11 + ch, policy);
-                float a[N], bq[N], cq[N], dq[N];
-                chunk_to_float<DT >= 0 ? DT : 0>(q00, a);
-                chunk_to_float<DT >= 0 ? DT : 0>(q01, bq);
-                chunk_to_float<DT >= 0 ? DT : 0>(q10, cq);
-                chunk_to_float<DT >= 0 ? DT : 0>(q11, dq);
+    for (int j0 = 0; j0 < N; j0 += RPB) {
+        float v[RPB][N];
+        if constexpr (VEC && !PROD) {
+            // Every lane of the refining warp reads its own window: a scalar load per element costs one
+            // L1 wavefront per lane and element (26 per keypoint at r = 2).  With W % 4 == 0 and a 16-byte
+            // aligned map, a window row is instead the 2 (r <= 2) or 3 aligned 16-byte chunks that contain
+            // it, and element i is picked out of them by the lane's chunk offset o = (x - r) & 3.
+            constexpr int NCH = R <= 2 ? 2 : 3;
+            const int xs = x - R, o = xs & 3;
+            float f[RPB][4 * NCH];
 #pragma unroll
-                for (int e = 0; e < N; ++e) {
-                    const float d = fmaf(w11, dq[e], fmaf(w10, cq[e], fmaf(w01, bq[e], w00 * a[e])));
-                    acc[it][e] = d;
-                    ss = fmaf(d, d, ss);
+            for (int jj = 0; jj < RPB; ++jj) {
+                if (j0 + jj < N) {
+                    const float4* rp = reinterpret_cast<const float4*>(S + static_cast<size_t>(y - R + j0 + jj) * W + (xs - o));
+#pragma unroll
+                    for (int k = 0; k < NCH; ++k) {
+                        float4 q = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                        if (4 * k < o + N) q = __ldg(rp + k);     // (a chunk past the window may lie past the map)
+                        f[jj][4 * k] = q.x; f[jj][4 * k + 1] = q.y; f[jj][4 * k + 2] = q.z; f[jj][4 * k + 3] = q.w;
+                    }
+                }
+            }
+#pragma unroll
+            for (int jj = 0; jj < RPB; ++jj) {
+                if (j0 + jj < N) {
+#pragma unroll
+                    for (int i = 0; i < N; ++i) {
+                        const float m0 = (o & 1) ? f[jj][i + 1] : f[jj][i];
+                        const float m1 = (o & 1) ? f[jj][i + 3] : f[jj][i + 2];   // i + 3 <= 2R + 3 < 4 NCH
+                        v[jj][i] = (o & 2) ? m1 : m0;
+                    }
+                }
+            }
+        } else {
+#pragma unroll
+            for (int jj = 0; jj < RPB; ++jj) {
+                if (j0 + jj < N) {
+                    const size_t e = static_cast<size_t>(y - R + j0 + jj) * W + (x - R);
+#pragma unroll
+                    for (int i = 0; i < N; ++i) v[jj][i] = score_at<PROD>(S, S2, e + i);
                 }
             }
         }
 #pragma unroll
-        for (int o = G / 2; o > 0; o >>= 1) ss += __shfl_xor_sync(gmask, ss, o);
-        const float inv = __frcp_rn(fmaxf(sqrtf(ss), 1e-12f));
-        uint4* o = reinterpret_cast<uint4*>(p.out_desc + slot * rowb);
+        for (int jj = 0; jj < RPB; ++jj) {
+            if (j0 + jj < N) {
 #pragma unroll
-        for (int it = 0; it < ITERS; ++it) {
-            const int ch = gl + G * it;
-            if (ch < p.nchunk) {
-                float f[N];
+                for (int i = 0; i < N; ++i) {
+                    const float w = ex2_approx((v[jj][i] - c) * kscale);
+                    col[i] += w;
+                    row[j0 + jj] += w;
+                }
+            }
+        }
+    }
+    float z = col[0], sx = 0.0f, sy = 0.0f;
 #pragma unroll
-                for (int e = 0; e < N; ++e) f[e] = acc[it][e] * inv;
-                o[ch] = float_to_chunk<DT >= 0 ? DT : 0>(f);
+    for (int i = 1; i < N; ++i) z += col[i];
+#pragma unroll
+    for (int a = 1; a <= R; ++a) {
+        sx = fmaf(static_cast<float>(a), col[R + a] - col[R - a], sx);
+        sy = fmaf(static_cast<float>(a), row[R + a] - row[R - a], sy);
+    }
+    const float inv_z = __frcp_rn(z);                        // z >= 1 (the centre weight is exactly 1)
+    dx = sx * inv_z;
+    dy = sy * inv_z;
+}
+
+template <bool PROD, bool VEC>
+__device__ __forceinline__ void refine_dispatch(int r, const float* __restrict__ S, const float* __restrict__ S2, int W,
+                                                int y, int x, float c, float kscale, float& dx, float& dy) {
+    switch (r) {                                             // (uniform)
+        case 1: refine_window<1, PROD, VEC>(S, S2, W, y, x, c, kscale, dx, dy); break;
+        case 2: refine_window<2, PROD, VEC>(S, S2, W, y, x, c, kscale, dx, dy); break;
+        case 3: refine_window<3, PROD, VEC>(S, S2, W, y, x, c, kscale, dx, dy); break;
+        default: refine_window<4, PROD, VEC>(S, S2, W, y, x, c, kscale, dx, dy); break;
+    }
+}
+
+struct SampleInfo {                     // phase 1 -> phase 2, one per slot (shared memory)
+    uint32_t o00, o01, o10, o11;        // descriptor-row index (v * Wd + u) of the four corners; o00 = ~0: padding slot
+    float w00, w01, w10, w11;
+};
+
+// DT: DKD_F32 / DKD_F16 descriptor maps, or -1 for keypoints only (launched with one warp per CTA).
+// G: lanes per keypoint in phase 2.  PROD: score = heat x reliability.
+template <int DT, int G, bool PROD>
+__global__ void __launch_bounds__(RG_THREADS, 4) k_refine_gather(const __grid_constant__ RGParams p) {
+    __shared__ __align__(16) SampleInfo s_info[RG_SLOTS];
+    const int b = blockIdx.y;
+    const int slot0 = blockIdx.x * RG_SLOTS;                 // first slot (within the image) of this CTA
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    pdl_wait();                                              // the selection of k_select is complete and visible
+
+    if (warp == 0) {
+        const int i_img = slot0 + lane;
+        SampleInfo si;
+        si.o00 = 0xffffffffu; si.o01 = si.o10 = si.o11 = 0u;
+        si.w00 = si.w01 = si.w10 = si.w11 = 0.0f;
+        if (i_img < p.top_k) {
+            const size_t slot = static_cast<size_t>(b) * p.top_k + i_img;
+            const int idx = __ldg(p.sel_idx + slot);
+            float2 kp = make_float2(0.0f, 0.0f), off = make_float2(0.0f, 0.0f);
+            float sc = 0.0f;                                 // step a5: zero padding
+            if (idx >= 0) {
+                const int W = p.W;
+                const int y = static_cast<int>(fast_div(static_cast<uint32_t>(idx), p.divW)), x = idx - y * W;
+                const float* S = p.score + static_cast<size_t>(b) * p.H * W;
+                const float* S2 = PROD ? p.score2 + static_cast<size_t>(b) * p.H * W : nullptr;
+                const float c = score_at<PROD>(S, S2, static_cast<size_t>(idx));
+                float dx, dy;
+                if (p.vec_window) refine_dispatch<PROD, true>(p.r, S, S2, W, y, x, c, p.kscale, dx, dy);
+                else refine_dispatch<PROD, false>(p.r, S, S2, W, y, x, c, p.kscale, dx, dy);
+                kp = make_float2(static_cast<float>(x - p.origin_x) + dx, static_cast<float>(y - p.origin_y) + dy);
+                off = make_float2(dx, dy);
+                sc = c;                                      // raw S at the integer peak (G7)
+                if (p.score_mode == DKD_SCORE_BILINEAR) {    // variant: S interpolated at the refined point (V2)
+                    const float fdx = floorf(dx), fdy = floorf(dy);
+                    int x0 = x + static_cast<int>(fdx), y0 = y + static_cast<int>(fdy);
+                    float fx = dx - fdx, fy = dy - fdy;
+                    if (x0 >= W - 1) { x0 = W - 1; fx = 0.0f; }      // |dx| <= r <= border: x0 >= 0 always
+                    if (y0 >= p.H - 1) { y0 = p.H - 1; fy = 0.0f; }
+                    const int x1 = x0 + 1 < W - 1 ? x0 + 1 : W - 1, y1 = y0 + 1 < p.H - 1 ? y0 + 1 : p.H - 1;
+                    const float s00 = score_at<PROD>(S, S2, static_cast<size_t>(y0) * W + x0);
+                    const float s01 = score_at<PROD>(S, S2, static_cast<size_t>(y0) * W + x1);
+                    const float s10 = score_at<PROD>(S, S2, static_cast<size_t>(y1) * W + x0);
+                    const float s11 = score_at<PROD>(S, S2, static_cast<size_t>(y1) * W + x1);
+                    const float top = fmaf(fx, s01 - s00, s00), bot = fmaf(fx, s11 - s10, s10);
+                    sc = fmaf(fy, bot - top, top);
+                }
+                if constexpr (DT >= 0) {
+                    int x0, x1, y0, y1;
+                    float fx, fy;
+                    sample_axis(x, dx, p.ax, x0, x1, fx);
+                    sample_axis(y, dy, p.ay, y0, y1, fy);
+                    const uint32_t Wd = static_cast<uint32_t>(p.ax.n);
+                    si.o00 = static_cast<uint32_t>(y0) * Wd + x0; si.o01 = static_cast<uint32_t>(y0) * Wd + x1;
+                    si.o10 = static_cast<uint32_t>(y1) * Wd + x0; si.o11 = static_cast<uint32_t>(y1) * Wd + x1;
+                    si.w00 = (1.0f - fy) * (1.0f - fx); si.w01 = (1.0f - fy) * fx;
+                    si.w10 = fy * (1.0f - fx); si.w11 = fy * fx;
+                }
+            }
+            reinterpret_cast<float2*>(p.out_kpts)[slot] = kp;
+            p.out_scores[slot] = sc;
+            if (p.out_off != nullptr) reinterpret_cast<float2*>(p.out_off)[slot] = off;
+        }
+        if constexpr (DT >= 0) {
+            DKD_ASSERT(lane < RG_SLOTS);
+            s_info[lane] = si;
+        }
+    }
+    if constexpr (DT < 0) return;                            // keypoints only
+
+    // ---- step a4: bilinear gather of the four corner rows (16-byte loads), fp32 accumulate, L2 norm
+    if constexpr (DT >= 0) {
+        __syncthreads();
+        constexpr int ITERS = (G == 32) ? DKD_MAX_ROW_BYTES / 16 / 32 : 1;   // chunks per lane
+        constexpr int KPR = RG_THREADS / G;                  // keypoints per round
+        constexpr int N = ChunkT<DT >= 0 ? DT : 0>::N;
+        const int gl = threadIdx.x & (G - 1);                // lane within the group
+        const unsigned gmask = (G == 32) ? 0xffffffffu : (((1u << G) - 1u) << ((threadIdx.x & 31) & ~(G - 1)));
+        const size_t rowb = static_cast<size_t>(p.nchunk) * 16;
+        const unsigned char* base = p.desc + static_cast<size_t>(b) * p.img_bytes;
+        const uint64_t policy = l2_evict_first_policy();
+        if constexpr (ITERS == 1 && RG_SLOTS / KPR <= 2) {
+            // one 16-byte chunk per lane and corner row: the corner loads of BOTH of this group's keypoints are
+            // issued before any of them is used (8 loads in flight per lane)
+            constexpr int U = RG_SLOTS / KPR;
+            uint4 q[U][4];
+            SampleInfo si[U];
+            bool live[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int k = threadIdx.x / G + u * KPR;
+                si[u] = s_info[k];
+                live[u] = slot0 + k < p.top_k && si[u].o00 != 0xffffffffu && gl < p.nchunk;
+                if (live[u]) {
+                    q[u][0] = ld_stream16(reinterpret_cast<const uint4*>(base + si[u].o00 * rowb) + gl, policy);
+                    q[u][1] = ld_stream16(reinterpret_cast<const uint4*>(base + si[u].o01 * rowb) + gl, policy);
+                    q[u][2] = ld_stream16(reinterpret_cast<const uint4*>(base + si[u].o10 * rowb) + gl, policy);
+                    q[u][3] = ld_stream16(reinterpret_cast<const uint4*>(base + si[u].o11 * rowb) + gl, policy);
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int k = threadIdx.x / G + u * KPR;
+                const int i_img = slot0 + k;
+                if (i_img >= p.top_k) break;                 // whole groups leave together
+                uint4* o = reinterpret_cast<uint4*>(p.out_desc + (static_cast<size_t>(b) * p.top_k + i_img) * rowb);
+                if (si[u].o00 == 0xffffffffu) {              // padding slot: zero descriptor
+                    if (gl < p.nchunk) o[gl] = make_uint4(0u, 0u, 0u, 0u);
+                    continue;
+                }
+                float acc[N];
+                float ss = 0.0f;
+                if (live[u]) {
+                    float a[N], bq[N], cq[N], dq[N];
+                    chunk_to_float<DT >= 0 ? DT : 0>(q[u][0], a);
+                    chunk_to_float<DT >= 0 ? DT : 0>(q[u][1], bq);
+                    chunk_to_float<DT >= 0 ? DT : 0>(q[u][2], cq);
+                    chunk_to_float<DT >= 0 ? DT : 0>(q[u][3], dq);
+#pragma unroll
+                    for (int e = 0; e < N; ++e) {
+                        const float d = fmaf(si[u].w11, dq[e], fmaf(si[u].w10, cq[e], fmaf(si[u].w01, bq[e], si[u].w00 * a[e])));
+                        acc[e] = d;
+                        ss = fmaf(d, d, ss);
+                    }
+                }
+#pragma unroll
+                for (int sft = G / 2; sft > 0; sft >>= 1) ss += __shfl_xor_sync(gmask, ss, sft);
+                const float inv = __frcp_rn(fmaxf(sqrtf(ss), 1e-12f));
+                if (live[u]) {
+                    float f[N];
+#pragma unroll
+                    for (int e = 0; e < N; ++e) f[e] = acc[e] * inv;
+                    o[gl] = float_to_chunk<DT >= 0 ? DT : 0>(f);
+                }
+            }
+        } else {
+#pragma unroll 1
+            for (int k = threadIdx.x / G; k < RG_SLOTS; k += KPR) {
+                const int i_img = slot0 + k;
+                if (i_img >= p.top_k) break;                 // whole groups leave together
+                const SampleInfo si = s_info[k];
+                uint4* o = reinterpret_cast<uint4*>(p.out_desc + (static_cast<size_t>(b) * p.top_k + i_img) * rowb);
+                if (si.o00 == 0xffffffffu) {                 // padding slot: zero descriptor
+                    for (int ch = gl; ch < p.nchunk; ch += G) o[ch] = make_uint4(0u, 0u, 0u, 0u);
+                    continue;
+                }
+                const uint4* p00 = reinterpret_cast<const uint4*>(base + si.o00 * rowb);
+                const uint4* p01 = reinterpret_cast<const uint4*>(base + si.o01 * rowb);
+                const uint4* p10 = reinterpret_cast<const uint4*>(base + si.o10 * rowb);
+                const uint4* p11 = reinterpret_cast<const uint4*>(base + si.o11 * rowb);
+                float acc[ITERS][N];
+                float ss = 0.0f;
+#pragma unroll
+                for (int it = 0; it < ITERS; ++it) {
+                    const int ch = gl + G * it;
+                    if (ch < p.nchunk) {
+                        const uint4 q00 = ld_stream16(p00 + ch, policy), q01 = ld_stream16(p01 + ch, policy);
+                        const uint4 q10 = ld_stream16(p10 + ch, policy), q11 = ld_stream16(p11 + ch, policy);
+                        float a[N], bq[N], cq[N], dq[N];
+                        chunk_to_float<DT >= 0 ? DT : 0>(q00, a);
+                        chunk_to_float<DT >= 0 ? DT : 0>(q01, bq);
+                        chunk_to_float<DT >= 0 ? DT : 0>(q10, cq);
+                        chunk_to_float<DT >= 0 ? DT : 0>(q11, dq);
+#pragma unroll
+                        for (int e = 0; e < N; ++e) {
+                            const float d = fmaf(si.w11, dq[e], fmaf(si.w10, cq[e], fmaf(si.w01, bq[e], si.w00 * a[e])));
+                            acc[it][e] = d;
+                            ss = fmaf(d, d, ss);
+                        }
+                    }
+                }
+#pragma unroll
+                for (int sft = G / 2; sft > 0; sft >>= 1) ss += __shfl_xor_sync(gmask, ss, sft);
+                const float inv = __frcp_rn(fmaxf(sqrtf(ss), 1e-12f));
+#pragma unroll
+                for (int it = 0; it < ITERS; ++it) {
+                    const int ch = gl + G * it;
+                    if (ch < p.nchunk) {
+                        float f[N];
+#pragma unroll
+                        for (int e = 0; e < N; ++e) f[e] = acc[it][e] * inv;
+                        o[ch] = float_to_chunk<DT >= 0 ? DT : 0>(f);
+                    }
+                }
             }
         }
     }

@@ -50,7 +50,7 @@ def test_library_is_sm100a_with_tma():
     assert "sm_100a" in elf
     full = subprocess.run(["cuobjdump", "-sass", path], capture_output=True, text=True).stdout
     funcs = [f for f in full.split("Function : ")[1:] if "k_nms_tma" in f.split("\n")[0]]
-    assert len(funcs) == 8                                       # radius 1..4 x {thr_up > 0, thr_up <= 0}
+    assert len(funcs) == 16                                      # radius 1..4 x {thr_up > 0, thr_up <= 0} x {S, heat x reliability}
     sass = funcs[0]
     assert "UTMALDG" in sass                                     # TMA tile loads in the NMS kernel
     assert "FMNMX3" in sass                                      # 3-input max of the separable window maximum

@@ -335,6 +335,71 @@ def test_capture_safe_inside_a_user_graph(ctx):
         assert torch.equal(getattr(want, n), getattr(out, n)), n
 
 
+def test_graph_cache_is_keyed_on_shapes_not_pointers():
+    """1000 calls that rotate through fresh output buffers and several input maps (and change thresh / T) stay
+    correct, and the library never captures or instantiates a second graph for the shape: the kernel nodes of the
+    cached graph are re-pointed in place."""
+    import paper_2607_01757_b200 as dkd
+    c = dkd.DKD(2, 96, 256, 128, 64)
+    try:
+        inputs = []
+        for seed in range(4):
+            score, desc = small_inputs(2, 96, 256, seed=40 + seed, nblobs=150, D=64, dtype=torch.float16, stride=1)
+            inputs.append((score, score.cuda(), desc))
+        params = [(0.2, 0.1), (0.3, 0.1), (0.2, 0.25)]
+        refs = {}
+        for i, (score, _, desc) in enumerate(inputs):
+            for j, (th, T) in enumerate(params):
+                refs[(i, j)] = oracle.extract(score.numpy(), desc.cpu().numpy(), 1, 2, th, 128, T)
+        outs = []
+        for it in range(1000):
+            i, j = it % 4, (it // 4) % 3
+            res = c.extract(inputs[i][1], inputs[i][2], 1, 2, params[j][0], 128, params[j][1])   # fresh outputs every call
+            outs.append((i, j, res))
+            if len(outs) == 50:                                   # check in batches (keeps 50 output sets alive at once)
+                for (ii, jj, rr) in outs:
+                    compare(rr, refs[(ii, jj)], torch.float16)
+                outs = []
+        st = c.graph_stats()
+        assert st["instantiated"] == 1, st                        # one shape -> one graph, ever
+        assert st["updated"] >= 990 and st["stream"] == 0, st
+        # a different shape (other top_k) is a second graph; the first one is still valid afterwards
+        c.extract(inputs[0][1], inputs[0][2], 1, 2, 0.2, 64, 0.1)
+        res = c.extract(inputs[1][1], inputs[1][2], 1, 2, 0.2, 128, 0.1)
+        compare(res, refs[(1, 0)], torch.float16)
+        assert c.graph_stats()["instantiated"] == 2
+    finally:
+        c.close()
+
+
+def test_unaligned_outputs_are_rejected_not_faulted(ctx):
+    import paper_2607_01757_b200 as dkd
+    s = torch.zeros((1, 32, 128), device="cuda")
+    out = ctx.alloc_outputs(1, 8, None, 0)
+    flat = torch.zeros(1 * 8 * 2 + 1, device="cuda")
+    out.kpts = flat[1:].view(1, 8, 2)                             # 4-byte aligned only: the kernel stores float2
+    with pytest.raises(dkd.DKDError) as e:
+        ctx.extract(s, None, 1, 2, 0.2, 8, 0.1, out=out)
+    assert e.value.code == -2
+    out = ctx.alloc_outputs(1, 8, None, 0)
+    out.scores = torch.zeros((1, 9), device="cuda")               # wrong shape: caught by the binding
+    with pytest.raises(dkd.DKDError):
+        ctx.extract(s, None, 1, 2, 0.2, 8, 0.1, out=out)
+    torch.cuda.synchronize()                                      # the context is still usable
+    ctx.extract(s, None, 1, 2, 0.2, 8, 0.1)
+    torch.cuda.synchronize()
+
+
+def test_host_path_validates_before_any_copy(ctx):
+    import paper_2607_01757_b200 as dkd
+    s = torch.zeros((1, 32, 128)).pin_memory()
+    for bad in (dict(r=0), dict(T=0.0), dict(r=7), dict(top_k=0)):
+        kw = dict(r=2, T=0.1, top_k=8)
+        kw.update(bad)
+        with pytest.raises(dkd.DKDError):
+            ctx.extract_host(s, None, 1, kw["r"], 0.2, kw["top_k"], kw["T"])
+
+
 def test_deterministic_across_runs(ctx):
     score, desc = small_inputs(2, 150, 400, seed=12, nblobs=500, D=64, dtype=torch.float16, stride=1)
     sd = score.cuda()

@@ -30,6 +30,14 @@ def _oracle_fn(score, desc, **kw):
             "desc": torch.from_numpy(R.desc)}
 
 
+def _dataclass_fn(score, desc, **kw):
+    """Returns the binding's own result type (DKDResult), as DKD.extract does; `desc`/`offsets` may be None."""
+    from paper_2607_01757_b200.binding import DKDResult
+    d = _oracle_fn(score, desc, **kw)
+    return DKDResult(kpts=d["kpts"].float(), scores=d["scores"], desc=None, count=d["count"], index=d["index"],
+                     offsets=None)
+
+
 def _worker(rank, world, port, q):
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
@@ -42,9 +50,18 @@ def _worker(rank, world, port, q):
     # timing reduction used by bench.py: max over ranks
     t = torch.tensor([1.0 + rank], dtype=torch.float64)
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    # the real return type (a dataclass with None fields), a batch smaller than the world, an empty batch
+    got_dc = sharded_extract(_dataclass_fn, score, desc, rank, world, gather=True, **kw)
+    got_one = sharded_extract(_dataclass_fn, score[:1], desc[:1], rank, world, gather=True, **kw)
+    got_none = sharded_extract(_dataclass_fn, score[:0], desc[:0], rank, world, gather=True, **kw)
+    local = sharded_extract(_dataclass_fn, score, desc, rank, world, gather=False, **kw)
     if rank == 0:
         want = _oracle_fn(score, desc, **kw)
         ok = all(torch.equal(got[k], want[k]) for k in want) and float(t) == float(world)
+        ok = ok and sorted(got_dc) == ["count", "index", "kpts", "scores"]
+        ok = ok and torch.equal(got_dc["index"], want["index"]) and torch.equal(got_dc["kpts"], want["kpts"].float())
+        ok = ok and got_one["index"].shape[0] == 1 and torch.equal(got_one["index"][0], want["index"][0])
+        ok = ok and got_none == {} and local.index.shape[0] == 3   # rank 0 owns 3 of the 5 images
         q.put(bool(ok))
     dist.barrier()
     dist.destroy_process_group()
