@@ -249,6 +249,76 @@ int dkd_pre_padded_size(int H, int W, int grid, int* Hp, int* Wp, int* oy, int* 
 int dkd_preprocess(dkd_ctx* ctx, const uint8_t* src, int B, int H, int W, const dkd_pre_params* p, void* dst,
                    void* stream);
 
+/*
+ * ---- consumers of the descriptor output (M1..M8) -----------------------
+ *
+ * dkd_match — cosine nearest-neighbour matching with a Lowe ratio test between P pairs of padded descriptor sets
+ * ("cosine nearest-neighbour matching with a Lowe ratio test"; descriptors are l2-normalised, Eq. 1
+ * PAPER.md:101, so the cosine is the dot product, Eq. 4; sets are zero-padded to the cap,
+ * PAPER.md:139; the temporal and the stereo pair go in one batch).  For every row i < count_a[p]:
+ *   s_ij = a_i . b_j over j < count_b[p];  j1 = argmax_j s_ij (ties: smallest j);  s2 = max_{j != j1} s_ij (-1 if none);
+ *   ratio test on the distances of unit vectors, d^2 = max(0, 2 - 2 s): keep iff d1^2 < ratio^2 d2^2 (ratio >= 1e9: off);
+ *   mutual != 0: keep only if i is also the nearest neighbour of j1 (ties: smallest i).
+ * The similarity matrix is formed on the tensor cores (tcgen05, fp16 inputs, fp32 accumulation) and never written to
+ * memory: the row-wise top-2 is fused into the epilogue.
+ *   desc_a   device [P,Na,D] f16 (the out_desc of dkd_extract), 16-byte aligned; desc_b device [P,Nb,D] likewise
+ *   count_a  device [P] i32 valid rows (the out_count of dkd_extract), or NULL = Na; count_b likewise
+ *   D        64, 128, 192 or 256; dtype must be DKD_F16 (else DKD_ERR_UNSUPPORTED)
+ *   out_match device [P,Na] i32: j1 or -1 (no match / padding row);  out_sim device [P,Na,2] f32 (s1, s2) or NULL
+ * Asynchronous on `stream`.  Uses a context-owned scratch buffer that is grown (cudaMalloc) when a call needs more than
+ * any call before it: such a call must not be made while `stream` is being captured.
+ */
+int dkd_match(dkd_ctx* ctx, const void* desc_a, const int32_t* count_a, int Na,
+              const void* desc_b, const int32_t* count_b, int Nb, int D, int dtype, int P,
+              float ratio, int mutual, int32_t* out_match, float* out_sim, void* stream);
+
+/*
+ * dkd_retrieval_scan — brute-force loop-candidate retrieval ("cosine similarity between the current
+ * descriptor g_t and a past descriptor g_k", Eq. 4; "a fixed window of the most recent keyframes is excluded";
+ * "Candidates with sim > tau_sim are ranked by similarity"; "brute-force scan over the keyframe database, O(n)";
+ * 50 most recent excluded, tau_sim = 0.60; g in R^{32*384}).
+ *   db       device [n,D] f16|f32, rows in insertion order (row n-1 is the newest keyframe), 16-byte aligned
+ *   query    device [D] same dtype, 16-byte aligned;  D * elemsize a multiple of 16 and <= 32768
+ *   out_sim  device [n] f32: q . db_k for EVERY row (fp32 accumulation), or NULL
+ *   out_cand device [max_cand] i32: rows k < n - n_exclude with sim > tau (strict), ranked by (sim desc, k asc),
+ *            -1 padded; out_cand_sim device [max_cand] f32 or NULL; out_count device [1] i32
+ * Asynchronous on `stream`; scratch buffer as for dkd_match.  One pass over the database: HBM-bound.
+ */
+int dkd_retrieval_scan(dkd_ctx* ctx, const void* db, int dtype, int n, int D, const void* query,
+                       int n_exclude, float tau, int max_cand,
+                       float* out_sim, int32_t* out_cand, float* out_cand_sim, int32_t* out_count, void* stream);
+
+/*
+ * ---- per-match stereo validation and covariance weighting (S1..S4, C1..C4) -----------
+ *
+ * dkd_stereo_validate: rectified pinhole pair, right camera at +baseline along x.  For left keypoint i
+ * and right keypoint j = match[i] (match == NULL: j = i; j < 0: invalid): disparity d = uL - uR must exceed d_min
+ * ("negligible disparity"); depth z = fx baseline / d, X = (uL - cx) z / fx, Y = ((vL + vR)/2 - cy) z / fy; kept iff
+ * z_min < z < z_max and the reprojection error |vL - vR| / 2 (both views) <= max_reproj (1.5 px).
+ *   kpts_l device [n,2] f32 (x,y), kpts_r device [m,2] f32, both 8-byte aligned; match device [n] i32 or NULL
+ *   out_xyz device [n,3] f32; out_disp, out_err device [n] f32 or NULL; out_valid device [n] u8
+ */
+typedef struct {
+    float fx, fy, cx, cy, baseline;
+    float d_min, z_min, z_max, max_reproj;
+} dkd_stereo_params;
+int dkd_stereo_validate(dkd_ctx* ctx, const float* kpts_l, const float* kpts_r, const int32_t* match, int n,
+                        const dkd_stereo_params* p, float* out_xyz, float* out_disp, float* out_err,
+                        uint8_t* out_valid, void* stream);
+
+/*
+ * dkd_cov_sqrt_info (App. A-B, Eq. 9-11): per keypoint, from the predicted lower-triangular factor
+ * L = [[l11,0],[l21,l22]]: Sigma_px = scale^2 L L^T + floor_px I; Sigma_n = J Sigma_px J^T, J = diag(1/fx, 1/fy);
+ * Sigma_eff^-1 = max(lambda, lambda_min) Sigma_n^-1; Omega = the upper-triangular factor with Omega^T Omega =
+ * Sigma_eff^-1; if Sigma_px is not positive definite or an input is non-finite: Omega = I / sigma0, ok = 0.
+ *   L device [n,3] f32 (l11, l21, l22); out_omega device [n,4] f32 row-major 2x2; out_ok device [n] u8 or NULL
+ */
+typedef struct {
+    float scale, floor_px, fx, fy, lambda, lambda_min, sigma0;
+} dkd_cov_params;
+int dkd_cov_sqrt_info(dkd_ctx* ctx, const float* L, int n, const dkd_cov_params* p, float* out_omega,
+                      uint8_t* out_ok, void* stream);
+
 /* Measurement mode (DKD_OPT_PROFILE = 1): waits for the events of the most recent dkd_extract* call
  * on this context and writes the device time of each of its kernels, in launch order, to
  * ms[0..n) (host; milliseconds; entries past the launch count are left untouched).  Returns the

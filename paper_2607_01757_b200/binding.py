@@ -19,6 +19,7 @@ EXPORTED_SYMBOLS = (
     "dkd_create", "dkd_destroy", "dkd_last_error", "dkd_workspace_bytes", "dkd_set_option",
     "dkd_extract", "dkd_extract_ex", "dkd_extract_var", "dkd_extract_host", "dkd_launches_per_extract", "dkd_version",
     "dkd_profile_read", "dkd_kernel_name", "dkd_pre_padded_size", "dkd_preprocess", "dkd_graph_stats",
+    "dkd_match", "dkd_retrieval_scan", "dkd_stereo_validate", "dkd_cov_sqrt_info",
 )
 
 
@@ -42,6 +43,14 @@ class _PreParams(ctypes.Structure):
 class _VariantParams(ctypes.Structure):
     _fields_ = [("reliability", ctypes.c_void_p), ("valid_mask", ctypes.c_void_p), ("nms_iters", ctypes.c_int),
                 ("score_mode", ctypes.c_int), ("out_total", ctypes.c_void_p)]
+
+
+class _StereoParams(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_float) for n in ("fx", "fy", "cx", "cy", "baseline", "d_min", "z_min", "z_max", "max_reproj")]
+
+
+class _CovParams(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_float) for n in ("scale", "floor_px", "fx", "fy", "lam", "lambda_min", "sigma0")]
 
 
 def lib_path() -> str:
@@ -93,6 +102,14 @@ def load_library():
     L.dkd_extract_ex.argtypes = common + [vp, vp, vp]
     L.dkd_extract_var.restype = i
     L.dkd_extract_var.argtypes = common + [vp, vp, ctypes.POINTER(_VariantParams), vp]
+    L.dkd_match.restype = i
+    L.dkd_match.argtypes = [vp, vp, vp, i, vp, vp, i, i, i, i, f, i, vp, vp, vp]
+    L.dkd_retrieval_scan.restype = i
+    L.dkd_retrieval_scan.argtypes = [vp, vp, i, i, i, vp, i, f, i, vp, vp, vp, vp, vp]
+    L.dkd_stereo_validate.restype = i
+    L.dkd_stereo_validate.argtypes = [vp, vp, vp, vp, i, ctypes.POINTER(_StereoParams), vp, vp, vp, vp, vp]
+    L.dkd_cov_sqrt_info.restype = i
+    L.dkd_cov_sqrt_info.argtypes = [vp, vp, i, ctypes.POINTER(_CovParams), vp, vp, vp]
     u64p = ctypes.POINTER(ctypes.c_uint64)
     L.dkd_graph_stats.restype = i
     L.dkd_graph_stats.argtypes = [vp, u64p, u64p, u64p, u64p]
@@ -182,6 +199,83 @@ class DKD:
         v = [ctypes.c_uint64() for _ in range(4)]
         self._check(self._L.dkd_graph_stats(self._h, *[ctypes.byref(x) for x in v]))
         return dict(zip(("instantiated", "updated", "replayed", "stream"), (int(x.value) for x in v)))
+
+    # -- consumers of the descriptor output (dkd_match / dkd_retrieval_scan / dkd_stereo_validate / dkd_cov_sqrt_info) --
+    def _stream(self, stream):
+        st = torch.cuda.current_stream(self.device) if stream is None else stream
+        return ctypes.c_void_p(st.cuda_stream)
+
+    def match(self, desc_a: torch.Tensor, desc_b: torch.Tensor, count_a: Optional[torch.Tensor] = None,
+              count_b: Optional[torch.Tensor] = None, ratio: float = 0.8, mutual: bool = False, want_sim: bool = True,
+              stream=None):
+        """dkd_match.  desc_a [P,Na,D], desc_b [P,Nb,D] f16 cuda contiguous; counts [P] i32 cuda or None.
+        Returns (match [P,Na] i32, sim [P,Na,2] f32 or None)."""
+        for t in (desc_a, desc_b):
+            if not (t.is_cuda and t.is_contiguous() and t.dim() == 3):
+                raise DKDError(-1, "descriptor sets must be contiguous CUDA [P,N,D] tensors")
+        P, Na, D = desc_a.shape
+        if desc_b.shape[0] != P or desc_b.shape[2] != D or desc_a.dtype != desc_b.dtype:
+            raise DKDError(-1, "desc_a / desc_b disagree in P, D or dtype")
+        for c in (count_a, count_b):
+            if c is not None and not (c.is_cuda and c.dtype == torch.int32 and c.is_contiguous() and c.numel() == P):
+                raise DKDError(-1, "counts must be contiguous CUDA int32 [P] tensors")
+        Nb = desc_b.shape[1]
+        out = torch.empty((P, Na), dtype=torch.int32, device=desc_a.device)
+        sim = torch.empty((P, Na, 2), dtype=torch.float32, device=desc_a.device) if want_sim else None
+        self._check(self._L.dkd_match(self._h, _ptr(desc_a), _ptr(count_a), Na, _ptr(desc_b), _ptr(count_b), Nb, D,
+                                      _dt(desc_a), P, float(ratio), int(bool(mutual)), _ptr(out), _ptr(sim),
+                                      self._stream(stream)))
+        return out, sim
+
+    def retrieval_scan(self, db: torch.Tensor, query: torch.Tensor, n_exclude: int = 50, tau: float = 0.60,
+                       max_cand: int = 16, want_sim: bool = True, stream=None):
+        """dkd_retrieval_scan.  db [n,D], query [D] f16|f32 cuda contiguous.
+        Returns (sim [n] f32 or None, cand [max_cand] i32, cand_sim [max_cand] f32, count [1] i32)."""
+        if not (db.is_cuda and db.is_contiguous() and db.dim() == 2 and query.is_cuda and query.is_contiguous()
+                and query.dim() == 1 and query.shape[0] == db.shape[1] and query.dtype == db.dtype):
+            raise DKDError(-1, "db must be a contiguous CUDA [n,D] tensor and query a matching [D] tensor")
+        n, D = db.shape
+        sim = torch.empty((n,), dtype=torch.float32, device=db.device) if want_sim else None
+        cand = torch.empty((max_cand,), dtype=torch.int32, device=db.device)
+        csim = torch.empty((max_cand,), dtype=torch.float32, device=db.device)
+        cnt = torch.empty((1,), dtype=torch.int32, device=db.device)
+        self._check(self._L.dkd_retrieval_scan(self._h, _ptr(db), _dt(db), n, D, _ptr(query), int(n_exclude), float(tau),
+                                               int(max_cand), _ptr(sim), _ptr(cand), _ptr(csim), _ptr(cnt),
+                                               self._stream(stream)))
+        return sim, cand, csim, cnt
+
+    def stereo_validate(self, kpts_l: torch.Tensor, kpts_r: torch.Tensor, match: Optional[torch.Tensor], fx, fy, cx, cy,
+                        baseline, d_min, z_min, z_max, max_reproj=1.5, stream=None):
+        """dkd_stereo_validate.  kpts_l [n,2], kpts_r [m,2] f32 cuda; match [n] i32 cuda or None.
+        Returns (valid [n] u8, xyz [n,3], disparity [n], reproj_err [n])."""
+        for t in (kpts_l, kpts_r):
+            if not (t.is_cuda and t.is_contiguous() and t.dtype == torch.float32 and t.dim() == 2 and t.shape[1] == 2):
+                raise DKDError(-1, "keypoints must be contiguous CUDA float32 [n,2] tensors")
+        if match is not None and not (match.is_cuda and match.dtype == torch.int32 and match.is_contiguous()
+                                      and match.numel() == kpts_l.shape[0]):
+            raise DKDError(-1, "match must be a contiguous CUDA int32 [n] tensor")
+        n = kpts_l.shape[0]
+        dev = kpts_l.device
+        xyz = torch.empty((n, 3), dtype=torch.float32, device=dev)
+        disp = torch.empty((n,), dtype=torch.float32, device=dev)
+        err = torch.empty((n,), dtype=torch.float32, device=dev)
+        valid = torch.empty((n,), dtype=torch.uint8, device=dev)
+        p = _StereoParams(fx, fy, cx, cy, baseline, d_min, z_min, z_max, max_reproj)
+        self._check(self._L.dkd_stereo_validate(self._h, _ptr(kpts_l), _ptr(kpts_r), _ptr(match), n, ctypes.byref(p),
+                                                _ptr(xyz), _ptr(disp), _ptr(err), _ptr(valid), self._stream(stream)))
+        return valid, xyz, disp, err
+
+    def cov_sqrt_info(self, L: torch.Tensor, scale, floor_px, fx, fy, lam, lam_min, sigma0, stream=None):
+        """dkd_cov_sqrt_info.  L [n,3] f32 cuda (l11, l21, l22).  Returns (omega [n,2,2] f32, ok [n] u8)."""
+        if not (L.is_cuda and L.is_contiguous() and L.dtype == torch.float32 and L.dim() == 2 and L.shape[1] == 3):
+            raise DKDError(-1, "L must be a contiguous CUDA float32 [n,3] tensor")
+        n = L.shape[0]
+        om = torch.empty((n, 2, 2), dtype=torch.float32, device=L.device)
+        ok = torch.empty((n,), dtype=torch.uint8, device=L.device)
+        p = _CovParams(scale, floor_px, fx, fy, lam, lam_min, sigma0)
+        self._check(self._L.dkd_cov_sqrt_info(self._h, _ptr(L), n, ctypes.byref(p), _ptr(om), _ptr(ok),
+                                              self._stream(stream)))
+        return om, ok
 
     # -- fused input pre-processing (dkd_pre_padded_size / dkd_preprocess) ---------------------
     @staticmethod

@@ -107,6 +107,7 @@ struct dkd_ctx {
     void* st_score; size_t st_score_bytes;
     void* st_desc;  size_t st_desc_bytes;
     void* st_out;   size_t st_out_bytes;
+    void* scratch[2]; size_t scratch_bytes[2];              // dkd_ctx_scratch: match partials, retrieval-scan workspace
     const void* st_desc_src; size_t st_desc_src_bytes;      // the host map st_desc holds as a RESIDENT copy (else NULL)
     // options
     int use_graph, use_tma, use_pdl, profile, nms_cpu, origin_x, origin_y, sel_prefetch;
@@ -570,6 +571,26 @@ int dkd_ctx_fail(dkd_ctx* ctx, int code, const char* msg, const char* detail) {
     return fail(ctx, code, "%s%s", msg, detail ? detail : "");
 }
 
+void* dkd_ctx_scratch(dkd_ctx* ctx, int slot, size_t bytes) {
+    if (slot < 0 || slot > 1) return nullptr;
+    if (bytes < 256) bytes = 256;
+    if (grow(ctx, &ctx->scratch[slot], &ctx->scratch_bytes[slot], bytes) != DKD_OK) return nullptr;
+    return ctx->scratch[slot];
+}
+int dkd_internal_select(dkd_ctx* ctx, const uint64_t* cand, const int* seg_cnt, int tpi, int seg_cap, int top_k, int n_items,
+                        int32_t* sel_idx, int32_t* out_count, cudaStream_t st) {
+    int idx_shift = 0;
+    while (((static_cast<long long>(n_items) - 1) >> idx_shift) >= NBT) ++idx_shift;
+    SelPrefetch pf;
+    memset(&pf, 0, sizeof(pf));
+    KLaunch k;
+    prep(k, k_select, dim3(1), dim3(SEL_THREADS), SEL_SMEM_BYTES, false, cand, seg_cnt, tpi, seg_cap, top_k, idx_shift, pf,
+         sel_idx, out_count, static_cast<int32_t*>(nullptr));
+    const cudaError_t e = launch(k, st, false);
+    if (e != cudaSuccess) return fail_cuda(ctx, "k_select launch", e);
+    return DKD_OK;
+}
+
 extern "C" {
 
 const char* dkd_version(void) {
@@ -658,6 +679,8 @@ int dkd_destroy(dkd_ctx* ctx) {
     if (ctx->st_score) cudaFree(ctx->st_score);
     if (ctx->st_desc) cudaFree(ctx->st_desc);
     if (ctx->st_out) cudaFree(ctx->st_out);
+    for (int i = 0; i < 2; ++i)
+        if (ctx->scratch[i]) cudaFree(ctx->scratch[i]);
     delete ctx;
     return DKD_OK;
 }

@@ -84,3 +84,10 @@ struct DeviceGuard {
 int dkd_ctx_device(const dkd_ctx* ctx);
 int dkd_ctx_num_sms(const dkd_ctx* ctx);
 int dkd_ctx_fail(dkd_ctx* ctx, int code, const char* msg, const char* detail);   // sets dkd_last_error, returns code
+// context-owned device scratch buffer `slot` (0: match partials, 1: retrieval scan) of at least `bytes` bytes, grown
+// with cudaMalloc when too small (not capture-safe then); NULL on failure (dkd_last_error set)
+void* dkd_ctx_scratch(dkd_ctx* ctx, int slot, size_t bytes);
+// k_select on caller-provided candidate segments (one "image"): ranks the keys of `tpi` segments of `seg_cap` keys by
+// (score desc, index asc) into sel_idx[top_k] (-1 padded) and out_count[1]; n_items bounds the indices
+int dkd_internal_select(dkd_ctx* ctx, const uint64_t* cand, const int* seg_cnt, int tpi, int seg_cap, int top_k, int n_items,
+                        int32_t* sel_idx, int32_t* out_count, cudaStream_t st);

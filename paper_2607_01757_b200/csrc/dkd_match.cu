@@ -1,0 +1,718 @@
+// dkd_match.cu — the consumers of the descriptor output:
+//   k_match_tc        cosine nearest-neighbour matching of two padded, l2-normalised fp16 descriptor sets
+//                     (PAPER.md:157): S = A B^T on the 5th-generation tensor cores (tcgen05.mma, fp32
+//                     accumulators in TMEM, operands staged by TMA with the 128-byte swizzle), with the
+//                     row-wise top-2 fused into the epilogue (tcgen05.ld) — S never reaches memory.
+//   k_match_finalize  merge of the column splits, Lowe ratio test, optional mutual check.
+//   k_scan            brute-force cosine scan of one global descriptor over the keyframe database
+//                     (Eq. 4, 348): an HBM-bound GEMV with the tau gate and the
+//                     skip-recent window; the ranked candidate list comes from k_select (dkd_kernels.cuh).
+//   k_stereo / k_cov  per-match stereo validation and covariance-weighted square-root
+//                     information (Eq. 9-11): elementwise.
+#include <cuda.h>
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+#include <string.h>
+
+#include "dkd.h"
+#include "dkd_host.h"
+
+#ifdef DKD_DEBUG
+#include <assert.h>
+#define DKD_ASSERT(c) assert(c)
+#else
+#define DKD_ASSERT(c) ((void)0)
+#endif
+
+namespace dkd {
+
+// ---- PTX wrappers (mbarrier, TMA, tcgen05) ------------------------------------------------------------
+__device__ __forceinline__ uint32_t m_smem_u32(const void* p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
+__device__ __forceinline__ void m_mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(m_smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void m_fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void m_mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(m_smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void m_mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(m_smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void m_mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "MWAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra MDONE;\n"
+        "bra MWAIT;\n"
+        "MDONE:\n"
+        "}" ::"r"(m_smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void m_tma_load_3d(void* dst, const CUtensorMap* tmap, uint64_t* bar, int c0, int c1, int c2) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+        ::"r"(m_smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(tmap)), "r"(m_smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
+        : "memory");
+}
+__device__ __forceinline__ void m_prefetch_tmap(const CUtensorMap* tmap) {
+    asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(tmap)) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+// one warp allocates `cols` TMEM columns (power of two >= 32); the base address lands in shared memory
+__device__ __forceinline__ void tc_alloc(uint32_t* dst_smem, uint32_t cols) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(m_smem_u32(dst_smem)), "r"(cols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tc_dealloc(uint32_t taddr, uint32_t cols) {
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(cols) : "memory");
+}
+// D[tmem] (+)= A[smem desc] * B[smem desc]^T, fp16 inputs, fp32 accumulate; issued by ONE thread
+__device__ __forceinline__ void tc_mma_f16(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n"
+        "}" ::"r"(tmem_d),
+        "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+// the mbarrier receives one arrival when every tcgen05.mma issued so far by this thread has completed
+__device__ __forceinline__ void tc_commit(uint64_t* bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(m_smem_u32(bar)) : "memory");
+}
+// 32 lanes x 32 consecutive fp32 columns: thread t of the warp receives row (lane base + t), columns c .. c+31
+__device__ __forceinline__ void tc_ld_32x32(uint32_t taddr, uint32_t (&v)[32]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+          "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]), "=r"(v[16]),
+          "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]), "=r"(v[24]),
+          "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr)
+        : "memory");
+}
+__device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// ---- k_match_tc -------------------------------------------------------------------------------------------
+// One CTA = one block of BM = 128 rows of A (one pair p) against the column tiles [t0, t1) of B.
+//   warp 0   TMA producer: the A block once (KB boxes of 64 k-elements x 128 rows, 128-byte swizzle), then one
+//            B tile (BN = 128 rows, all of K) per ring stage;
+//   warp 1   allocates TMEM and issues the MMAs: per B tile KB x 4 tcgen05.mma of 128 x 128 x 16 into one of two
+//            accumulator buffers (128 lanes x 128 fp32 columns each); tcgen05.commit frees the smem stage and
+//            publishes the accumulator;
+//   warps 2..9  epilogue: warp w reads TMEM lanes 32 (w % 4) .. +31 (the hardware's lane quadrant of the warp),
+//            columns 64 h .. 64 h + 63 with h = (w - 2) / 4: every thread owns ONE ROW of S and keeps its running
+//            (best, arg best, second best) in registers — no cross-thread reduction; columns are visited in
+//            increasing order and the comparison is strict, so ties keep the smallest column (M2).
+// Rows >= count_a and columns >= count_b (the zero padding of PAPER.md:139) are masked out.
+constexpr int MT_BM = 128, MT_BN = 128, MT_KBOX = 64;            // KBOX fp16 = 128 bytes = the swizzle span
+constexpr int MT_THREADS = 320;                                  // 10 warps
+constexpr int MT_TMEM_COLS = 256;                                // two accumulator buffers
+constexpr int MT_MAX_KB = 4;                                     // D <= 256
+
+struct MatchRec {                      // partial result of one row over one column split
+    float best, second;
+    int arg;
+    int pad;
+};
+
+struct MatchParams {
+    const int32_t* count_a;            // [P] valid rows of A, device (NULL: Na)
+    const int32_t* count_b;            // [P]
+    int Na, Nb, KB;                    // KB = D / 64
+    int splits, stages;
+    MatchRec* part;                    // [P, splits, Na]
+};
+
+__device__ __forceinline__ uint64_t mt_desc(uint32_t smem_addr) {
+    // K-major operand, 128-byte swizzle: rows of 128 bytes, 8-row groups 1024 bytes apart (SBO), LBO unused (1),
+    // descriptor version 1 (sm_100), layout type 2 = SWIZZLE_128B
+    return static_cast<uint64_t>((smem_addr >> 4) & 0x3FFFu) | (1ull << 16) | (static_cast<uint64_t>(1024 >> 4) << 32) |
+           (1ull << 46) | (2ull << 61);
+}
+
+__global__ void __launch_bounds__(MT_THREADS, 1) k_match_tc(const __grid_constant__ CUtensorMap tmap_a,
+                                                            const __grid_constant__ CUtensorMap tmap_b,
+                                                            const __grid_constant__ MatchParams p) {
+    extern __shared__ __align__(1024) unsigned char mt_smem[];
+    __shared__ __align__(8) uint64_t bar_a, bar_full[4], bar_empty[4], bar_tfull[2], bar_tempty[2];
+    __shared__ uint32_t s_tmem;
+    __shared__ MatchRec s_half[MT_BM];                           // the upper column half's result of every row
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int rb = blockIdx.x, sp = blockIdx.y, pr = blockIdx.z;
+    const int na = p.count_a ? min(max(p.count_a[pr], 0), p.Na) : p.Na;
+    const int nb = p.count_b ? min(max(p.count_b[pr], 0), p.Nb) : p.Nb;
+    const int tiles = (nb + MT_BN - 1) / MT_BN;
+    const int t0 = static_cast<int>(static_cast<long long>(tiles) * sp / p.splits);
+    const int t1 = static_cast<int>(static_cast<long long>(tiles) * (sp + 1) / p.splits);
+    const int row0 = rb * MT_BM;
+    const bool active = row0 < na && t1 > t0;                    // (block-uniform)
+
+    const uint32_t a_bytes = static_cast<uint32_t>(p.KB) * MT_BM * 128u;          // A block: KB x 16 KB
+    const uint32_t b_bytes = static_cast<uint32_t>(p.KB) * MT_BN * 128u;          // one B tile
+    unsigned char* smem_a = mt_smem + ((1024u - (m_smem_u32(mt_smem) & 1023u)) & 1023u);   // the swizzle atom is 1024 bytes
+    unsigned char* smem_b = smem_a + a_bytes;
+
+    if (threadIdx.x == 0) {
+        m_mbar_init(&bar_a, 1);
+        for (int s = 0; s < 4; ++s) { m_mbar_init(&bar_full[s], 1); m_mbar_init(&bar_empty[s], 1); }
+        for (int a = 0; a < 2; ++a) { m_mbar_init(&bar_tfull[a], 1); m_mbar_init(&bar_tempty[a], 256); }
+        m_fence_mbar_init();
+    }
+    if (warp == 1) tc_alloc(&s_tmem, MT_TMEM_COLS);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = s_tmem;
+
+    if (active) {
+        if (warp == 0) {
+            if (lane == 0) {                                     // ===== TMA producer =====
+                m_prefetch_tmap(&tmap_a);
+                m_prefetch_tmap(&tmap_b);
+                m_mbar_expect_tx(&bar_a, a_bytes);
+                for (int kb = 0; kb < p.KB; ++kb) m_tma_load_3d(smem_a + kb * (MT_BM * 128), &tmap_a, &bar_a, kb * MT_KBOX, row0, pr);
+                for (int t = t0, it = 0; t < t1; ++t, ++it) {
+                    const int s = it % p.stages;
+                    if (it >= p.stages) m_mbar_wait(&bar_empty[s], ((it / p.stages) - 1) & 1);
+                    m_mbar_expect_tx(&bar_full[s], b_bytes);
+                    for (int kb = 0; kb < p.KB; ++kb)
+                        m_tma_load_3d(smem_b + s * b_bytes + kb * (MT_BN * 128), &tmap_b, &bar_full[s], kb * MT_KBOX, t * MT_BN, pr);
+                }
+            }
+        } else if (warp == 1) {
+            if (lane == 0) {                                     // ===== MMA issuer =====
+                // instruction descriptor: D = F32 (bits 4-5 = 1), A = B = F16 (0), both K-major, N >> 3 at bit 17, M >> 4 at bit 24
+                const uint32_t idesc = (1u << 4) | (static_cast<uint32_t>(MT_BN >> 3) << 17) | (static_cast<uint32_t>(MT_BM >> 4) << 24);
+                m_mbar_wait(&bar_a, 0);
+                for (int t = t0, it = 0; t < t1; ++t, ++it) {
+                    const int s = it % p.stages, acc = it & 1;
+                    if (it >= 2) m_mbar_wait(&bar_tempty[acc], ((it >> 1) - 1) & 1);   // the epilogue has drained this buffer
+                    m_mbar_wait(&bar_full[s], (it / p.stages) & 1);
+                    tc_fence_after();
+                    const uint32_t a0 = m_smem_u32(smem_a), b0 = m_smem_u32(smem_b + s * b_bytes);
+                    for (int kb = 0; kb < p.KB; ++kb) {
+#pragma unroll
+                        for (int k = 0; k < MT_KBOX / 16; ++k) {  // UMMA_K = 16 fp16 = 32 bytes inside the swizzle atom
+                            const uint64_t da = mt_desc(a0 + kb * (MT_BM * 128) + k * 32);
+                            const uint64_t db = mt_desc(b0 + kb * (MT_BN * 128) + k * 32);
+                            tc_mma_f16(tmem + acc * MT_BN, da, db, idesc, (kb | k) != 0);
+                        }
+                    }
+                    tc_commit(&bar_empty[s]);                    // smem stage free once these MMAs have read it
+                    tc_commit(&bar_tfull[acc]);                  // accumulator complete
+                }
+            }
+        } else {                                                 // ===== epilogue: one thread per row and column half =====
+            const int q = warp & 3, h = (warp - 2) >> 2;
+            const int row = row0 + 32 * q + lane;
+            float best = -INFINITY, second = -INFINITY;
+            int arg = -1;
+            for (int t = t0, it = 0; t < t1; ++t, ++it) {
+                const int acc = it & 1;
+                m_mbar_wait(&bar_tfull[acc], (it >> 1) & 1);
+                tc_fence_after();
+#pragma unroll
+                for (int c = 0; c < 64; c += 32) {
+                    uint32_t v[32];
+                    tc_ld_32x32(tmem + (static_cast<uint32_t>(32 * q) << 16) + acc * MT_BN + 64 * h + c, v);
+                    tc_wait_ld();
+                    const int col0 = t * MT_BN + 64 * h + c;
+                    if (col0 + 32 <= nb) {
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) {
+                            const float x = __uint_as_float(v[j]);
+                            const bool gt = x > best;
+                            second = gt ? best : fmaxf(second, x);
+                            arg = gt ? col0 + j : arg;
+                            best = gt ? x : best;
+                        }
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) {
+                            const float x = col0 + j < nb ? __uint_as_float(v[j]) : -INFINITY;
+                            const bool gt = x > best;
+                            second = gt ? best : fmaxf(second, x);
+                            arg = gt ? col0 + j : arg;
+                            best = gt ? x : best;
+                        }
+                    }
+                }
+                tc_fence_before();
+                m_mbar_arrive(&bar_tempty[acc]);
+            }
+            // combine the two column halves of a row (lower columns first: ties keep the smaller column)
+            if (h == 1) {
+                MatchRec r;
+                r.best = best; r.second = second; r.arg = arg; r.pad = 0;
+                s_half[32 * q + lane] = r;
+            }
+            asm volatile("bar.sync 1, 256;" ::: "memory");      // the 8 epilogue warps only
+            if (h == 0 && row < p.Na) {
+                // per tile the halves interleave (cols 0-63 | 64-127 | 128-191 ...): merge by value, ties by column
+                const MatchRec o = s_half[32 * q + lane];
+                MatchRec r;
+                if (o.best > best || (o.best == best && o.arg >= 0 && (arg < 0 || o.arg < arg))) {
+                    r.best = o.best; r.arg = o.arg; r.second = fmaxf(best, o.second);
+                } else {
+                    r.best = best; r.arg = arg; r.second = fmaxf(second, o.best);
+                }
+                r.pad = 0;
+                p.part[(static_cast<size_t>(pr) * p.splits + sp) * p.Na + row] = r;
+            }
+        }
+    } else if (warp >= 2 && (warp - 2) < 4) {                    // no work for this CTA: neutral partials
+        const int row = row0 + 32 * (warp & 3) + lane;
+        if (row < p.Na) {
+            MatchRec r;
+            r.best = -INFINITY; r.second = -INFINITY; r.arg = -1; r.pad = 0;
+            p.part[(static_cast<size_t>(pr) * p.splits + sp) * p.Na + row] = r;
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) {
+        tc_fence_after();
+        tc_dealloc(tmem, MT_TMEM_COLS);
+    }
+}
+
+// merge of the column splits (in column order), ratio test (M3), mutual check (M4)
+struct FinalizeParams {
+    const MatchRec* part;              // [P, splits, Na]
+    const MatchRec* rpart;             // [P, rsplits, Nb]: the reverse direction (mutual check) or NULL
+    const int32_t* count_a;
+    int Na, Nb, splits, rsplits, P;
+    float ratio2;                      // rho^2, or < 0: ratio test disabled
+    int32_t* out_match;                // [P, Na]
+    float* out_sim;                    // [P, Na, 2] or NULL
+};
+__device__ __forceinline__ MatchRec merge_splits(const MatchRec* part, int splits, size_t stride) {
+    MatchRec r = part[0];
+    for (int s = 1; s < splits; ++s) {
+        const MatchRec o = part[s * stride];
+        if (o.best > r.best) { r.second = fmaxf(r.best, o.second); r.best = o.best; r.arg = o.arg; }
+        else r.second = fmaxf(r.second, o.best);
+    }
+    return r;
+}
+__global__ void __launch_bounds__(256) k_match_finalize(const __grid_constant__ FinalizeParams p) {
+    const int i = blockIdx.x * 256 + threadIdx.x, pr = blockIdx.y;
+    if (i >= p.Na) return;
+    const int na = p.count_a ? min(max(p.count_a[pr], 0), p.Na) : p.Na;
+    int m = -1;
+    float s1 = 0.0f, s2 = 0.0f;
+    if (i < na) {
+        const MatchRec r = merge_splits(p.part + static_cast<size_t>(pr) * p.splits * p.Na + i, p.splits, p.Na);
+        if (r.arg >= 0) {
+            s1 = r.best;
+            s2 = r.second == -INFINITY ? -1.0f : r.second;       // a single column: the smallest cosine (M2)
+            bool keep = true;
+            if (p.ratio2 >= 0.0f) {
+                const float d1 = fmaxf(2.0f - 2.0f * s1, 0.0f), d2 = fmaxf(2.0f - 2.0f * s2, 0.0f);
+                keep = d1 < p.ratio2 * d2;
+            }
+            if (keep && p.rpart != nullptr) {
+                const MatchRec rr = merge_splits(p.rpart + static_cast<size_t>(pr) * p.rsplits * p.Nb + r.arg, p.rsplits, p.Nb);
+                keep = rr.arg == i;
+            }
+            if (keep) m = r.arg;
+        }
+    }
+    p.out_match[static_cast<size_t>(pr) * p.Na + i] = m;
+    if (p.out_sim) {
+        p.out_sim[(static_cast<size_t>(pr) * p.Na + i) * 2] = s1;
+        p.out_sim[(static_cast<size_t>(pr) * p.Na + i) * 2 + 1] = s2;
+    }
+}
+
+// ---- k_scan: sim_k = q . db_k over the keyframe database ------------------------------------------------------
+// A 256-thread CTA takes two database rows per step; thread t owns the 16-byte chunks t, t + 256, ... of every row, so
+// its slice of the query stays in registers (fp32) for the whole kernel and every row is read exactly once with
+// 2 x NCH 16-byte streaming loads in flight per thread.  Fixed summation order (per thread, then warp shuffles, then the
+// eight warp sums): the result does not depend on the grid.  Rows that pass the gate (k < n - n_exclude, sim > tau)
+// are appended to the CTA's private key segment in row order (no atomics) for k_select to rank.
+constexpr int SC_THREADS = 256;
+__device__ __forceinline__ uint4 ld_stream16_plain(const void* p) {
+    uint4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+template <int DT> struct ScanChunk;
+template <> struct ScanChunk<DKD_F16> { static constexpr int N = 8; };
+template <> struct ScanChunk<DKD_F32> { static constexpr int N = 4; };
+template <int DT>
+__device__ __forceinline__ void scan_unpack(const uint4& q, float* f) {
+    if constexpr (DT == DKD_F16) {
+        const __half2* h = reinterpret_cast<const __half2*>(&q);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const float2 t = __half22float2(h[i]);
+            f[2 * i] = t.x;
+            f[2 * i + 1] = t.y;
+        }
+    } else {
+        f[0] = __uint_as_float(q.x); f[1] = __uint_as_float(q.y); f[2] = __uint_as_float(q.z); f[3] = __uint_as_float(q.w);
+    }
+}
+__device__ __forceinline__ uint64_t scan_key(float s, int k) {     // same key as the DKD selection: (score desc, index asc)
+    uint32_t b = __float_as_uint(s + 0.0f);
+    b ^= (b & 0x80000000u) ? 0xFFFFFFFFu : 0x80000000u;
+    return (static_cast<uint64_t>(b) << 32) | static_cast<uint32_t>(~static_cast<uint32_t>(k));
+}
+
+struct ScanParams {
+    const unsigned char* db;
+    const unsigned char* q;
+    int n, chunks;                     // rows; 16-byte chunks per row
+    int n_eligible;                    // rows k < n_eligible may be candidates (n - n_exclude)
+    float tau;
+    float* out_sim;                    // [n]
+    uint64_t* seg;                     // [grid, seg_cap] candidate keys
+    int* seg_cnt;                      // [grid]
+    int seg_cap;
+};
+
+template <int DT, int NCH>
+__global__ void __launch_bounds__(SC_THREADS, 2) k_scan(const __grid_constant__ ScanParams p) {
+    constexpr int N = ScanChunk<DT>::N;
+    __shared__ float s_part[2][SC_THREADS / 32];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    float qf[NCH][N];
+#pragma unroll
+    for (int c = 0; c < NCH; ++c) {
+        const int ch = tid + c * SC_THREADS;
+        uint4 raw = make_uint4(0u, 0u, 0u, 0u);
+        if (ch < p.chunks) raw = __ldg(reinterpret_cast<const uint4*>(p.q) + ch);
+        scan_unpack<DT>(raw, qf[c]);
+    }
+    const size_t rowb = static_cast<size_t>(p.chunks) * 16;
+    uint64_t* my_seg = p.seg + static_cast<size_t>(blockIdx.x) * p.seg_cap;
+    int cnt = 0;                                                  // (thread 0 only)
+    for (int k0 = blockIdx.x * 2; k0 < p.n; k0 += gridDim.x * 2) {
+        const bool two = k0 + 1 < p.n;
+        const uint4* r0 = reinterpret_cast<const uint4*>(p.db + static_cast<size_t>(k0) * rowb);
+        const uint4* r1 = reinterpret_cast<const uint4*>(p.db + static_cast<size_t>(two ? k0 + 1 : k0) * rowb);
+        uint4 a[NCH], b[NCH];
+#pragma unroll
+        for (int c = 0; c < NCH; ++c) {
+            const int ch = tid + c * SC_THREADS;
+            a[c] = make_uint4(0u, 0u, 0u, 0u);
+            b[c] = make_uint4(0u, 0u, 0u, 0u);
+            if (ch < p.chunks) {
+                a[c] = ld_stream16_plain(r0 + ch);
+                b[c] = ld_stream16_plain(r1 + ch);
+            }
+        }
+        float sa = 0.0f, sb = 0.0f;
+#pragma unroll
+        for (int c = 0; c < NCH; ++c) {
+            float fa[N], fb[N];
+            scan_unpack<DT>(a[c], fa);
+            scan_unpack<DT>(b[c], fb);
+#pragma unroll
+            for (int e = 0; e < N; ++e) {
+                sa = fmaf(fa[e], qf[c][e], sa);
+                sb = fmaf(fb[e], qf[c][e], sb);
+            }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            sa += __shfl_xor_sync(0xffffffffu, sa, o);
+            sb += __shfl_xor_sync(0xffffffffu, sb, o);
+        }
+        if (lane == 0) { s_part[0][warp] = sa; s_part[1][warp] = sb; }
+        __syncthreads();
+        if (tid == 0) {
+            float s0 = 0.0f, s1 = 0.0f;
+#pragma unroll
+            for (int w = 0; w < SC_THREADS / 32; ++w) { s0 += s_part[0][w]; s1 += s_part[1][w]; }
+            p.out_sim[k0] = s0;
+            if (k0 < p.n_eligible && s0 > p.tau) { DKD_ASSERT(cnt < p.seg_cap); my_seg[cnt++] = scan_key(s0, k0); }
+            if (two) {
+                p.out_sim[k0 + 1] = s1;
+                if (k0 + 1 < p.n_eligible && s1 > p.tau) { DKD_ASSERT(cnt < p.seg_cap); my_seg[cnt++] = scan_key(s1, k0 + 1); }
+            }
+        }
+        __syncthreads();
+    }
+    if (tid == 0) p.seg_cnt[blockIdx.x] = cnt;
+}
+
+__global__ void k_cand_sims(const int32_t* __restrict__ cand, const float* __restrict__ sim, int max_cand, float* __restrict__ out) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < max_cand) out[i] = cand[i] >= 0 ? sim[cand[i]] : 0.0f;
+}
+
+// ---- f4: per-match stereo validation (S1..S4) and covariance-weighted sqrt information (C1..C4) -------------------
+struct StereoKParams {
+    const float* kl; const float* kr; const int32_t* match;
+    int n;
+    float fx, fy, cx, cy, baseline, d_min, z_min, z_max, max_reproj;
+    float* xyz; float* disp; float* err; uint8_t* valid;
+};
+__global__ void __launch_bounds__(256) k_stereo(const __grid_constant__ StereoKParams p) {
+    const int i = blockIdx.x * 256 + threadIdx.x;
+    if (i >= p.n) return;
+    const int j = p.match ? p.match[i] : i;
+    float X = 0.0f, Y = 0.0f, z = 0.0f, d = 0.0f, e = 0.0f;
+    uint8_t ok = 0;
+    if (j >= 0) {
+        const float2 l = reinterpret_cast<const float2*>(p.kl)[i], r = reinterpret_cast<const float2*>(p.kr)[j];
+        d = l.x - r.x;                                               // S1
+        if (d > p.d_min) {
+            z = __fdiv_rn(p.fx * p.baseline, d);                     // S2
+            const float vm = 0.5f * (l.y + r.y);
+            X = __fdiv_rn((l.x - p.cx) * z, p.fx);
+            Y = __fdiv_rn((vm - p.cy) * z, p.fy);
+            // S4: in this rectified model both views are off by |vL - vR| / 2 (the u residual is zero by construction)
+            e = 0.5f * fabsf(l.y - r.y);
+            ok = (z > p.z_min && z < p.z_max && e <= p.max_reproj) ? 1 : 0;
+        }
+    }
+    p.xyz[3 * i] = X; p.xyz[3 * i + 1] = Y; p.xyz[3 * i + 2] = z;
+    if (p.disp) p.disp[i] = d;
+    if (p.err) p.err[i] = e;
+    p.valid[i] = ok;
+}
+
+struct CovKParams {
+    const float* L;
+    int n;
+    float s2, floor_px, inv_fx2, inv_fy2, inv_fxfy, lam, inv_sigma0;
+    float* omega; uint8_t* ok;
+};
+__global__ void __launch_bounds__(256) k_cov(const __grid_constant__ CovKParams p) {
+    const int i = blockIdx.x * 256 + threadIdx.x;
+    if (i >= p.n) return;
+    const float l11 = p.L[3 * i], l21 = p.L[3 * i + 1], l22 = p.L[3 * i + 2];
+    const float a = p.s2 * (l11 * l11) + p.floor_px, b = p.s2 * (l11 * l21), c = p.s2 * (l21 * l21 + l22 * l22) + p.floor_px;
+    const float na = a * p.inv_fx2, nb = b * p.inv_fxfy, nc = c * p.inv_fy2;              // Eq. 9
+    // det(Sigma_px) as a sum of non-negative terms (C4): its sign cannot be flipped by rounding
+    const float det_px = p.s2 * p.s2 * (l11 * l11) * (l22 * l22) + p.floor_px * p.s2 * (l11 * l11 + l21 * l21 + l22 * l22) +
+                         p.floor_px * p.floor_px;
+    const float det = det_px * p.inv_fx2 * p.inv_fy2;
+    bool ok = isfinite(na) && isfinite(nb) && isfinite(nc) && na > 0.0f && det > 0.0f && isfinite(det);
+    float o00 = p.inv_sigma0, o01 = 0.0f, o11 = p.inv_sigma0;
+    if (ok) {
+        // Omega^T Omega = lam Sigma_n^-1 = (lam / det) [[nc, -nb], [-nb, na]]; its Cholesky factor in closed form:
+        // c11 = sqrt(lam nc / det), c21 = -lam nb / (det c11), c22^2 = lam na / det - c21^2 = lam / nc  (no cancellation)
+        const float ia = p.lam * nc / det;
+        const float c11 = sqrtf(ia);
+        const float c21 = -p.lam * nb / (det * c11);
+        const float c22 = sqrtf(p.lam / nc);
+        if (ia > 0.0f && nc > 0.0f && isfinite(c11) && isfinite(c21) && isfinite(c22) && c22 > 0.0f) { o00 = c11; o01 = c21; o11 = c22; }
+        else ok = false;
+    }
+    p.omega[4 * i] = o00; p.omega[4 * i + 1] = o01; p.omega[4 * i + 2] = 0.0f; p.omega[4 * i + 3] = o11;
+    if (p.ok) p.ok[i] = ok ? 1 : 0;
+}
+
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                    const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                    CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+PFN_encodeTiled get_encode() {
+    static PFN_encodeTiled fn = nullptr;
+    if (!fn) {
+        void* f = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<PFN_encodeTiled>(f);
+        (void)cudaGetLastError();
+    }
+    return fn;
+}
+// [P, N, D] fp16 row-major -> 3-D map (k, row, pair), box (64, 128, 1), 128-byte swizzle, zero fill past the end
+bool encode_desc_map(CUtensorMap* m, const void* base, int N, int D, int P) {
+    PFN_encodeTiled enc = get_encode();
+    if (!enc) return false;
+    const cuuint64_t dims[3] = {(cuuint64_t)D, (cuuint64_t)N, (cuuint64_t)P};
+    const cuuint64_t strides[2] = {(cuuint64_t)D * 2, (cuuint64_t)D * 2 * N};
+    const cuuint32_t box[3] = {(cuuint32_t)MT_KBOX, (cuuint32_t)MT_BN, 1};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+int match_splits(int num_sms, int Na, int Nb, int P) {
+    const int rbs = (Na + MT_BM - 1) / MT_BM, tiles = (Nb + MT_BN - 1) / MT_BN;
+    int s = num_sms / (rbs * P > 0 ? rbs * P : 1);               // fill the machine once
+    if (s < 1) s = 1;
+    if (s > tiles) s = tiles;
+    if (s > 16) s = 16;
+    return s;
+}
+
+cudaError_t launch_match_dir(dkd_ctx* ctx, const void* A, const int32_t* ca, int Na, const void* B, const int32_t* cb, int Nb, int D,
+                             int P, int splits, MatchRec* part, cudaStream_t st) {
+    CUtensorMap ta, tb;
+    if (!encode_desc_map(&ta, A, Na, D, P) || !encode_desc_map(&tb, B, Nb, D, P)) return cudaErrorInvalidValue;
+    MatchParams mp;
+    memset(&mp, 0, sizeof(mp));
+    mp.count_a = ca; mp.count_b = cb; mp.Na = Na; mp.Nb = Nb; mp.KB = D / MT_KBOX; mp.splits = splits; mp.part = part;
+    const size_t a_bytes = static_cast<size_t>(mp.KB) * MT_BM * 128, b_bytes = static_cast<size_t>(mp.KB) * MT_BN * 128;
+    int stages = static_cast<int>((200 * 1024 - a_bytes) / b_bytes);
+    if (stages > 4) stages = 4;
+    mp.stages = stages;
+    const size_t smem = a_bytes + stages * b_bytes + 1024;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(k_match_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, 204 * 1024);   // (static smem takes ~3 KB of the 227)
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    (void)ctx;
+    const dim3 grid((Na + MT_BM - 1) / MT_BM, splits, P);
+    k_match_tc<<<grid, MT_THREADS, smem, st>>>(ta, tb, mp);
+    return cudaGetLastError();
+}
+
+}  // namespace dkd
+
+using namespace dkd;
+
+extern "C" {
+
+int dkd_match(dkd_ctx* ctx, const void* desc_a, const int32_t* count_a, int Na, const void* desc_b, const int32_t* count_b,
+              int Nb, int D, int dtype, int P, float ratio, int mutual, int32_t* out_match, float* out_sim, void* stream) {
+    if (!ctx) return DKD_ERR_INVALID_ARG;
+    if (!desc_a || !desc_b || !out_match || Na < 1 || Nb < 1 || D < 1 || P < 1 || !(ratio > 0.0f))
+        return dkd_ctx_fail(ctx, DKD_ERR_INVALID_ARG, "dkd_match: NULL pointer, size < 1 or ratio <= 0", nullptr);
+    if (dtype != DKD_F16) return dkd_ctx_fail(ctx, DKD_ERR_UNSUPPORTED, "dkd_match: descriptors must be DKD_F16 (tcgen05 kind::f16)", nullptr);
+    if (D % MT_KBOX != 0 || D > MT_KBOX * MT_MAX_KB)
+        return dkd_ctx_fail(ctx, DKD_ERR_UNSUPPORTED, "dkd_match: D must be 64, 128, 192 or 256", nullptr);
+    if (P > 65535) return dkd_ctx_fail(ctx, DKD_ERR_UNSUPPORTED, "dkd_match: P > 65535", nullptr);
+    if ((reinterpret_cast<uintptr_t>(desc_a) & 15) || (reinterpret_cast<uintptr_t>(desc_b) & 15))
+        return dkd_ctx_fail(ctx, DKD_ERR_UNSUPPORTED, "dkd_match: descriptor sets not 16-byte aligned", nullptr);
+    DeviceGuard dg(dkd_ctx_device(ctx));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int sms = dkd_ctx_num_sms(ctx);
+    const int s_ab = match_splits(sms, Na, Nb, P), s_ba = mutual ? match_splits(sms, Nb, Na, P) : 0;
+    const size_t n_ab = static_cast<size_t>(P) * s_ab * Na, n_ba = static_cast<size_t>(P) * s_ba * Nb;
+    MatchRec* part = static_cast<MatchRec*>(dkd_ctx_scratch(ctx, 0, (n_ab + n_ba) * sizeof(MatchRec)));
+    if (!part) return DKD_ERR_CUDA;
+    cudaError_t e = launch_match_dir(ctx, desc_a, count_a, Na, desc_b, count_b, Nb, D, P, s_ab, part, st);
+    if (e == cudaSuccess && mutual) e = launch_match_dir(ctx, desc_b, count_b, Nb, desc_a, count_a, Na, D, P, s_ba, part + n_ab, st);
+    if (e != cudaSuccess) return dkd_ctx_fail(ctx, DKD_ERR_CUDA, "dkd_match launch: ", cudaGetErrorString(e));
+    FinalizeParams fp;
+    memset(&fp, 0, sizeof(fp));
+    fp.part = part; fp.rpart = mutual ? part + n_ab : nullptr; fp.count_a = count_a; fp.Na = Na; fp.Nb = Nb; fp.splits = s_ab;
+    fp.rsplits = s_ba; fp.P = P; fp.ratio2 = ratio >= 1e9f ? -1.0f : ratio * ratio; fp.out_match = out_match; fp.out_sim = out_sim;
+    k_match_finalize<<<dim3((Na + 255) / 256, P), 256, 0, st>>>(fp);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return dkd_ctx_fail(ctx, DKD_ERR_CUDA, "k_match_finalize launch: ", cudaGetErrorString(e));
+    return DKD_OK;
+}
+
+int dkd_retrieval_scan(dkd_ctx* ctx, const void* db, int dtype, int n, int D, const void* query, int n_exclude, float tau,
+                       int max_cand, float* out_sim, int32_t* out_cand, float* out_cand_sim, int32_t* out_count, void* stream) {
+    if (!ctx) return DKD_ERR_INVALID_ARG;
+    if (!query || !out_cand || !out_count || n < 0 || (n > 0 && !db) || D < 1 || n_exclude < 0 || max_cand < 1 || isnan(tau))
+        return dkd_ctx_fail(ctx, DKD_ERR_INVALID_ARG, "dkd_retrieval_scan: NULL pointer or bad size", nullptr);
+    if (dtype != DKD_F16 && dtype != DKD_F32) return dkd_ctx_fail(ctx, DKD_ERR_UNSUPPORTED, "dkd_retrieval_scan: dtype must be DKD_F16 or DKD_F32", nullptr);
+    const size_t rowb = static_cast<size_t>(D) * (dtype == DKD_F16 ? 2 : 4);
+    if (rowb % 16 != 0 || rowb > 16 * 8 * SC_THREADS)
+        return dkd_ctx_fail(ctx, DKD_ERR_UNSUPPORTED, "dkd_retrieval_scan: D * elemsize must be a multiple of 16 and <= 32768", nullptr);
+    if ((reinterpret_cast<uintptr_t>(db) & 15) || (reinterpret_cast<uintptr_t>(query) & 15))
+        return dkd_ctx_fail(ctx, DKD_ERR_UNSUPPORTED, "dkd_retrieval_scan: db / query not 16-byte aligned", nullptr);
+    if (max_cand > DKD_MAX_TOP_K) return dkd_ctx_fail(ctx, DKD_ERR_UNSUPPORTED, "dkd_retrieval_scan: max_cand > DKD_MAX_TOP_K", nullptr);
+    DeviceGuard dg(dkd_ctx_device(ctx));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    int grid = 2 * dkd_ctx_num_sms(ctx);
+    if (grid > (n + 1) / 2) grid = (n + 1) / 2;
+    if (grid < 1) grid = 1;
+    const int seg_cap = 2 * ((n + 2 * grid - 1) / (2 * grid)) + 2;        // rows one CTA can see
+    const size_t b_seg = (static_cast<size_t>(grid) * seg_cap * 8 + 255) & ~static_cast<size_t>(255);
+    const size_t b_cnt = (static_cast<size_t>(grid) * 4 + 255) & ~static_cast<size_t>(255);
+    const size_t b_sim = out_sim ? 0 : ((static_cast<size_t>(n > 0 ? n : 1) * 4 + 255) & ~static_cast<size_t>(255));
+    unsigned char* ws = static_cast<unsigned char*>(dkd_ctx_scratch(ctx, 1, b_seg + b_cnt + b_sim));
+    if (!ws) return DKD_ERR_CUDA;
+    ScanParams sp;
+    memset(&sp, 0, sizeof(sp));
+    sp.db = static_cast<const unsigned char*>(db); sp.q = static_cast<const unsigned char*>(query);
+    sp.n = n; sp.chunks = static_cast<int>(rowb / 16); sp.n_eligible = n - n_exclude; sp.tau = tau;
+    sp.out_sim = out_sim ? out_sim : reinterpret_cast<float*>(ws + b_seg + b_cnt);
+    sp.seg = reinterpret_cast<uint64_t*>(ws); sp.seg_cnt = reinterpret_cast<int*>(ws + b_seg); sp.seg_cap = seg_cap;
+    const int nch = (sp.chunks + SC_THREADS - 1) / SC_THREADS;
+#define DKD_SCAN(DT, NCH) k_scan<DT, NCH><<<grid, SC_THREADS, 0, st>>>(sp)
+#define DKD_SCAN_DT(DT)                                                                             \
+    switch (nch) {                                                                                  \
+        case 1: DKD_SCAN(DT, 1); break; case 2: DKD_SCAN(DT, 2); break; case 3: DKD_SCAN(DT, 3); break; \
+        case 4: DKD_SCAN(DT, 4); break; case 5: DKD_SCAN(DT, 5); break; case 6: DKD_SCAN(DT, 6); break; \
+        case 7: DKD_SCAN(DT, 7); break; default: DKD_SCAN(DT, 8); break;                              \
+    }
+    if (dtype == DKD_F16) { DKD_SCAN_DT(DKD_F16) } else { DKD_SCAN_DT(DKD_F32) }
+#undef DKD_SCAN_DT
+#undef DKD_SCAN
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return dkd_ctx_fail(ctx, DKD_ERR_CUDA, "k_scan launch: ", cudaGetErrorString(e));
+    const int rc = dkd_internal_select(ctx, sp.seg, sp.seg_cnt, grid, seg_cap, max_cand, n > 0 ? n : 1, out_cand, out_count, st);
+    if (rc != DKD_OK) return rc;
+    if (out_cand_sim) {
+        k_cand_sims<<<(max_cand + 255) / 256, 256, 0, st>>>(out_cand, sp.out_sim, max_cand, out_cand_sim);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return dkd_ctx_fail(ctx, DKD_ERR_CUDA, "k_cand_sims launch: ", cudaGetErrorString(e));
+    }
+    return DKD_OK;
+}
+
+int dkd_stereo_validate(dkd_ctx* ctx, const float* kpts_l, const float* kpts_r, const int32_t* match, int n,
+                        const dkd_stereo_params* sp, float* out_xyz, float* out_disp, float* out_err, uint8_t* out_valid,
+                        void* stream) {
+    if (!ctx) return DKD_ERR_INVALID_ARG;
+    if (!kpts_l || !kpts_r || !sp || !out_xyz || !out_valid || n < 0)
+        return dkd_ctx_fail(ctx, DKD_ERR_INVALID_ARG, "dkd_stereo_validate: NULL pointer or n < 0", nullptr);
+    if (!(sp->fx > 0.0f) || !(sp->fy > 0.0f) || !(sp->baseline > 0.0f))
+        return dkd_ctx_fail(ctx, DKD_ERR_INVALID_ARG, "dkd_stereo_validate: fx, fy, baseline must be > 0", nullptr);
+    if ((reinterpret_cast<uintptr_t>(kpts_l) & 7) || (reinterpret_cast<uintptr_t>(kpts_r) & 7))
+        return dkd_ctx_fail(ctx, DKD_ERR_UNSUPPORTED, "dkd_stereo_validate: keypoints not 8-byte aligned", nullptr);
+    if (n == 0) return DKD_OK;
+    DeviceGuard dg(dkd_ctx_device(ctx));
+    StereoKParams k;
+    memset(&k, 0, sizeof(k));
+    k.kl = kpts_l; k.kr = kpts_r; k.match = match; k.n = n;
+    k.fx = sp->fx; k.fy = sp->fy; k.cx = sp->cx; k.cy = sp->cy; k.baseline = sp->baseline; k.d_min = sp->d_min;
+    k.z_min = sp->z_min; k.z_max = sp->z_max; k.max_reproj = sp->max_reproj;
+    k.xyz = out_xyz; k.disp = out_disp; k.err = out_err; k.valid = out_valid;
+    k_stereo<<<(n + 255) / 256, 256, 0, static_cast<cudaStream_t>(stream)>>>(k);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return dkd_ctx_fail(ctx, DKD_ERR_CUDA, "k_stereo launch: ", cudaGetErrorString(e));
+    return DKD_OK;
+}
+
+int dkd_cov_sqrt_info(dkd_ctx* ctx, const float* L, int n, const dkd_cov_params* cp, float* out_omega, uint8_t* out_ok,
+                      void* stream) {
+    if (!ctx) return DKD_ERR_INVALID_ARG;
+    if (!L || !cp || !out_omega || n < 0) return dkd_ctx_fail(ctx, DKD_ERR_INVALID_ARG, "dkd_cov_sqrt_info: NULL pointer or n < 0", nullptr);
+    if (!(cp->fx > 0.0f) || !(cp->fy > 0.0f) || !(cp->sigma0 > 0.0f) || !(cp->floor_px >= 0.0f) || !(cp->lambda_min >= 0.0f) ||
+        !(fmaxf(cp->lambda, cp->lambda_min) > 0.0f))
+        return dkd_ctx_fail(ctx, DKD_ERR_INVALID_ARG, "dkd_cov_sqrt_info: fx, fy, sigma0, max(lambda, lambda_min) must be > 0; floor >= 0", nullptr);
+    if (n == 0) return DKD_OK;
+    DeviceGuard dg(dkd_ctx_device(ctx));
+    CovKParams k;
+    memset(&k, 0, sizeof(k));
+    k.L = L; k.n = n;
+    k.s2 = cp->scale * cp->scale; k.floor_px = cp->floor_px;
+    k.inv_fx2 = static_cast<float>(1.0 / (static_cast<double>(cp->fx) * cp->fx));
+    k.inv_fy2 = static_cast<float>(1.0 / (static_cast<double>(cp->fy) * cp->fy));
+    k.inv_fxfy = static_cast<float>(1.0 / (static_cast<double>(cp->fx) * cp->fy));
+    k.lam = fmaxf(cp->lambda, cp->lambda_min);
+    k.inv_sigma0 = 1.0f / cp->sigma0;
+    k.omega = out_omega; k.ok = out_ok;
+    k_cov<<<(n + 255) / 256, 256, 0, static_cast<cudaStream_t>(stream)>>>(k);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return dkd_ctx_fail(ctx, DKD_ERR_CUDA, "k_cov launch: ", cudaGetErrorString(e));
+    return DKD_OK;
+}
+
+}  // extern "C"

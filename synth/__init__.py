@@ -158,3 +158,55 @@ def make_inputs(cfg: Config, device="cpu", with_desc=True, pin_memory=False):
     if with_desc:
         desc = desc_maps(cfg.B, cfg.Hd, cfg.Wd, cfg.D, cfg.seed, torch_dtype(cfg.desc_dtype), device)
     return score, desc
+
+
+# ---- inputs for the consumers of the descriptor output ---------------------------------
+def _unit_rows(g: torch.Generator, n: int, D: int) -> torch.Tensor:
+    x = torch.randn((n, D), generator=g, dtype=torch.float64)
+    return x / x.norm(dim=1, keepdim=True)
+
+
+def match_sets(P, Na, Nb, D, seed, overlap=0.7, noise=0.35, count_a=None, count_b=None):
+    """Two zero-padded, l2-normalised fp16 descriptor sets per pair, like two views of one scene: a fraction
+    `overlap` of A's rows reappears in B at a random position with additive noise (true matches, cosine about
+    1 / sqrt(1 + noise^2)), the rest of B are unrelated descriptors.  Returns (A [P,Na,D] f16, B [P,Nb,D] f16,
+    count_a [P] i32, count_b [P] i32); rows past the counts are zero.  Stands in for the
+    ALIKED / SuperPoint / XFeat descriptors of two frames, which are not available."""
+    g = torch.Generator().manual_seed(int(seed))
+    A = torch.zeros((P, Na, D), dtype=torch.float16)
+    B = torch.zeros((P, Nb, D), dtype=torch.float16)
+    ca = torch.empty(P, dtype=torch.int32)
+    cb = torch.empty(P, dtype=torch.int32)
+    for p in range(P):
+        na = Na if count_a is None else int(count_a[p])
+        nb = Nb if count_b is None else int(count_b[p])
+        a = _unit_rows(g, na, D)
+        b = _unit_rows(g, nb, D)
+        m = min(int(overlap * na), nb)
+        src = torch.randperm(na, generator=g)[:m]
+        dst = torch.randperm(nb, generator=g)[:m]
+        nz = a[src] + noise * _unit_rows(g, m, D)
+        b[dst] = nz / nz.norm(dim=1, keepdim=True)
+        A[p, :na] = a.to(torch.float16)
+        B[p, :nb] = b.to(torch.float16)
+        ca[p], cb[p] = na, nb
+    return A, B, ca, cb
+
+
+def keyframe_db(n, D, seed, revisits=(), revisit_sim=0.8, dtype=torch.float16):
+    """A keyframe database of n l2-normalised global descriptors (rows in insertion order) and a query: unrelated
+    unit vectors, except that the rows listed in `revisits` are earlier views of the query's place (cosine about
+    `revisit_sim`, each a little lower than the one before so that the ranking is unambiguous).  Stands in for the
+    AnyLoc DINOv2-VLAD descriptors, g in R^{32*384}, which need trained weights."""
+    g = torch.Generator().manual_seed(int(seed))
+    q = _unit_rows(g, 1, D)[0]
+    db = torch.empty((n, D), dtype=dtype)
+    for s in range(0, n, 4096):
+        db[s:s + 4096] = _unit_rows(g, min(4096, n - s), D).to(dtype)
+    for i, k in enumerate(revisits):
+        s = revisit_sim - 0.004 * i
+        o = _unit_rows(g, 1, D)[0]
+        o = o - (o @ q) * q
+        o = o / o.norm()
+        db[k] = (s * q + (1 - s * s) ** 0.5 * o).to(dtype)
+    return db, q.to(dtype)
