@@ -278,7 +278,7 @@ int dkd_match(dkd_ctx* ctx, const void* desc_a, const int32_t* count_a, int Na,
  * "Candidates with sim > tau_sim are ranked by similarity"; "brute-force scan over the keyframe database, O(n)";
  * 50 most recent excluded, tau_sim = 0.60; g in R^{32*384}).
  *   db       device [n,D] f16|f32, rows in insertion order (row n-1 is the newest keyframe), 16-byte aligned
- *   query    device [D] same dtype, 16-byte aligned;  D * elemsize a multiple of 16 and <= 32768
+ *   query    device [D] same dtype, 16-byte aligned;  D * elemsize a multiple of 16, D <= 16384
  *   out_sim  device [n] f32: q . db_k for EVERY row (fp32 accumulation), or NULL
  *   out_cand device [max_cand] i32: rows k < n - n_exclude with sim > tau (strict), ranked by (sim desc, k asc),
  *            -1 padded; out_cand_sim device [max_cand] f32 or NULL; out_count device [1] i32

@@ -26,18 +26,27 @@ def nvcc() -> str:
     return "nvcc"
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    stale = force or not os.path.exists(LIB) or any(os.path.getmtime(d) > os.path.getmtime(LIB) for d in DEPS)
+LIB_DEBUG = os.path.join(_HERE, "libdkd_debug.so")
+
+
+def build(force: bool = False, verbose: bool = False, debug: bool = False) -> str:
+    """Builds libdkd.so, or with debug=True libdkd_debug.so: the same sources with -DDKD_DEBUG, i.e. device-side
+    bounds checks (assert) on every workspace / shared-memory index and on the mbarrier ring arithmetic.  The GPU
+    tests run their random sweep and worst-case inputs under it (DKD_LIBRARY=libdkd_debug.so)."""
+    lib = LIB_DEBUG if debug else LIB
+    stale = force or not os.path.exists(lib) or any(os.path.getmtime(d) > os.path.getmtime(lib) for d in DEPS)
     if stale:
-        tmp = LIB + f".tmp{os.getpid()}"
+        tmp = lib + f".tmp{os.getpid()}"
         cmd = [nvcc(), *NVCC_FLAGS, "-I", os.path.join(ROOT, "include"), "-I", CSRC]
+        if debug:
+            cmd += ["-DDKD_DEBUG"]
         if verbose:
             cmd += ["-Xptxas", "-v"]
         cmd += [*SOURCES, "-o", tmp]
         subprocess.check_call(cmd)
-        os.replace(tmp, LIB)
-    return LIB
+        os.replace(tmp, lib)
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, debug="--debug" in sys.argv))

@@ -618,7 +618,7 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
                     const int e = e0 + 32 * u + lane;
                     uint64_t k = kk[u];
                     if (lo == 0) {
-                        if (e < total) keys[gbase + e] = k;
+                        if (e < total) { DKD_ASSERT(gbase + e >= 0 && gbase + e < SORT_CAP); keys[gbase + e] = k; }
                     } else {
                         const bool take = (e < total) && (k >= lo);
                         const unsigned bal = __ballot_sync(FULL, take);
@@ -626,7 +626,7 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
                             int pb = 0;
                             if (lane == 0) pb = atomicAdd(&s_n, __popc(bal));
                             pb = __shfl_sync(FULL, pb, 0);
-                            if (take) keys[pb + __popc(bal & ((1u << lane) - 1u))] = k;
+                            if (take) { DKD_ASSERT(pb + __popc(bal & ((1u << lane) - 1u)) < SORT_CAP); keys[pb + __popc(bal & ((1u << lane) - 1u))] = k; }
                         }
                         if (!take) k = 0ull;
                     }
@@ -723,7 +723,10 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
         const unsigned kb = static_cast<unsigned>(k >> 32);
         return kb == hi ? key_index(k) >> idx_shift : NBT + static_cast<int>((hi - kb) >> shift);
     };
-    for (int i = tid; i < m; i += SEL_THREADS) atomicAdd(&cur[bucket_of(keys[i])], 1);
+    for (int i = tid; i < m; i += SEL_THREADS) {
+        DKD_ASSERT(bucket_of(keys[i]) >= 0 && bucket_of(keys[i]) < NBK);
+        atomicAdd(&cur[bucket_of(keys[i])], 1);
+    }
     __syncthreads();
     {   // exclusive scan of the NBK bucket counts (5 consecutive buckets per thread), largest bucket
         int c4[NBK / SEL_THREADS];
@@ -765,7 +768,10 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
         for (int i = tid; i < m; i += SEL_THREADS) {        // scatter into bucket order
             const uint64_t k = keys[i];
             const int d = bucket_of(k);
-            sorted[base[d] + atomicAdd(&cur[d], 1)] = k;
+            DKD_ASSERT(d >= 0 && d < NBK);
+            const int pos = base[d] + atomicAdd(&cur[d], 1);
+            DKD_ASSERT(pos >= 0 && pos < m && pos < SORT_CAP);
+            sorted[pos] = k;
         }
         __syncthreads();
         for (int i = tid; i < m; i += SEL_THREADS) {        // exact rank inside the own bucket
@@ -781,6 +787,7 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
                 rank += r8;
             }
             for (; j < s1; ++j) rank += sorted[j] > k ? 1 : 0;
+            DKD_ASSERT(rank >= 0 && rank < m);
             if (rank < K) {
                 out[rank] = key_index(k);
                 prefetch_window(pf, b, key_index(k));

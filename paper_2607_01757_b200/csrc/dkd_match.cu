@@ -337,12 +337,15 @@ __global__ void __launch_bounds__(256) k_match_finalize(const __grid_constant__ 
 }
 
 // ---- k_scan: sim_k = q . db_k over the keyframe database ------------------------------------------------------
-// A 256-thread CTA takes two database rows per step; thread t owns the 16-byte chunks t, t + 256, ... of every row, so
-// its slice of the query stays in registers (fp32) for the whole kernel and every row is read exactly once with
-// 2 x NCH 16-byte streaming loads in flight per thread.  Fixed summation order (per thread, then warp shuffles, then the
-// eight warp sums): the result does not depend on the grid.  Rows that pass the gate (k < n - n_exclude, sim > tau)
-// are appended to the CTA's private key segment in row order (no atomics) for k_select to rank.
+// One WARP per database row, SC_R rows at a time: lane l owns the 16-byte chunks l, l + 32, ... of a row, SC_R x SC_U of
+// them in flight per lane (streaming loads, no L1 allocation), multiplied with the query held in shared memory as
+// fp32.  No block-wide barrier after the query is staged, no cross-warp reduction: a row's sum is its lanes' sequential
+// partial sums combined by a shuffle tree — a fixed order that does not depend on the grid.  Rows that pass the gate
+// (k < n - n_exclude, sim > tau) are appended by lane 0 to the warp's private key segment in row order (no atomics) for
+// k_select to rank.  Every row is read exactly once: HBM-bound.
 constexpr int SC_THREADS = 256;
+constexpr int SC_U = 4;                                            // chunks per lane and row in flight
+constexpr int SC_R = 4;                                            // rows per warp step (the query chunk is unpacked once for all of them)
 __device__ __forceinline__ uint4 ld_stream16_plain(const void* p) {
     uint4 r;
     asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
@@ -378,75 +381,84 @@ struct ScanParams {
     int n_eligible;                    // rows k < n_eligible may be candidates (n - n_exclude)
     float tau;
     float* out_sim;                    // [n]
-    uint64_t* seg;                     // [grid, seg_cap] candidate keys
-    int* seg_cnt;                      // [grid]
+    uint64_t* seg;                     // [warps of the grid, seg_cap] candidate keys
+    int* seg_cnt;                      // [warps of the grid]
     int seg_cap;
 };
 
-template <int DT, int NCH>
+template <int DT>
 __global__ void __launch_bounds__(SC_THREADS, 2) k_scan(const __grid_constant__ ScanParams p) {
     constexpr int N = ScanChunk<DT>::N;
-    __shared__ float s_part[2][SC_THREADS / 32];
+    extern __shared__ __align__(16) float s_q[];                  // the query as fp32: chunks * N floats
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    float qf[NCH][N];
+    for (int ch = tid; ch < p.chunks; ch += SC_THREADS) {
+        float f[N];
+        scan_unpack<DT>(__ldg(reinterpret_cast<const uint4*>(p.q) + ch), f);
 #pragma unroll
-    for (int c = 0; c < NCH; ++c) {
-        const int ch = tid + c * SC_THREADS;
-        uint4 raw = make_uint4(0u, 0u, 0u, 0u);
-        if (ch < p.chunks) raw = __ldg(reinterpret_cast<const uint4*>(p.q) + ch);
-        scan_unpack<DT>(raw, qf[c]);
+        for (int e = 0; e < N; ++e) s_q[ch * N + e] = f[e];
     }
+    __syncthreads();
+    const int gw = blockIdx.x * (SC_THREADS / 32) + warp, nw = gridDim.x * (SC_THREADS / 32);
     const size_t rowb = static_cast<size_t>(p.chunks) * 16;
-    uint64_t* my_seg = p.seg + static_cast<size_t>(blockIdx.x) * p.seg_cap;
-    int cnt = 0;                                                  // (thread 0 only)
-    for (int k0 = blockIdx.x * 2; k0 < p.n; k0 += gridDim.x * 2) {
-        const bool two = k0 + 1 < p.n;
-        const uint4* r0 = reinterpret_cast<const uint4*>(p.db + static_cast<size_t>(k0) * rowb);
-        const uint4* r1 = reinterpret_cast<const uint4*>(p.db + static_cast<size_t>(two ? k0 + 1 : k0) * rowb);
-        uint4 a[NCH], b[NCH];
+    uint64_t* my_seg = p.seg + static_cast<size_t>(gw) * p.seg_cap;
+    int cnt = 0;
+    for (int k0 = SC_R * gw; k0 < p.n; k0 += SC_R * nw) {
+        const uint4* rp[SC_R];
 #pragma unroll
-        for (int c = 0; c < NCH; ++c) {
-            const int ch = tid + c * SC_THREADS;
-            a[c] = make_uint4(0u, 0u, 0u, 0u);
-            b[c] = make_uint4(0u, 0u, 0u, 0u);
-            if (ch < p.chunks) {
-                a[c] = ld_stream16_plain(r0 + ch);
-                b[c] = ld_stream16_plain(r1 + ch);
+        for (int r = 0; r < SC_R; ++r)                            // rows past the end alias the last row (discarded below)
+            rp[r] = reinterpret_cast<const uint4*>(p.db + static_cast<size_t>(k0 + r < p.n ? k0 + r : p.n - 1) * rowb);
+        float acc[SC_R];
+#pragma unroll
+        for (int r = 0; r < SC_R; ++r) acc[r] = 0.0f;
+        for (int c0 = lane; c0 < p.chunks; c0 += 32 * SC_U) {
+            uint4 raw[SC_U][SC_R];
+#pragma unroll
+            for (int u = 0; u < SC_U; ++u) {
+                const int ch = c0 + 32 * u;
+#pragma unroll
+                for (int r = 0; r < SC_R; ++r) {
+                    raw[u][r] = make_uint4(0u, 0u, 0u, 0u);
+                    if (ch < p.chunks) raw[u][r] = ld_stream16_plain(rp[r] + ch);
+                }
             }
-        }
-        float sa = 0.0f, sb = 0.0f;
 #pragma unroll
-        for (int c = 0; c < NCH; ++c) {
-            float fa[N], fb[N];
-            scan_unpack<DT>(a[c], fa);
-            scan_unpack<DT>(b[c], fb);
+            for (int u = 0; u < SC_U; ++u) {
+                const int ch = c0 + 32 * u;
+                if (ch < p.chunks) {
+                    float fq[N];
+                    const float4* qp = reinterpret_cast<const float4*>(s_q + ch * N);
 #pragma unroll
-            for (int e = 0; e < N; ++e) {
-                sa = fmaf(fa[e], qf[c][e], sa);
-                sb = fmaf(fb[e], qf[c][e], sb);
+                    for (int v = 0; v < N / 4; ++v) {
+                        const float4 t = qp[v];
+                        fq[4 * v] = t.x; fq[4 * v + 1] = t.y; fq[4 * v + 2] = t.z; fq[4 * v + 3] = t.w;
+                    }
+#pragma unroll
+                    for (int r = 0; r < SC_R; ++r) {
+                        float f[N];
+                        scan_unpack<DT>(raw[u][r], f);
+#pragma unroll
+                        for (int e = 0; e < N; ++e) acc[r] = fmaf(f[e], fq[e], acc[r]);
+                    }
+                }
             }
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
-            sa += __shfl_xor_sync(0xffffffffu, sa, o);
-            sb += __shfl_xor_sync(0xffffffffu, sb, o);
-        }
-        if (lane == 0) { s_part[0][warp] = sa; s_part[1][warp] = sb; }
-        __syncthreads();
-        if (tid == 0) {
-            float s0 = 0.0f, s1 = 0.0f;
 #pragma unroll
-            for (int w = 0; w < SC_THREADS / 32; ++w) { s0 += s_part[0][w]; s1 += s_part[1][w]; }
-            p.out_sim[k0] = s0;
-            if (k0 < p.n_eligible && s0 > p.tau) { DKD_ASSERT(cnt < p.seg_cap); my_seg[cnt++] = scan_key(s0, k0); }
-            if (two) {
-                p.out_sim[k0 + 1] = s1;
-                if (k0 + 1 < p.n_eligible && s1 > p.tau) { DKD_ASSERT(cnt < p.seg_cap); my_seg[cnt++] = scan_key(s1, k0 + 1); }
+            for (int r = 0; r < SC_R; ++r) acc[r] += __shfl_xor_sync(0xffffffffu, acc[r], o);
+        }
+        if (lane == 0) {
+#pragma unroll
+            for (int r = 0; r < SC_R; ++r) {
+                const int k = k0 + r;
+                if (k < p.n) {
+                    p.out_sim[k] = acc[r];
+                    if (k < p.n_eligible && acc[r] > p.tau) { DKD_ASSERT(cnt < p.seg_cap); my_seg[cnt++] = scan_key(acc[r], k); }
+                }
             }
         }
-        __syncthreads();
     }
-    if (tid == 0) p.seg_cnt[blockIdx.x] = cnt;
+    if (lane == 0) p.seg_cnt[gw] = cnt;
 }
 
 __global__ void k_cand_sims(const int32_t* __restrict__ cand, const float* __restrict__ sim, int max_cand, float* __restrict__ out) {
@@ -621,19 +633,21 @@ int dkd_retrieval_scan(dkd_ctx* ctx, const void* db, int dtype, int n, int D, co
         return dkd_ctx_fail(ctx, DKD_ERR_INVALID_ARG, "dkd_retrieval_scan: NULL pointer or bad size", nullptr);
     if (dtype != DKD_F16 && dtype != DKD_F32) return dkd_ctx_fail(ctx, DKD_ERR_UNSUPPORTED, "dkd_retrieval_scan: dtype must be DKD_F16 or DKD_F32", nullptr);
     const size_t rowb = static_cast<size_t>(D) * (dtype == DKD_F16 ? 2 : 4);
-    if (rowb % 16 != 0 || rowb > 16 * 8 * SC_THREADS)
-        return dkd_ctx_fail(ctx, DKD_ERR_UNSUPPORTED, "dkd_retrieval_scan: D * elemsize must be a multiple of 16 and <= 32768", nullptr);
+    if (rowb % 16 != 0 || D > 16384)
+        return dkd_ctx_fail(ctx, DKD_ERR_UNSUPPORTED, "dkd_retrieval_scan: D * elemsize must be a multiple of 16 and D <= 16384", nullptr);
     if ((reinterpret_cast<uintptr_t>(db) & 15) || (reinterpret_cast<uintptr_t>(query) & 15))
         return dkd_ctx_fail(ctx, DKD_ERR_UNSUPPORTED, "dkd_retrieval_scan: db / query not 16-byte aligned", nullptr);
     if (max_cand > DKD_MAX_TOP_K) return dkd_ctx_fail(ctx, DKD_ERR_UNSUPPORTED, "dkd_retrieval_scan: max_cand > DKD_MAX_TOP_K", nullptr);
     DeviceGuard dg(dkd_ctx_device(ctx));
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    constexpr int WPB = SC_THREADS / 32;
     int grid = 2 * dkd_ctx_num_sms(ctx);
-    if (grid > (n + 1) / 2) grid = (n + 1) / 2;
+    if (grid > (n + SC_R * WPB - 1) / (SC_R * WPB)) grid = (n + SC_R * WPB - 1) / (SC_R * WPB);
     if (grid < 1) grid = 1;
-    const int seg_cap = 2 * ((n + 2 * grid - 1) / (2 * grid)) + 2;        // rows one CTA can see
-    const size_t b_seg = (static_cast<size_t>(grid) * seg_cap * 8 + 255) & ~static_cast<size_t>(255);
-    const size_t b_cnt = (static_cast<size_t>(grid) * 4 + 255) & ~static_cast<size_t>(255);
+    const int nwarps = grid * WPB;
+    const int seg_cap = SC_R * ((n + SC_R * nwarps - 1) / (SC_R * nwarps)) + SC_R;      // rows one warp can see
+    const size_t b_seg = (static_cast<size_t>(nwarps) * seg_cap * 8 + 255) & ~static_cast<size_t>(255);
+    const size_t b_cnt = (static_cast<size_t>(nwarps) * 4 + 255) & ~static_cast<size_t>(255);
     const size_t b_sim = out_sim ? 0 : ((static_cast<size_t>(n > 0 ? n : 1) * 4 + 255) & ~static_cast<size_t>(255));
     unsigned char* ws = static_cast<unsigned char*>(dkd_ctx_scratch(ctx, 1, b_seg + b_cnt + b_sim));
     if (!ws) return DKD_ERR_CUDA;
@@ -643,20 +657,19 @@ int dkd_retrieval_scan(dkd_ctx* ctx, const void* db, int dtype, int n, int D, co
     sp.n = n; sp.chunks = static_cast<int>(rowb / 16); sp.n_eligible = n - n_exclude; sp.tau = tau;
     sp.out_sim = out_sim ? out_sim : reinterpret_cast<float*>(ws + b_seg + b_cnt);
     sp.seg = reinterpret_cast<uint64_t*>(ws); sp.seg_cnt = reinterpret_cast<int*>(ws + b_seg); sp.seg_cap = seg_cap;
-    const int nch = (sp.chunks + SC_THREADS - 1) / SC_THREADS;
-#define DKD_SCAN(DT, NCH) k_scan<DT, NCH><<<grid, SC_THREADS, 0, st>>>(sp)
-#define DKD_SCAN_DT(DT)                                                                             \
-    switch (nch) {                                                                                  \
-        case 1: DKD_SCAN(DT, 1); break; case 2: DKD_SCAN(DT, 2); break; case 3: DKD_SCAN(DT, 3); break; \
-        case 4: DKD_SCAN(DT, 4); break; case 5: DKD_SCAN(DT, 5); break; case 6: DKD_SCAN(DT, 6); break; \
-        case 7: DKD_SCAN(DT, 7); break; default: DKD_SCAN(DT, 8); break;                              \
+    const size_t smem_q = static_cast<size_t>(D) * 4;
+    static bool scan_attr = false;
+    if (!scan_attr) {
+        cudaError_t ea = cudaFuncSetAttribute(k_scan<DKD_F16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+        if (ea == cudaSuccess) ea = cudaFuncSetAttribute(k_scan<DKD_F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+        if (ea != cudaSuccess) return dkd_ctx_fail(ctx, DKD_ERR_CUDA, "k_scan attribute: ", cudaGetErrorString(ea));
+        scan_attr = true;
     }
-    if (dtype == DKD_F16) { DKD_SCAN_DT(DKD_F16) } else { DKD_SCAN_DT(DKD_F32) }
-#undef DKD_SCAN_DT
-#undef DKD_SCAN
+    if (dtype == DKD_F16) k_scan<DKD_F16><<<grid, SC_THREADS, smem_q, st>>>(sp);
+    else k_scan<DKD_F32><<<grid, SC_THREADS, smem_q, st>>>(sp);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return dkd_ctx_fail(ctx, DKD_ERR_CUDA, "k_scan launch: ", cudaGetErrorString(e));
-    const int rc = dkd_internal_select(ctx, sp.seg, sp.seg_cnt, grid, seg_cap, max_cand, n > 0 ? n : 1, out_cand, out_count, st);
+    const int rc = dkd_internal_select(ctx, sp.seg, sp.seg_cnt, nwarps, seg_cap, max_cand, n > 0 ? n : 1, out_cand, out_count, st);
     if (rc != DKD_OK) return rc;
     if (out_cand_sim) {
         k_cand_sims<<<(max_cand + 255) / 256, 256, 0, st>>>(out_cand, sp.out_sim, max_cand, out_cand_sim);
