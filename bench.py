@@ -13,13 +13,19 @@ through the C-ABI (`dkd_extract`, one cached CUDA-graph launch).  Per rank:
   * value / ms_per_step : K steps on inputs resident in HBM, CUDA events on the launching stream,
                           barrier + synchronize on both sides, max over ranks.  Cold inputs: the steps
                           rotate through R distinct seeded input sets whose touched bytes exceed L2.
-  * e2e                 : the same K steps through `dkd_extract_host` with pinned HOST buffers — the
-                          host->device copy of the score maps AND the descriptor map and the
-                          device->host copy of every output are inside the timed region.
+  * e2e                 : the same K steps through `dkd_extract_host` with pinned HOST buffers, everything inside
+                          the timed region: the score maps are copied host->device, the descriptor corner rows
+                          are read in place from the pinned map over PCIe (counted as h2d bytes), and the kernels
+                          store every output into the pinned host tensors (d2h bytes); synchronised per step.
+  * fresh_buffers       : the same steps with output buffers the cached graph has not seen (kernel-node update path).
   * batch64 / roofline  : config c5 (B=64 1080p, BASELINE.json configs[4]); whole-path frames/s,
                           keypoints/s, credited GB/s, and the dominant kernel's duration measured with
                           CUDA events (library measurement mode) against MEASURED_PEAKS.json.
-  * cpu_baseline        : the CPU oracle as it stands, timed on this box's host cores on c2 (rank 0).
+  * variants_c5         : c5 with the heat x reliability and validity-mask variants (NMS credited 8 B / 9 B per pixel).
+  * match / retrieval   : the consumers of the descriptors: tcgen05 matching (tensor roofline) and
+                          the keyframe-database cosine scan (HBM roofline).
+  * cpu_baseline        : the CPU oracle as it stands, timed on this box's host cores on c2 (rank 0); also with one
+                          thread, and on a sample of c5.
 
 `--impl reference` times the oracle (the reference arm of this tier) on the same config and metric.
 Nothing here reads /root/reference.  Only the cpu_baseline / reference legs touch `oracle/`.
@@ -53,7 +59,7 @@ def parse_args():
     ap.add_argument("--batch64-steps", type=int, default=30)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=0, help="0 = min(steps, 100)")
-    ap.add_argument("--leg", default="all", choices=["all", "c2", "c5", "pre"],
+    ap.add_argument("--leg", default="all", choices=["all", "c2", "c5", "pre", "match"],
                     help="profiling aid: c5 = shortest possible c2 legs (13 c2 launches) then the batch-64 leg; "
                          "c2 = no batch-64 leg; pre = shortest c2 legs, then only the pre-processing kernel.  "
                          "The driver's bench line is --leg all.")
@@ -71,18 +77,32 @@ def peaks():
     return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
-def ncu_traffic(kernel):
-    """dram read + write bytes of one launch of `kernel` at c5, from the committed ncu --set full summary
-    (profiles/traffic_c5.csv: a text table copied from the capture, not something measured in this run)."""
-    tp = os.path.join(ROOT, "profiles", "traffic_c5.csv")
+def kernels_sha():
+    """Fingerprint of the device code the committed ncu table was captured from (first 12 hex digits of the sha256 of
+    the kernel sources)."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2607_01757_b200", "csrc")
+    for f in ("dkd_kernels.cuh", "dkd_match.cu"):
+        h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:12]
+
+
+def ncu_traffic(kernel, table="traffic_c5.csv"):
+    """(dram read + write bytes of one launch of `kernel`, provenance) from the committed ncu --set full summary
+    (profiles/traffic_*.csv: a text table copied from the capture, not something measured in this run).  The table
+    records the fingerprint of the kernel sources it was captured from: `current` says whether it still matches."""
+    tp = os.path.join(ROOT, "profiles", table)
     try:
         import csv
         for row in csv.DictReader(open(tp)):
             if row["kernel"] == kernel:
-                return int(row["dram_read_bytes"]) + int(row["dram_write_bytes"])
+                sha = row.get("kernels_sha", "")
+                return (int(row["dram_read_bytes"]) + int(row["dram_write_bytes"]),
+                        {"file": "profiles/" + table, "kernels_sha": sha, "current": sha == kernels_sha()})
     except Exception:                                            # noqa: BLE001
         pass
-    return None
+    return None, None
 
 
 class ClockSampler:
@@ -139,6 +159,18 @@ class ClockSampler:
         s = sorted(self.samples)
         return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz,
                 "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+def tensor_peak():
+    """Dense fp16/bf16 tensor peak for a kernel timed alone: MEASURED_PEAKS.json bf16_tflops (burst), else the
+    profiling guide's fallback."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["bf16_tflops"]), "measured (MEASURED_PEAKS.json bf16_tflops, burst; fp16 = bf16 rate)"
+        except Exception:                                        # noqa: BLE001
+            pass
+    return 1590.0, "fallback (B200_PROFILING.md)"
 
 
 def dist_env():
@@ -239,9 +271,9 @@ def run_ours(args):
     sampler = ClockSampler(local)
     cfg = synth.CONFIGS["c2"]
     esz = 2 if cfg.desc_dtype == "f16" else 4
-    if args.leg in ("c5", "pre"):
+    if args.leg in ("c5", "pre", "match"):
         args.sets, args.steps, args.warmup, args.e2e_steps, args.no_cpu_baseline = 1, 1, 3, 1, True
-    if args.leg == "pre":
+    if args.leg in ("pre", "match"):
         args.no_batch64 = True
     if args.leg == "c2":
         args.no_batch64 = True
@@ -284,7 +316,7 @@ def run_ours(args):
 
     # single-shot latency (enqueue -> outputs complete), one pair at a time
     lat = []
-    for i in range(min(200, max(K, 20)) if args.leg not in ("c5", "pre") else 1):
+    for i in range(min(200, max(K, 20)) if args.leg not in ("c5", "pre", "match") else 1):
         torch.cuda.synchronize()
         t0 = time.perf_counter()
         calls[i % R]()
@@ -346,7 +378,7 @@ def run_ours(args):
 
     # the same steps as plain stream launches (DKD_OPT_USE_GRAPH = 0: three PDL-linked launches per step)
     stream_us = None
-    if args.leg not in ("c5", "pre"):
+    if args.leg not in ("c5", "pre", "match"):
         ctx.set_option(OPT_USE_GRAPH, 0)
         for i in range(Wm):
             calls[i % R]()
@@ -361,10 +393,37 @@ def run_ours(args):
         stream_us = max_over_ranks(ev0.elapsed_time(ev1) / K) * 1e3 / world
         ctx.set_option(OPT_USE_GRAPH, 1)
 
+    # the same steps with output buffers the cached graph has not seen: every call hands the library another output set,
+    # so each launch goes through the kernel-node update path of the shape-keyed graph cache (no capture, no instantiate)
+    fresh = None
+    if args.leg not in ("c5", "pre", "match"):
+        NF = 8
+        fouts = [[ctx.alloc_outputs(cfg.B, cfg.top_k, sets[j][1], cfg.D, want_index=False, want_offsets=False) for _ in range(NF)]
+                 for j in range(min(R, 8))]
+        fcalls = [[ctx.bind(sets[j][0], sets[j][1], cfg.stride, cfg.r, cfg.thresh, cfg.top_k, cfg.T, o, stream) for o in fouts[j]]
+                  for j in range(len(fouts))]
+        st0 = ctx.graph_stats()
+        for i in range(Wm):
+            fcalls[i % len(fcalls)][i % NF]()
+        barrier()
+        torch.cuda.synchronize()
+        ev0.record(stream)
+        for i in range(K):
+            fcalls[i % len(fcalls)][(i // len(fcalls)) % NF]()
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        barrier()
+        st1 = ctx.graph_stats()
+        fresh = {"value": max_over_ranks(ev0.elapsed_time(ev1) / K) * 1e3 / world, "unit": UNIT,
+                 "graphs_instantiated_during": st1["instantiated"] - st0["instantiated"],
+                 "node_updates_during": st1["updated"] - st0["updated"],
+                 "what": "same steps, every call with another output set (pointer miss): the cached graph's kernel nodes are updated in place"}
+        del fouts, fcalls
+
     # per-kernel device time at c2 (library measurement mode: plain launches + events)
     ctx.set_option(OPT_PROFILE, 1)
     kt2 = {}
-    nprof = 50 if args.leg not in ("c5", "pre") else 0
+    nprof = 50 if args.leg not in ("c5", "pre", "match") else 0
     for i in range(nprof + 5 if nprof else 0):
         calls[i % R]()
         d = ctx.profile_read()
@@ -471,15 +530,101 @@ def run_ours(args):
             #   nms: the score maps, read once;  refine_gather: corner rows + outputs;  select: candidate keys
             algo = {"nms": cb5["score"], "refine_gather": cb5["corners"] + cb5["outputs"], "select": 0}
             dom = max(kt5, key=kt5.get)
-            traffic = ncu_traffic(dom)
+            traffic, traffic_src = ncu_traffic(dom)
             ach = algo.get(dom, 0) / (kt5[dom] * 1e-6) / 1e9
             roof = {"bound": "hbm", "kernel": dom, "workload": "c5 (B=64 1920x1080)", "achieved": ach, "peak": hbm_peak,
-                    "unit": "GB/s", "frac": ach / hbm_peak, "traffic": traffic, "peak_source": peak_src,
+                    "unit": "GB/s", "frac": ach / hbm_peak, "traffic": traffic, "traffic_source": traffic_src,
+                    "peak_source": peak_src,
                     "algorithmic_bytes": algo.get(dom, 0), "kernel_us": kt5[dom],
                     "whole_path": {"achieved": gbs, "frac": gbs / hbm_peak, "credited_bytes": cb5["total"]}}
+            # the variants of SURVEY.md 8(f) f2 at c5: heat x reliability streamed as a second TMA stream (the NMS now
+            # moves 8 B per pixel), and the validity mask (read only at candidates)
+            var5 = None
+            if args.leg in ("all", "c5") and world == 1:
+                var5 = {}
+                g5 = torch.Generator(device=dev).manual_seed(5)
+                rel5 = torch.rand(score5.shape, generator=g5, device=dev) * 0.5 + 0.5
+                msk5 = (torch.rand(score5.shape, generator=g5, device=dev) < 0.9).to(torch.uint8)
+                ctx5.set_option(OPT_PROFILE, 1)
+                for name, kw, bpp in (("reliability", dict(reliability=rel5), 8), ("mask", dict(valid_mask=msk5), 4),
+                                      ("reliability+mask", dict(reliability=rel5, valid_mask=msk5), 8)):
+                    acc = {}
+                    for i in range(8):
+                        ctx5.extract(score5, desc5, c5.stride, c5.r, 0.1 if "reliability" in name else c5.thresh, c5.top_k, c5.T,
+                                     out=out5, want_index=False, want_offsets=False, **kw)
+                        d = ctx5.profile_read()
+                        if i >= 3:
+                            for k, v in d.items():
+                                acc[k] = acc.get(k, 0.0) + v * 1e3 / 5
+                    nb = c5.B * c5.H * c5.W * bpp
+                    var5[name] = {"kernel_us": acc, "nms_algorithmic_bytes": nb, "nms_gbs": nb / acc["nms"] / 1e3,
+                                  "nms_frac_of_hbm_peak": nb / acc["nms"] / 1e3 / hbm_peak}
+                ctx5.set_option(OPT_PROFILE, 0)
+                del rel5, msk5
+            b64["variants"] = var5
             del score5, desc5, out5, call5
             ctx5.close()
             torch.cuda.empty_cache()
+
+    # ---- consumers of the descriptors: tcgen05 matching and the keyframe-database scan -----------
+    match_leg, retr_leg = None, None
+    if args.leg in ("all", "match") and world == 1:
+        tf_peak, tf_src = tensor_peak()
+        ctxm = dkd.DKD(2, 64, 128, 64, 0, device=local)
+
+        def graph_time(fn, per_graph, reps):
+            """GPU time of one call: `per_graph` calls captured into one graph (no Python between them), replayed."""
+            fn(None)
+            torch.cuda.synchronize()
+            gph = torch.cuda.CUDAGraph()
+            cs = torch.cuda.Stream(device=dev)
+            with torch.cuda.stream(cs), torch.cuda.graph(gph, stream=cs):
+                for _ in range(per_graph):
+                    fn(cs)
+            for _ in range(3):
+                gph.replay()
+            torch.cuda.synchronize()
+            ev0.record(stream)
+            for _ in range(reps):
+                gph.replay()
+            ev1.record(stream)
+            torch.cuda.synchronize()
+            return ev0.elapsed_time(ev1) * 1e3 / (reps * per_graph)
+
+        match_leg = {"what": "dkd_match: P = 2 pairs (temporal + stereo, PAPER.md:132) of N x N x D fp16 descriptor sets, ratio 0.8; "
+                             "us per call = k_match_tc + k_match_finalize, GPU time from graph replays",
+                     "peak_tflops": tf_peak, "peak_source": tf_src, "sizes": {}}
+        for (Nn, Dd) in ((256, 128), (1024, 128), (2048, 256), (4096, 128), (4096, 256)):
+            A, Bm, cnta, cntb = synth.match_sets(2, Nn, Nn, Dd, seed=Nn + Dd)
+            A, Bm, cnta, cntb = A.to(dev), Bm.to(dev), cnta.to(dev), cntb.to(dev)
+            us = graph_time(lambda s_: ctxm.match(A, Bm, cnta, cntb, ratio=0.8, stream=s_), 10, 10)
+            fl = 2.0 * Nn * Nn * Dd * 2
+            match_leg["sizes"][f"N{Nn}_D{Dd}"] = {"us": us, "flops": fl, "tflops": fl / us / 1e6, "frac_of_tensor_peak": fl / us / 1e6 / tf_peak}
+        big = match_leg["sizes"]["N4096_D256"]
+        match_leg["roofline"] = {"bound": "tensor", "kernel": "k_match_tc", "workload": "P=2 N=4096 D=256 fp16", "achieved": big["tflops"],
+                                 "peak": tf_peak, "unit": "TFLOP/s", "frac": big["frac_of_tensor_peak"], "traffic": None,
+                                 "peak_source": tf_src, "algorithmic_flops": big["flops"], "kernel_us": big["us"]}
+        # retrieval: AnyLoc-sized descriptors (32 x 384 = 12288, PAPER.md:149); 20 000 keyframes = 492 MB > L2
+        nk, Dg = 20000, 12288
+        gq = torch.Generator(device=dev).manual_seed(11)
+        db = torch.randn((nk, Dg), generator=gq, device=dev)
+        db = (db / db.norm(dim=1, keepdim=True)).half()
+        qv = db[17].float() * 0.8 + 0.6 * torch.nn.functional.normalize(torch.randn(Dg, generator=gq, device=dev), dim=0)
+        qv = torch.nn.functional.normalize(qv, dim=0).half()
+        us = graph_time(lambda s_: ctxm.retrieval_scan(db, qv, 50, 0.60, 16, stream=s_), 4, 10)
+        _, cand, _, cnt = ctxm.retrieval_scan(db, qv, 50, 0.60, 16)
+        torch.cuda.synchronize()
+        assert int(cnt[0]) == 1 and int(cand[0]) == 17
+        nbytes = nk * Dg * 2
+        tr, tr_src = ncu_traffic("scan", "traffic_f3.csv")
+        retr_leg = {"what": "dkd_retrieval_scan: one 12288-d fp16 query over 20000 keyframes (492 MB > L2), skip 50 newest, tau 0.60; "
+                            "us per call = k_scan + k_select + k_cand_sims", "us": us,
+                    "roofline": {"bound": "hbm", "kernel": "k_scan (+ select)", "workload": "n=20000 D=12288 fp16", "achieved": nbytes / us / 1e3,
+                                 "peak": hbm_peak, "unit": "GB/s", "frac": nbytes / us / 1e3 / hbm_peak, "traffic": tr,
+                                 "traffic_source": tr_src, "peak_source": peak_src, "algorithmic_bytes": nbytes, "kernel_us": us}}
+        del db, qv
+        ctxm.close()
+        torch.cuda.empty_cache()
 
     # ---- fused input pre-processing kernel (SURVEY.md 8(f) f1; PAPER.md:126-128): stereo pair + batch 64 ----
     pre = None
@@ -543,6 +688,30 @@ def run_ours(args):
         cpu = {"value": ts[len(ts) // 2] * 1e6, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
                "sample": f"the full c2 stereo pair (O1-O5 incl. descriptors), median of {len(ts)} runs, host-resident inputs",
                "best": ts[0] * 1e6}
+        # the same oracle on ONE thread, and on a sample of c5 (two figures, an oracle time beside c5)
+        try:
+            import ctypes
+            gomp = ctypes.CDLL("libgomp.so.1")
+            nthr = oracle.num_threads()
+            gomp.omp_set_num_threads(1)
+            t1 = []
+            for _ in range(3):
+                t0 = time.perf_counter()
+                oracle.extract(s_np, d_np, cfg.stride, cfg.r, cfg.thresh, cfg.top_k, cfg.T)
+                t1.append(time.perf_counter() - t0)
+            gomp.omp_set_num_threads(nthr)
+            cpu["one_thread"] = {"value": min(t1) * 1e6, "unit": UNIT, "cores": 1, "sample": "the full c2 stereo pair, best of 3"}
+        except Exception as e:                                   # noqa: BLE001
+            cpu["one_thread"] = {"error": str(e)}
+        if not args.no_batch64:
+            c5c = synth.CONFIGS["c5"]
+            s5 = synth.score_maps(4, c5c.H, c5c.W, c5c.seed, c5c.base, c5c.nblobs).numpy()
+            t0 = time.perf_counter()
+            oracle.extract(s5, None, 1, c5c.r, c5c.thresh, c5c.top_k, c5c.T)
+            dt5 = time.perf_counter() - t0
+            cpu["c5"] = {"value": dt5 / 4 * c5c.B * 1e6, "unit": "us per batch of 64 (extrapolated)", "cores": oracle.num_threads(),
+                         "sample": "steps O1-O3, O5 on 4 of the 64 frames of c5 (keypoints only: the 34 GB descriptor map is not "
+                                   "materialised on the host), scaled to 64 frames"}
 
     if rank == 0:
         us_pair = ms_step * 1e3 / world
@@ -560,6 +729,7 @@ def run_ours(args):
                            "what": "single shot: enqueue -> stream idle, host clock"},
             "stream_launch": {"value": stream_us, "unit": UNIT,
                               "what": "same steps with DKD_OPT_USE_GRAPH = 0: three PDL-linked launches per step instead of one graph launch"},
+            "fresh_buffers": fresh,
             "kernel_us_c2": kt2,
             "clocks": sampler.summary(),
             "e2e": {"value": e2e_us / world, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
@@ -571,7 +741,7 @@ def run_ours(args):
                                   "d2h_bytes_per_step": d2h,
                                   "what": "same, descriptor map left on the device by the previous call (network output)"},
             "gpu_launches": K * 3,
-            "batch64": b64, "roofline": roof, "cpu_baseline": cpu, "preprocess": pre, "cap_sweep": cap_sweep, "other_configs": other_cfgs,
+            "batch64": b64, "roofline": roof, "cpu_baseline": cpu, "match": match_leg, "retrieval": retr_leg, "preprocess": pre, "cap_sweep": cap_sweep, "other_configs": other_cfgs,
             "context": "paper: whole pipeline 29-47 FPS mono / 18-33 FPS stereo on Jetson AGX Orin (PAPER.md:5) — other hardware, whole system",
         }
         print(json.dumps(line), flush=True)

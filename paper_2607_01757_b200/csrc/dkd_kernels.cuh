@@ -107,6 +107,19 @@ __device__ __forceinline__ uint64_t l2_evict_first_policy() {
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
     return p;
 }
+// The candidate lists are small (a few MB) and are read back by k_select right after the NMS pass has streamed half a
+// gigabyte through L2: written with an evict-last policy they are still in L2 when k_select gathers them.
+__device__ __forceinline__ uint64_t l2_evict_last_policy() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void st_keep_u64(uint64_t* p, uint64_t v, uint64_t policy) {
+    asm volatile("st.global.L2::cache_hint.b64 [%0], %1, %2;" ::"l"(p), "l"(v), "l"(policy) : "memory");
+}
+__device__ __forceinline__ void st_keep_s32(int* p, int v, uint64_t policy) {
+    asm volatile("st.global.L2::cache_hint.b32 [%0], %1, %2;" ::"l"(p), "r"(v), "l"(policy) : "memory");
+}
 __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* tmap) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(tmap)) : "memory");
 }
@@ -221,7 +234,7 @@ template <int R, bool PROD>
 __device__ __forceinline__ int nms_emit(const unsigned (&neg)[4], unsigned colmask, int X, int yc, int H, int W,
                                         const float4 (&cat)[TH + 2 * R], const float* __restrict__ rows,
                                         const float* __restrict__ rows2, const uint8_t* __restrict__ mask_img,
-                                        uint64_t* __restrict__ seg, int seg_room) {
+                                        uint64_t* __restrict__ seg, int seg_room, uint64_t keep) {
     constexpr unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     unsigned rowmask = 0xffu;                                // bit TH-1-o = output row o is valid
@@ -265,7 +278,7 @@ __device__ __forceinline__ int nms_emit(const unsigned (&neg)[4], unsigned colma
         const unsigned tb = __ballot_sync(FULL, take);
         if (take) {
             DKD_ASSERT(cnt + __popc(tb & ((1u << lane) - 1u)) < seg_room);
-            seg[cnt + __popc(tb & ((1u << lane) - 1u))] = key;
+            st_keep_u64(seg + cnt + __popc(tb & ((1u << lane) - 1u)), key, keep);
         }
         cnt += __popc(tb);
         bal = __ballot_sync(FULL, w != 0u);
@@ -359,6 +372,7 @@ __global__ void __launch_bounds__(NMS_WARPS * 32, PROD ? 1 : 2) k_nms_tma(const 
     uint64_t* bar = bars + warp * NMS_STAGES;
 
     const uint64_t policy = l2_evict_first_policy();
+    const uint64_t keep = l2_evict_last_policy();
     // issue side (every lane tracks the cursor, lane 0 issues): next box = chunk ic of unit iteration iit
     int iit = 0, ic = 0, issued = 0;
     UnitCoords iu = unit_coords(first, p);
@@ -420,14 +434,14 @@ __global__ void __launch_bounds__(NMS_WARPS * 32, PROD ? 1 : 2) k_nms_tma(const 
             unsigned neg[4];
             nms_rows<R, NEGT>(cat, p.thr_up, neg);
             ucnt += nms_emit<R, PROD>(neg, colmask, X, cu.y0 + TH * c, p.H, p.W, cat, rows, rows2, mask_img, useg + ucnt,
-                                      p.cpu * SEG_CAP - ucnt);
+                                      p.cpu * SEG_CAP - ucnt, keep);
             __syncwarp();                                    // every lane is done with stage s
             issue_box();                                     // (the other NMS_STAGES-1 boxes stay in flight meanwhile)
             ++consumed;
 #pragma unroll
             for (int q = 0; q < 2 * R; ++q) cat[q] = cat[TH + q];   // the 2R rows above the next strip-tile
         }
-        if (lane == 0) seg_cnt[u] = ucnt;
+        if (lane == 0) st_keep_s32(seg_cnt + u, ucnt, keep);
         if (it + 1 < n_my) cu = unit_coords(first + (it + 1) * step, p);
     }
 }
@@ -477,7 +491,8 @@ __global__ void __launch_bounds__(PLAIN_WARPS * 32) k_nms_plain(const float* __r
     unsigned neg[4];
     nms_rows<R, true>(cat, p.thr_up, neg);
     const int cnt = nms_emit<R, false>(neg, strip_colmask(X, p.W, R), X, y0, p.H, p.W, cat, boxes[warp], nullptr,
-                                       mask ? mask + b * img_px : nullptr, cand + static_cast<size_t>(t) * SEG_CAP, SEG_CAP);
+                                       mask ? mask + b * img_px : nullptr, cand + static_cast<size_t>(t) * SEG_CAP, SEG_CAP,
+                                       l2_evict_last_policy());
     if (lane == 0) seg_cnt[t] = cnt;
 }
 
