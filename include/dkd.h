@@ -161,7 +161,10 @@ int dkd_extract_ex(dkd_ctx* ctx,
  *                mask that culls features near the image periphery").  Masked pixels still take part
  *                in every window maximum and in the refinement windows.
  *   nms_iters    0 = one (2r+1)^2 max-pool pass (north_star).  n > 0 = the iterated suppress-and-recover NMS of "the
- *                original PyTorch NMS" with n recovery rounds (the published procedure uses 2).
+ *                original PyTorch NMS" with n recovery rounds (the published procedure uses 2):
+ *                M = (S == maxpool S); n times: supp = maxpool(M) > 0, S' = supp ? 0 : S, M |= (S' == maxpool S') & !supp,
+ *                windows clipped at the image edge; border exclusion and threshold apply to the final mask.  Runs in its
+ *                own tiled shared-memory kernel; (2 n + 1) r must be <= 40 (DKD_ERR_UNSUPPORTED otherwise).
  *   score_mode   DKD_SCORE_RAW: out_scores = S at the integer peak (bit-exact).  DKD_SCORE_BILINEAR: out_scores = S
  *                interpolated bilinearly at the refined position (x+dx, y+dy).  Selection and order always use the
  *                raw score.

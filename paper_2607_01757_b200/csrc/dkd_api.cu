@@ -276,13 +276,27 @@ void plan_rg(const ExtractArgs& a, const int32_t* sel, bool pdl, KLaunch& k) {
 // The launches of one extract (launch geometry + argument values).  Pure host work: nothing touches a stream.
 cudaError_t build_plan(dkd_ctx* ctx, const ExtractArgs& a, Plan& pl) {
     const NmsPlan plan = nms_plan(ctx, a);
-    const int tpi = plan.strips_x * plan.segs;              // candidate segments (NMS units) per image
-    cudaError_t e;
-    switch (a.r) {
-        case 1: e = plan_nms<1>(ctx, a, plan, pl.k[0]); break;
-        case 2: e = plan_nms<2>(ctx, a, plan, pl.k[0]); break;
-        case 3: e = plan_nms<3>(ctx, a, plan, pl.k[0]); break;
-        default: e = plan_nms<4>(ctx, a, plan, pl.k[0]); break;
+    int tpi = plan.strips_x * plan.segs;                    // candidate segments (NMS units) per image
+    int seg_cap = plan.cpu * SEG_CAP;
+    cudaError_t e = cudaSuccess;
+    if (a.nms_iters > 0) {                                  // variant V1: tiles of T x T pixels, one segment each
+        IterParams ip;
+        memset(&ip, 0, sizeof(ip));
+        ip.score = a.score; ip.score2 = a.score2; ip.mask = a.mask; ip.H = a.H; ip.W = a.W; ip.r = a.r; ip.iters = a.nms_iters;
+        ip.halo = (2 * a.nms_iters + 1) * a.r;
+        ip.T = (IT_REG - 2 * ip.halo) & ~7;
+        ip.tiles_x = (a.W + ip.T - 1) / ip.T; ip.tiles_y = (a.H + ip.T - 1) / ip.T;
+        ip.thresh = a.thresh; ip.cand = ctx->cand; ip.seg_cnt = ctx->tile_cnt;
+        prep(pl.k[0], k_nms_iter, dim3(ip.tiles_x * ip.tiles_y, a.B), dim3(IT_THREADS), IT_SMEM_BYTES, false, ip);
+        tpi = ip.tiles_x * ip.tiles_y;
+        seg_cap = ip.T * ip.T;
+    } else {
+        switch (a.r) {
+            case 1: e = plan_nms<1>(ctx, a, plan, pl.k[0]); break;
+            case 2: e = plan_nms<2>(ctx, a, plan, pl.k[0]); break;
+            case 3: e = plan_nms<3>(ctx, a, plan, pl.k[0]); break;
+            default: e = plan_nms<4>(ctx, a, plan, pl.k[0]); break;
+        }
     }
     if (e != cudaSuccess) return e;
     int32_t* sel = a.out_index ? a.out_index : ctx->sel_idx;
@@ -298,7 +312,7 @@ cudaError_t build_plan(dkd_ctx* ctx, const ExtractArgs& a, Plan& pl) {
         pf.img_px = static_cast<size_t>(a.H) * a.W;
     }
     prep(pl.k[1], k_select, dim3(a.B), dim3(SEL_THREADS), SEL_SMEM_BYTES, pdl, ctx->cand, ctx->tile_cnt, tpi,
-         plan.cpu * SEG_CAP, a.top_k, idx_shift, pf, sel, a.out_count, a.out_total);
+         seg_cap, a.top_k, idx_shift, pf, sel, a.out_count, a.out_total);
     plan_rg(a, sel, pdl, pl.k[2]);
     pl.n = 3;
     return cudaSuccess;
@@ -338,7 +352,14 @@ int validate_shapes(dkd_ctx* ctx, const ExtractArgs& a) {
             return fail(ctx, DKD_ERR_UNSUPPORTED, "desc_dtype must be DKD_F32 or DKD_F16");
     }
     if (a.r > DKD_MAX_RADIUS) return fail(ctx, DKD_ERR_UNSUPPORTED, "r > DKD_MAX_RADIUS");
-    if (a.nms_iters > 0) return fail(ctx, DKD_ERR_UNSUPPORTED, "iterated NMS (nms_iters > 0) is not built yet");
+    if (a.nms_iters > 0) {
+        const long long halo = (2LL * a.nms_iters + 1) * a.r;
+        if (halo > 40) return fail(ctx, DKD_ERR_UNSUPPORTED, "iterated NMS: (2 nms_iters + 1) r must be <= 40");
+        const int T = (IT_REG - 2 * static_cast<int>(halo)) & ~7;
+        const long long tiles = static_cast<long long>((a.W + T - 1) / T) * ((a.H + T - 1) / T) * a.B;
+        if (tiles * T * T > static_cast<long long>(ctx->max_tiles) * SEG_CAP)
+            return fail(ctx, DKD_ERR_CAPACITY, "iterated NMS: candidate workspace too small for these tiles (raise the dkd_create maxima)");
+    }
     if (a.B > 65535) return fail(ctx, DKD_ERR_UNSUPPORTED, "B > 65535");
     if (a.desc) {
         const size_t rowb = static_cast<size_t>(a.D) * (a.desc_dtype == DKD_F16 ? 2 : 4);
@@ -649,6 +670,7 @@ int dkd_create(const dkd_create_params* p, dkd_ctx** out) {
     CKC(setup_nms<3>(ctx));
     CKC(setup_nms<4>(ctx));
     CKC(cudaFuncSetAttribute(k_select, cudaFuncAttributeMaxDynamicSharedMemorySize, SEL_SMEM_BYTES));
+    CKC(cudaFuncSetAttribute(k_nms_iter, cudaFuncAttributeMaxDynamicSharedMemorySize, IT_SMEM_BYTES));
     const size_t tx = (p->max_w + STRIP_W - 1) / STRIP_W, ty = (p->max_h + TH - 1) / TH;
     ctx->max_tiles = tx * (ty + MAX_CPU - 1) * p->max_batch;   // segments of whole units: up to MAX_CPU-1 spare strip-tiles per strip
     const size_t b_cand = align256(ctx->max_tiles * SEG_CAP * sizeof(uint64_t));

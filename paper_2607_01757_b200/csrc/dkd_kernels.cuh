@@ -496,6 +496,146 @@ __global__ void __launch_bounds__(PLAIN_WARPS * 32) k_nms_plain(const float* __r
     if (lane == 0) seg_cnt[t] = cnt;
 }
 
+// ---- k_nms_iter: the iterated suppress-and-recover NMS variant (V1) -----------------------
+//   M = (S == maxpool(S));  repeat n times:  supp = maxpool(M) > 0;  S' = supp ? 0 : S;  M |= (S' == maxpool(S')) & !supp
+// with (2r+1)^2 windows clipped at the image edge.  The mask at a pixel depends on S within (2n+1) r pixels, so a CTA
+// loads an IT_REG x IT_REG region (out-of-image pixels = -inf) into shared memory, runs every pooling stage on the
+// whole region as a separable row / column pass (values near the region's edge are wrong, but no output of the inner
+// T x T tile, T = IT_REG - 2 (2n+1) r, depends on them), applies border / threshold / validity mask to the tile and
+// appends its candidates to the tile's private segment (block scan, no atomics) for k_select.  A variant kernel: plain
+// loads, no TMA; the single-pass kernels above stay the hot path.
+constexpr int IT_REG = 104;
+constexpr int IT_THREADS = 256;
+constexpr int IT_SMEM_BYTES = IT_REG * IT_REG * (3 * 4 + 3);
+struct IterParams {
+    const float* score;
+    const float* score2;
+    const uint8_t* mask;
+    int H, W, r, iters, T, halo, tiles_x, tiles_y;
+    float thresh;
+    uint64_t* cand;
+    int* seg_cnt;
+};
+__global__ void __launch_bounds__(IT_THREADS, 1) k_nms_iter(const __grid_constant__ IterParams p) {
+    extern __shared__ __align__(16) unsigned char it_smem[];
+    constexpr int NPX = IT_REG * IT_REG;
+    float* S = reinterpret_cast<float*>(it_smem);
+    float* Sp = S + NPX;
+    float* tmp = Sp + NPX;
+    uint8_t* M = reinterpret_cast<uint8_t*>(tmp + NPX);
+    uint8_t* tb = M + NPX;
+    uint8_t* sup = tb + NPX;
+    __shared__ int s_scan[IT_THREADS / 32];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tx = blockIdx.x % p.tiles_x, ty = blockIdx.x / p.tiles_x, b = blockIdx.y;
+    const int x0 = tx * p.T - p.halo, y0 = ty * p.T - p.halo;     // image coordinates of the region's origin
+    const size_t img_px = static_cast<size_t>(p.H) * p.W;
+    const float* img = p.score + b * img_px;
+    const float* img2 = p.score2 ? p.score2 + b * img_px : nullptr;
+    const int r = p.r;
+    pdl_launch_dependents();
+    for (int i = tid; i < NPX; i += IT_THREADS) {
+        const int ry = i / IT_REG, rx = i - ry * IT_REG, gy = y0 + ry, gx = x0 + rx;
+        float v = -INFINITY;
+        if (gy >= 0 && gy < p.H && gx >= 0 && gx < p.W) {
+            const size_t e = static_cast<size_t>(gy) * p.W + gx;
+            v = __ldg(img + e);
+            if (img2) v = __fmul_rn(v, __ldg(img2 + e));
+        }
+        S[i] = v;
+    }
+    __syncthreads();
+    // separable window maximum of `src` over the region: row pass into tmp, then the column pass is folded into its user
+    auto row_max = [&](const float* src) {
+        for (int i = tid; i < NPX; i += IT_THREADS) {
+            const int ry = i / IT_REG, rx = i - ry * IT_REG;
+            const int a = rx - r < 0 ? 0 : rx - r, e = rx + r >= IT_REG ? IT_REG - 1 : rx + r;
+            float m = src[ry * IT_REG + a];
+            for (int x = a + 1; x <= e; ++x) m = fmaxf(m, src[ry * IT_REG + x]);
+            tmp[i] = m;
+        }
+    };
+    auto col_max_at = [&](int ry, int rx) {
+        const int a = ry - r < 0 ? 0 : ry - r, e = ry + r >= IT_REG ? IT_REG - 1 : ry + r;
+        float m = tmp[a * IT_REG + rx];
+        for (int y = a + 1; y <= e; ++y) m = fmaxf(m, tmp[y * IT_REG + rx]);
+        return m;
+    };
+    row_max(S);
+    __syncthreads();
+    for (int i = tid; i < NPX; i += IT_THREADS) {
+        const int ry = i / IT_REG, rx = i - ry * IT_REG;
+        M[i] = (S[i] != -INFINITY && S[i] == col_max_at(ry, rx)) ? 1 : 0;      // out-of-image pixels are never maxima
+    }
+    __syncthreads();
+    for (int it = 0; it < p.iters; ++it) {
+        for (int i = tid; i < NPX; i += IT_THREADS) {            // supp = dilate(M): row pass
+            const int ry = i / IT_REG, rx = i - ry * IT_REG;
+            const int a = rx - r < 0 ? 0 : rx - r, e = rx + r >= IT_REG ? IT_REG - 1 : rx + r;
+            uint8_t m = 0;
+            for (int x = a; x <= e; ++x) m |= M[ry * IT_REG + x];
+            tb[i] = m;
+        }
+        __syncthreads();
+        for (int i = tid; i < NPX; i += IT_THREADS) {            // column pass, and S' = supp ? 0 : S
+            const int ry = i / IT_REG, rx = i - ry * IT_REG;
+            const int a = ry - r < 0 ? 0 : ry - r, e = ry + r >= IT_REG ? IT_REG - 1 : ry + r;
+            uint8_t m = 0;
+            for (int y = a; y <= e; ++y) m |= tb[y * IT_REG + rx];
+            sup[i] = m;
+            Sp[i] = S[i] == -INFINITY ? -INFINITY : (m ? 0.0f : S[i]);
+        }
+        __syncthreads();
+        row_max(Sp);
+        __syncthreads();
+        for (int i = tid; i < NPX; i += IT_THREADS) {            // recover: maxima of S' outside the suppression mask
+            const int ry = i / IT_REG, rx = i - ry * IT_REG;
+            if (!sup[i] && Sp[i] != -INFINITY && Sp[i] == col_max_at(ry, rx)) M[i] = 1;
+        }
+        __syncthreads();
+    }
+    // the inner T x T tile: border exclusion, strict threshold, validity mask -> keys, compacted in pixel order
+    const int tile_px = p.T * p.T;
+    const uint8_t* vm = p.mask ? p.mask + b * img_px : nullptr;
+    auto is_cand = [&](int t, int& idx, float& v) {
+        const int ly = t / p.T, lx = t - ly * p.T;
+        const int gy = ty * p.T + ly, gx = tx * p.T + lx;
+        if (gy < r || gy >= p.H - r || gx < r || gx >= p.W - r) return false;
+        const int ri = (ly + p.halo) * IT_REG + lx + p.halo;
+        v = S[ri];
+        idx = gy * p.W + gx;
+        return M[ri] != 0 && v > p.thresh && (vm == nullptr || __ldg(vm + idx) != 0);
+    };
+    // each thread owns a contiguous run of the tile's pixels, so the segment is filled in pixel order
+    const int per = (tile_px + IT_THREADS - 1) / IT_THREADS;
+    const int t_lo = tid * per, t_hi = min(t_lo + per, tile_px);
+    int mine = 0;
+    for (int t = t_lo; t < t_hi; ++t) {
+        int idx;
+        float v;
+        mine += is_cand(t, idx, v) ? 1 : 0;
+    }
+    int incl = mine;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int up = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += up;
+    }
+    if (lane == 31) s_scan[warp] = incl;
+    __syncthreads();
+    int base = 0;
+    for (int w = 0; w < warp; ++w) base += s_scan[w];
+    int pos = base + incl - mine;
+    const int seg_id = (b * p.tiles_y + ty) * p.tiles_x + tx;
+    uint64_t* seg = p.cand + static_cast<size_t>(seg_id) * tile_px;
+    for (int t = t_lo; t < t_hi; ++t) {
+        int idx;
+        float v;
+        if (is_cand(t, idx, v)) { DKD_ASSERT(pos < tile_px); seg[pos++] = make_key(v, idx); }
+    }
+    if (tid == IT_THREADS - 1) p.seg_cnt[seg_id] = base + incl;
+}
+
 // ---- k_select: per-image top-k select + order ---------------------------------------------------
 // One CTA per image.  n = sum of the image's strip-tile counts.
 //   gather        : every key (n = sum of the image's strip-tile counts) is copied into shared memory.

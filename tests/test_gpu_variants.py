@@ -147,9 +147,53 @@ def test_xfeat_like_config_with_reliability_full_size():
         c.close()
 
 
-def test_iterated_nms_is_reported_as_unsupported_until_built(ctx):
+@pytest.mark.parametrize("r,iters", [(1, 1), (2, 1), (2, 2), (3, 2), (4, 2), (2, 3), (1, 5)])
+@pytest.mark.parametrize("HW", [(75, 300), (130, 97), (203, 252)])
+def test_iterated_suppress_and_recover_nms(ctx, r, iters, HW):
+    H, W = HW
+    score, desc, rel, vm = inputs(2, H, W, seed=11 * r + iters + H, nblobs=400, D=64)
+    res = ctx.extract(score.cuda(), desc, 1, r, 0.15, 256, 0.1, nms_iters=iters, want_total=True)
+    ref = oracle.extract_var(score.numpy(), desc.cpu().numpy(), 1, r, 0.15, 256, 0.1, nms_iters=iters)
+    compare_var(res, ref, torch.float16)
+    single = oracle.extract_var(score.numpy(), None, 1, r, 0.15, 256, 0.1)
+    assert np.all(ref.total > single.total)                                   # recovery adds candidates
+
+
+def test_iterated_nms_composes_with_the_other_variants_and_plateaus(ctx):
+    score, desc, rel, vm = inputs(2, 140, 260, seed=3, nblobs=300, D=32, dtype=torch.float32)
+    res = ctx.extract(score.cuda(), desc, 1, 2, 0.05, 300, 0.1, nms_iters=2, reliability=rel.cuda(), valid_mask=vm.cuda(),
+                      score_mode=1, want_total=True)
+    ref = oracle.extract_var(score.numpy(), desc.cpu().numpy(), 1, 2, 0.05, 300, 0.1, nms_iters=2, reliability=rel.numpy(),
+                             valid_mask=vm.numpy(), score_mode=1)
+    compare_var(res, ref, torch.float32, bilinear=True)
+    # plateaus and exact ties (quantised map), image smaller than one tile, border pixels
+    g = torch.Generator().manual_seed(8)
+    q = (torch.randint(0, 6, (1, 40, 50), generator=g).float() / 6.0)
+    res = ctx.extract(q.cuda(), None, 1, 2, 0.1, 2048, 0.1, nms_iters=2, want_total=True)
+    ref = oracle.extract_var(q.numpy(), None, 1, 2, 0.1, 2048, 0.1, nms_iters=2)
+    compare_var(res, ref)
+    assert ref.total[0] > 50
+
+
+def test_iterated_nms_full_size_c2():
+    import paper_2607_01757_b200 as dkd
+    cfg = synth.CONFIGS["c2"]
+    c = dkd.DKD(cfg.B, cfg.H, cfg.W, cfg.top_k, cfg.D)
+    try:
+        score, desc = synth.make_inputs(cfg, device="cuda")
+        res = c.extract(score.cuda(), desc, cfg.stride, cfg.r, cfg.thresh, cfg.top_k, cfg.T, nms_iters=2, want_total=True)
+        ref = oracle.extract_var(score.numpy(), desc.cpu().numpy(), cfg.stride, cfg.r, cfg.thresh, cfg.top_k, cfg.T, nms_iters=2)
+        compare_var(res, ref, torch.float16)
+    finally:
+        c.close()
+
+
+def test_iterated_nms_limits(ctx):
     import paper_2607_01757_b200 as dkd
     s = torch.zeros((1, 32, 128), device="cuda")
     with pytest.raises(dkd.DKDError) as e:
-        ctx.extract(s, None, 1, 2, 0.2, 8, 0.1, nms_iters=2)
+        ctx.extract(s, None, 1, 4, 0.2, 8, 0.1, nms_iters=5)                  # (2*5+1)*4 = 44 > 40
     assert e.value.code == -2
+    with pytest.raises(dkd.DKDError) as e:
+        ctx.extract(s, None, 1, 2, 0.2, 8, 0.1, nms_iters=-1)
+    assert e.value.code == -1
