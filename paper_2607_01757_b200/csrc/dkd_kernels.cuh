@@ -1285,58 +1285,62 @@ __global__ void __launch_bounds__(RG_THREADS, 4) k_refine_gather(const __grid_co
         const size_t rowb = static_cast<size_t>(p.nchunk) * 16;
         const unsigned char* base = p.desc + static_cast<size_t>(b) * p.img_bytes;
         const uint64_t policy = l2_evict_first_policy();
-        if constexpr (ITERS == 1 && RG_SLOTS / KPR <= 2) {
-            // one 16-byte chunk per lane and corner row: the corner loads of BOTH of this group's keypoints are
-            // issued before any of them is used (8 loads in flight per lane)
-            constexpr int U = RG_SLOTS / KPR;
-            uint4 q[U][4];
-            SampleInfo si[U];
-            bool live[U];
+        if (p.nchunk <= G) {                                 // (uniform) one 16-byte chunk per lane and corner row:
+            // the corner loads of TWO of this group's keypoints are issued before any of them is used
+            // (8 loads in flight per lane); G = 8: one pass of one keypoint, G = 16: one pass, G = 32: two passes
+            constexpr int ROUNDS = RG_SLOTS / KPR;           // keypoints per lane group
+            constexpr int U = ROUNDS >= 2 ? 2 : 1;
+#pragma unroll 1
+            for (int k0 = 0; k0 < ROUNDS; k0 += U) {
+                uint4 q[U][4];
+                SampleInfo si[U];
+                bool live[U];
 #pragma unroll
-            for (int u = 0; u < U; ++u) {
-                const int k = threadIdx.x / G + u * KPR;
-                si[u] = s_info[k];
-                live[u] = slot0 + k < p.top_k && si[u].o00 != 0xffffffffu && gl < p.nchunk;
-                if (live[u]) {
-                    q[u][0] = ld_stream16(reinterpret_cast<const uint4*>(base + si[u].o00 * rowb) + gl, policy);
-                    q[u][1] = ld_stream16(reinterpret_cast<const uint4*>(base + si[u].o01 * rowb) + gl, policy);
-                    q[u][2] = ld_stream16(reinterpret_cast<const uint4*>(base + si[u].o10 * rowb) + gl, policy);
-                    q[u][3] = ld_stream16(reinterpret_cast<const uint4*>(base + si[u].o11 * rowb) + gl, policy);
-                }
-            }
-#pragma unroll
-            for (int u = 0; u < U; ++u) {
-                const int k = threadIdx.x / G + u * KPR;
-                const int i_img = slot0 + k;
-                if (i_img >= p.top_k) break;                 // whole groups leave together
-                uint4* o = reinterpret_cast<uint4*>(p.out_desc + (static_cast<size_t>(b) * p.top_k + i_img) * rowb);
-                if (si[u].o00 == 0xffffffffu) {              // padding slot: zero descriptor
-                    if (gl < p.nchunk) o[gl] = make_uint4(0u, 0u, 0u, 0u);
-                    continue;
-                }
-                float acc[N];
-                float ss = 0.0f;
-                if (live[u]) {
-                    float a[N], bq[N], cq[N], dq[N];
-                    chunk_to_float<DT >= 0 ? DT : 0>(q[u][0], a);
-                    chunk_to_float<DT >= 0 ? DT : 0>(q[u][1], bq);
-                    chunk_to_float<DT >= 0 ? DT : 0>(q[u][2], cq);
-                    chunk_to_float<DT >= 0 ? DT : 0>(q[u][3], dq);
-#pragma unroll
-                    for (int e = 0; e < N; ++e) {
-                        const float d = fmaf(si[u].w11, dq[e], fmaf(si[u].w10, cq[e], fmaf(si[u].w01, bq[e], si[u].w00 * a[e])));
-                        acc[e] = d;
-                        ss = fmaf(d, d, ss);
+                for (int u = 0; u < U; ++u) {
+                    const int k = threadIdx.x / G + (k0 + u) * KPR;
+                    si[u] = s_info[k];
+                    live[u] = slot0 + k < p.top_k && si[u].o00 != 0xffffffffu && gl < p.nchunk;
+                    if (live[u]) {
+                        q[u][0] = ld_stream16(reinterpret_cast<const uint4*>(base + si[u].o00 * rowb) + gl, policy);
+                        q[u][1] = ld_stream16(reinterpret_cast<const uint4*>(base + si[u].o01 * rowb) + gl, policy);
+                        q[u][2] = ld_stream16(reinterpret_cast<const uint4*>(base + si[u].o10 * rowb) + gl, policy);
+                        q[u][3] = ld_stream16(reinterpret_cast<const uint4*>(base + si[u].o11 * rowb) + gl, policy);
                     }
                 }
 #pragma unroll
-                for (int sft = G / 2; sft > 0; sft >>= 1) ss += __shfl_xor_sync(gmask, ss, sft);
-                const float inv = __frcp_rn(fmaxf(sqrtf(ss), 1e-12f));
-                if (live[u]) {
-                    float f[N];
+                for (int u = 0; u < U; ++u) {
+                    const int k = threadIdx.x / G + (k0 + u) * KPR;
+                    const int i_img = slot0 + k;
+                    if (i_img >= p.top_k) break;             // whole groups leave together
+                    uint4* o = reinterpret_cast<uint4*>(p.out_desc + (static_cast<size_t>(b) * p.top_k + i_img) * rowb);
+                    if (si[u].o00 == 0xffffffffu) {          // padding slot: zero descriptor
+                        if (gl < p.nchunk) o[gl] = make_uint4(0u, 0u, 0u, 0u);
+                        continue;
+                    }
+                    float acc[N];
+                    float ss = 0.0f;
+                    if (live[u]) {
+                        float a[N], bq[N], cq[N], dq[N];
+                        chunk_to_float<DT >= 0 ? DT : 0>(q[u][0], a);
+                        chunk_to_float<DT >= 0 ? DT : 0>(q[u][1], bq);
+                        chunk_to_float<DT >= 0 ? DT : 0>(q[u][2], cq);
+                        chunk_to_float<DT >= 0 ? DT : 0>(q[u][3], dq);
 #pragma unroll
-                    for (int e = 0; e < N; ++e) f[e] = acc[e] * inv;
-                    o[gl] = float_to_chunk<DT >= 0 ? DT : 0>(f);
+                        for (int e = 0; e < N; ++e) {
+                            const float d = fmaf(si[u].w11, dq[e], fmaf(si[u].w10, cq[e], fmaf(si[u].w01, bq[e], si[u].w00 * a[e])));
+                            acc[e] = d;
+                            ss = fmaf(d, d, ss);
+                        }
+                    }
+#pragma unroll
+                    for (int sft = G / 2; sft > 0; sft >>= 1) ss += __shfl_xor_sync(gmask, ss, sft);
+                    const float inv = __frcp_rn(fmaxf(sqrtf(ss), 1e-12f));
+                    if (live[u]) {
+                        float f[N];
+#pragma unroll
+                        for (int e = 0; e < N; ++e) f[e] = acc[e] * inv;
+                        o[gl] = float_to_chunk<DT >= 0 ? DT : 0>(f);
+                    }
                 }
             }
         } else {
