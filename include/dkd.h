@@ -159,7 +159,7 @@ int dkd_extract_ex(dkd_ctx* ctx,
  *                refinement all use the product.
  *   valid_mask   device [B,H,W] u8: a pixel can be a keypoint only where the mask is non-zero ("a fisheye validity
  *                mask that culls features near the image periphery").  Masked pixels still take part
- *                in every window maximum and in the refinement windows.
+ *                in every window maximum and in the refinement windows.  (Read once per candidate, by the selection kernel.)
  *   nms_iters    0 = one (2r+1)^2 max-pool pass (north_star).  n > 0 = the iterated suppress-and-recover NMS of "the
  *                original PyTorch NMS" with n recovery rounds (the published procedure uses 2):
  *                M = (S == maxpool S); n times: supp = maxpool(M) > 0, S' = supp ? 0 : S, M |= (S' == maxpool S') & !supp,

@@ -201,15 +201,15 @@ cudaError_t plan_nms(dkd_ctx* ctx, const ExtractArgs& a, const NmsPlan& p, KLaun
         const bool negt = !(p.thr_up > 0.0f);                // a -0.0 score may be a candidate: fold it onto +0
 #define DKD_PREP_TMA(NEGT, PROD)                                                                                         \
     prep(k, k_nms_tma<R, NEGT, PROD>, dim3(grid), dim3(NMS_WARPS * 32), smem, false, tmap, tmap2, p, a.score, a.score2, \
-         a.mask, ctx->cand, ctx->tile_cnt)
+         ctx->cand, ctx->tile_cnt)
         if (prod) { if (negt) DKD_PREP_TMA(true, true); else DKD_PREP_TMA(false, true); }
         else { if (negt) DKD_PREP_TMA(true, false); else DKD_PREP_TMA(false, false); }
 #undef DKD_PREP_TMA
     } else {
         const int total = p.strips_x * p.chunks_y * a.B;
         const dim3 grid((total + PLAIN_WARPS - 1) / PLAIN_WARPS);
-        if (prod) prep(k, k_nms_plain<R, true>, grid, dim3(PLAIN_WARPS * 32), 0, false, a.score, a.score2, a.mask, p, total, ctx->cand, ctx->tile_cnt);
-        else prep(k, k_nms_plain<R, false>, grid, dim3(PLAIN_WARPS * 32), 0, false, a.score, a.score2, a.mask, p, total, ctx->cand, ctx->tile_cnt);
+        if (prod) prep(k, k_nms_plain<R, true>, grid, dim3(PLAIN_WARPS * 32), 0, false, a.score, a.score2, p, total, ctx->cand, ctx->tile_cnt);
+        else prep(k, k_nms_plain<R, false>, grid, dim3(PLAIN_WARPS * 32), 0, false, a.score, a.score2, p, total, ctx->cand, ctx->tile_cnt);
     }
     return cudaSuccess;
 }
@@ -303,13 +303,16 @@ cudaError_t build_plan(dkd_ctx* ctx, const ExtractArgs& a, Plan& pl) {
     int idx_shift = 0;                                       // (H*W - 1) >> idx_shift < NBT: index buckets of the top ties
     while (((static_cast<long long>(a.H) * a.W - 1) >> idx_shift) >= NBT) ++idx_shift;
     const bool pdl = ctx->use_pdl != 0;
-    SelPrefetch pf;
+    SelExtra pf;
     memset(&pf, 0, sizeof(pf));
+    pf.img_px = static_cast<size_t>(a.H) * a.W;
+    // variant V5: the single-pass NMS kernels leave the validity mask to the gather of k_select (one byte per candidate,
+    // read where the kernel is latency-bound anyway, instead of a dependent load inside the NMS emit loop)
+    if (a.nms_iters == 0) pf.vmask = a.mask;
     if (ctx->sel_prefetch) {
         const FastDiv dw = make_fastdiv(static_cast<uint32_t>(a.W));
         pf.score = a.score; pf.score2 = a.score2; pf.W = a.W; pf.r = a.r;
         pf.div_m = dw.m; pf.div_s1 = dw.s1; pf.div_s2 = dw.s2;
-        pf.img_px = static_cast<size_t>(a.H) * a.W;
     }
     prep(pl.k[1], k_select, dim3(a.B), dim3(SEL_THREADS), SEL_SMEM_BYTES, pdl, ctx->cand, ctx->tile_cnt, tpi,
          seg_cap, a.top_k, idx_shift, pf, sel, a.out_count, a.out_total);
@@ -602,7 +605,7 @@ int dkd_internal_select(dkd_ctx* ctx, const uint64_t* cand, const int* seg_cnt, 
                         int32_t* sel_idx, int32_t* out_count, cudaStream_t st) {
     int idx_shift = 0;
     while (((static_cast<long long>(n_items) - 1) >> idx_shift) >= NBT) ++idx_shift;
-    SelPrefetch pf;
+    SelExtra pf;
     memset(&pf, 0, sizeof(pf));
     KLaunch k;
     prep(k, k_select, dim3(1), dim3(SEL_THREADS), SEL_SMEM_BYTES, false, cand, seg_cnt, tpi, seg_cap, top_k, idx_shift, pf,

@@ -233,8 +233,8 @@ __device__ __forceinline__ void nms_rows(const float4 (&cat)[TH + 2 * R], float 
 template <int R, bool PROD>
 __device__ __forceinline__ int nms_emit(const unsigned (&neg)[4], unsigned colmask, int X, int yc, int H, int W,
                                         const float4 (&cat)[TH + 2 * R], const float* __restrict__ rows,
-                                        const float* __restrict__ rows2, const uint8_t* __restrict__ mask_img,
-                                        uint64_t* __restrict__ seg, int seg_room, uint64_t keep) {
+                                        const float* __restrict__ rows2, uint64_t* __restrict__ seg, int seg_room,
+                                        uint64_t keep) {
     constexpr unsigned FULL = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     unsigned rowmask = 0xffu;                                // bit TH-1-o = output row o is valid
@@ -258,9 +258,7 @@ __device__ __forceinline__ int nms_emit(const unsigned (&neg)[4], unsigned colma
             w &= w - 1u;
             const int k = bit >> 3, o = TH - 1 - (bit & 7);
             const int idx = (yc + o) * W + X + k;
-            // validity-mask variant: keypoints only where the mask is non-zero; masked pixels
-            // still take part in every window maximum (V5)
-            take = mask_img == nullptr || __ldg(mask_img + idx) != 0;
+            take = true;                                     // (the validity mask, variant V5, is applied by k_select's gather)
             float v;
             if (o >= R) {
                 DKD_ASSERT((o - R) * BOX_W + 4 * lane + k < BOX_W * TH);
@@ -357,7 +355,6 @@ __global__ void __launch_bounds__(NMS_WARPS * 32, PROD ? 1 : 2) k_nms_tma(const 
                                                                           const __grid_constant__ NmsPlan p,
                                                                           const float* __restrict__ score,
                                                                           const float* __restrict__ score2,
-                                                                          const uint8_t* __restrict__ mask,
                                                                           uint64_t* __restrict__ cand,
                                                                           int* __restrict__ seg_cnt) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -415,7 +412,6 @@ __global__ void __launch_bounds__(NMS_WARPS * 32, PROD ? 1 : 2) k_nms_tma(const 
         const int u = first + it * step;                     // the unit's candidate segment: p.cpu * SEG_CAP keys
         DKD_ASSERT(u >= 0 && u < p.units);
         uint64_t* useg = cand + static_cast<size_t>(u) * (p.cpu * SEG_CAP);
-        const uint8_t* mask_img = mask ? mask + cu.b * img_px : nullptr;
         int ucnt = 0;                                        // warp-uniform running count of the segment
         for (int c = 0; c < cu.nch; ++c) {
             const int s = consumed % NMS_STAGES;
@@ -433,7 +429,7 @@ __global__ void __launch_bounds__(NMS_WARPS * 32, PROD ? 1 : 2) k_nms_tma(const 
             }
             unsigned neg[4];
             nms_rows<R, NEGT>(cat, p.thr_up, neg);
-            ucnt += nms_emit<R, PROD>(neg, colmask, X, cu.y0 + TH * c, p.H, p.W, cat, rows, rows2, mask_img, useg + ucnt,
+            ucnt += nms_emit<R, PROD>(neg, colmask, X, cu.y0 + TH * c, p.H, p.W, cat, rows, rows2, useg + ucnt,
                                       p.cpu * SEG_CAP - ucnt, keep);
             __syncwarp();                                    // every lane is done with stage s
             issue_box();                                     // (the other NMS_STAGES-1 boxes stay in flight meanwhile)
@@ -452,7 +448,6 @@ constexpr int PLAIN_WARPS = 4;
 template <int R, bool PROD>
 __global__ void __launch_bounds__(PLAIN_WARPS * 32) k_nms_plain(const float* __restrict__ score,
                                                                 const float* __restrict__ score2,
-                                                                const uint8_t* __restrict__ mask,
                                                                 const __grid_constant__ NmsPlan p, int total,
                                                                 uint64_t* __restrict__ cand,
                                                                 int* __restrict__ seg_cnt) {
@@ -491,8 +486,7 @@ __global__ void __launch_bounds__(PLAIN_WARPS * 32) k_nms_plain(const float* __r
     unsigned neg[4];
     nms_rows<R, true>(cat, p.thr_up, neg);
     const int cnt = nms_emit<R, false>(neg, strip_colmask(X, p.W, R), X, y0, p.H, p.W, cat, boxes[warp], nullptr,
-                                       mask ? mask + b * img_px : nullptr, cand + static_cast<size_t>(t) * SEG_CAP, SEG_CAP,
-                                       l2_evict_last_policy());
+                                       cand + static_cast<size_t>(t) * SEG_CAP, SEG_CAP, l2_evict_last_policy());
     if (lane == 0) seg_cnt[t] = cnt;
 }
 
@@ -673,7 +667,8 @@ __device__ __forceinline__ int block_sum_1024(int v, int* s_red) {
 // The refinement that follows reads the (2r+1)^2 window of every kept keypoint: k_select, which knows the kept
 // indices first and has bandwidth to spare, asks L2 for those rows (first and last element of each window row:
 // one or two sectors), so that k_refine_gather's dependent window loads hit L2 instead of paying a DRAM round trip.
-struct SelPrefetch {
+struct SelExtra {
+    const uint8_t* vmask;               // validity mask [B,H,W] (variant V5) or NULL: keys on masked pixels are dropped in the gather
     const float* score;                 // NULL: no prefetch
     const float* score2;                // reliability map (product variant) or NULL
     int W, r;
@@ -681,7 +676,7 @@ struct SelPrefetch {
     size_t img_px;
 };
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
-__device__ __forceinline__ void prefetch_window(const SelPrefetch& pf, int b, int idx) {
+__device__ __forceinline__ void prefetch_window(const SelExtra& pf, int b, int idx) {
     if (pf.score == nullptr) return;
     const uint32_t t = __umulhi(pf.div_m, static_cast<uint32_t>(idx));
     const int y = static_cast<int>((t + ((static_cast<uint32_t>(idx) - t) >> pf.div_s1)) >> pf.div_s2), x = idx - y * pf.W;
@@ -701,7 +696,7 @@ __device__ __forceinline__ void prefetch_window(const SelPrefetch& pf, int b, in
 
 __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __restrict__ cand,
                                                            const int* __restrict__ seg_cnt, int tpi, int seg_cap,
-                                                           int top_k, int idx_shift, const SelPrefetch pf,
+                                                           int top_k, int idx_shift, const SelExtra pf,
                                                            int32_t* __restrict__ sel_idx,
                                                            int32_t* __restrict__ out_count,
                                                            int32_t* __restrict__ out_total) {
@@ -720,6 +715,7 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
     constexpr unsigned FULL = 0xffffffffu;
     const int b = blockIdx.x;
     const int* cnt = seg_cnt + static_cast<size_t>(b) * tpi;             // tpi segments of seg_cap keys per image
+    const uint8_t* vm = pf.vmask ? pf.vmask + b * pf.img_px : nullptr;
     const uint64_t* seg0 = cand + static_cast<size_t>(b) * tpi * seg_cap;
 
     pdl_launch_dependents();
@@ -747,7 +743,7 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
             const int total = __shfl_sync(FULL, incl, 31);
             if (total == 0) continue;                           // warp-uniform
             int gbase = 0;
-            if (lo == 0) {                                      // all keys are kept: reserve the slots at once
+            if (lo == 0 && vm == nullptr) {                     // all keys are kept: reserve the slots at once
                 if (lane == 0) gbase = atomicAdd(&s_n, total);
                 gbase = __shfl_sync(FULL, gbase, 0);
                 if (gbase + total > SORT_CAP) continue;         // too many candidates (rare): counted, radix select below
@@ -768,20 +764,26 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
                     kk[u] = 0ull;
                     if (e < total) kk[u] = seg0[static_cast<size_t>(t0 + tl) * seg_cap + (e - excl)];
                 }
+                if (vm != nullptr) {                            // variant V5: a key on a masked pixel is no candidate
+#pragma unroll
+                    for (int u = 0; u < GU; ++u)
+                        if (kk[u] != 0ull && __ldg(vm + key_index(kk[u])) == 0) kk[u] = 0ull;
+                }
 #pragma unroll
                 for (int u = 0; u < GU; ++u) {
                     const int e = e0 + 32 * u + lane;
                     uint64_t k = kk[u];
-                    if (lo == 0) {
+                    if (lo == 0 && vm == nullptr) {
                         if (e < total) { DKD_ASSERT(gbase + e >= 0 && gbase + e < SORT_CAP); keys[gbase + e] = k; }
                     } else {
-                        const bool take = (e < total) && (k >= lo);
+                        const bool take = (e < total) && k != 0ull && (k >= lo);
                         const unsigned bal = __ballot_sync(FULL, take);
                         if (bal) {
                             int pb = 0;
                             if (lane == 0) pb = atomicAdd(&s_n, __popc(bal));
                             pb = __shfl_sync(FULL, pb, 0);
-                            if (take) { DKD_ASSERT(pb + __popc(bal & ((1u << lane) - 1u)) < SORT_CAP); keys[pb + __popc(bal & ((1u << lane) - 1u))] = k; }
+                            // (first pass with a mask: the count may pass SORT_CAP -> counted, not stored, radix select below)
+                            if (take && pb + __popc(bal) <= SORT_CAP) keys[pb + __popc(bal & ((1u << lane) - 1u))] = k;
                         }
                         if (!take) k = 0ull;
                     }
@@ -814,7 +816,8 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
                         int digit = 256;                        // dummy bin: past the end / outside the prefix
                         if (e < c) {
                             const uint64_t k = seg[e];
-                            const bool match = (shift == 56) || ((k >> (shift + 8)) == (prefix >> (shift + 8)));
+                            bool match = (shift == 56) || ((k >> (shift + 8)) == (prefix >> (shift + 8)));
+                            if (match && vm != nullptr) match = __ldg(vm + key_index(k)) != 0;
                             if (match) digit = static_cast<int>((k >> shift) & 255u);
                         }
                         const unsigned peers = __match_any_sync(FULL, digit);
