@@ -143,12 +143,14 @@ cudaError_t setup_nms(dkd_ctx* ctx) {
     cudaError_t e;
     if ((e = cudaFuncSetAttribute(k_nms_tma<R, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, NMS_SMEM_BYTES)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(k_nms_tma<R, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, NMS_SMEM_BYTES)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(k_nms_tma<R, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * NMS_SMEM_BYTES)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(k_nms_tma<R, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * NMS_SMEM_BYTES)) != cudaSuccess) return e;
     int n = 0;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_nms_tma<R, true, false>, NMS_WARPS * 32, NMS_SMEM_BYTES);
-    ctx->nms_ctas_per_sm[R] = n > 0 ? n : 1;
+    ctx->nms_ctas_per_sm[R] = n > 0 ? (n < NMS_CTAS ? n : NMS_CTAS) : 1;
     if (e != cudaSuccess) return e;
+    ctx->nms_ctas_per_sm_prod[R] = 1;
+    if (2 * NMS_SMEM_BYTES > 227 * 1024) return e;          // (tuning builds with a deeper ring: no product variant)
+    if ((e = cudaFuncSetAttribute(k_nms_tma<R, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * NMS_SMEM_BYTES)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_nms_tma<R, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * NMS_SMEM_BYTES)) != cudaSuccess) return e;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_nms_tma<R, true, true>, NMS_WARPS * 32, 2 * NMS_SMEM_BYTES);
     ctx->nms_ctas_per_sm_prod[R] = n > 0 ? n : 1;
     return e;
@@ -163,7 +165,7 @@ NmsPlan nms_plan(const dkd_ctx* ctx, const ExtractArgs& a) {   // (a.use_tma == 
     p.chunks_y = (a.H + TH - 1) / TH;
     // S > thresh  <=>  S >= nextafter(thresh, +inf): the threshold joins the window maximum (dkd_kernels.cuh)
     p.thr_up = nextafterf(a.thresh, INFINITY);
-    const long long slots = 2LL * ctx->num_sms * NMS_WARPS;  // resident warps
+    const long long slots = static_cast<long long>(NMS_CTAS) * ctx->num_sms * NMS_WARPS;  // resident warps
     int best = 1;
     for (int cpu = MAX_CPU; cpu >= 1; --cpu) {
         const int segs = (p.chunks_y + cpu - 1) / cpu;

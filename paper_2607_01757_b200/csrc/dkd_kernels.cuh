@@ -49,8 +49,19 @@ constexpr int RG_THREADS = 256;          // k_refine_gather: 8 warps, 8..32 keyp
 constexpr int BOX_BYTES = BOX_W * TH * 4;                                                // 4 KB
 // Every resident warp keeps NMS_STAGES-1 boxes in flight while it works on one: bytes in flight per
 // SM >= 2 CTAs x warps x (stages-1) x 4 KB = 128 KB (HBM latency x bandwidth needs ~50 KB per SM).
-constexpr int NMS_WARPS = 8;             // per CTA, 2 CTAs/SM: 16 warps x <= 128 registers
-constexpr int NMS_STAGES = 3;
+// (-DDKD_NMS_WARPS / _STAGES / _CTAS: tuning builds only — DESIGN.md 7.5 quotes what 8 and 12 warps per SM cost)
+#ifndef DKD_NMS_WARPS
+#define DKD_NMS_WARPS 8
+#endif
+#ifndef DKD_NMS_STAGES
+#define DKD_NMS_STAGES 3
+#endif
+#ifndef DKD_NMS_CTAS
+#define DKD_NMS_CTAS 2
+#endif
+constexpr int NMS_WARPS = DKD_NMS_WARPS;  // per CTA, 2 CTAs/SM: 16 warps x <= 128 registers
+constexpr int NMS_STAGES = DKD_NMS_STAGES;
+constexpr int NMS_CTAS = DKD_NMS_CTAS;    // CTAs per SM the kernel is compiled and launched for
 constexpr int NMS_SMEM_BYTES = NMS_WARPS * NMS_STAGES * BOX_BYTES;                        // 96 KB per CTA
 
 // ---- 64-bit selection key ---------------------------------------------------------------------
@@ -350,7 +361,7 @@ __device__ __forceinline__ void load_head(float4 (&cat)[TH + 2 * R], const float
 // No CTA-wide barrier after set-up: a warp only ever waits for its own boxes.  Dynamic smem:
 // NMS_SMEM_BYTES, 128-byte aligned; warp w owns NMS_STAGES boxes.  NEGT: thr_up <= 0 (see nms_rows).
 template <int R, bool NEGT, bool PROD>
-__global__ void __launch_bounds__(NMS_WARPS * 32, PROD ? 1 : 2) k_nms_tma(const __grid_constant__ CUtensorMap tmap,
+__global__ void __launch_bounds__(NMS_WARPS * 32, PROD ? 1 : NMS_CTAS) k_nms_tma(const __grid_constant__ CUtensorMap tmap,
                                                                           const __grid_constant__ CUtensorMap tmap2,
                                                                           const __grid_constant__ NmsPlan p,
                                                                           const float* __restrict__ score,
