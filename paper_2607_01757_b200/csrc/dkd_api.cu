@@ -605,6 +605,7 @@ void* dkd_ctx_scratch(dkd_ctx* ctx, int slot, size_t bytes) {
 }
 int dkd_internal_select(dkd_ctx* ctx, const uint64_t* cand, const int* seg_cnt, int tpi, int seg_cap, int top_k, int n_items,
                         int32_t* sel_idx, int32_t* out_count, cudaStream_t st) {
+    if ((seg_cap & 1) || misaligned(cand, 16)) return fail(ctx, DKD_ERR_INVALID_ARG, "internal: candidate segments must be 16-byte aligned");
     int idx_shift = 0;
     while (((static_cast<long long>(n_items) - 1) >> idx_shift) >= NBT) ++idx_shift;
     SelExtra pf;

@@ -705,6 +705,77 @@ __device__ __forceinline__ void prefetch_window(const SelExtra& pf, int b, int i
     }
 }
 
+// MSB-first 8-bit radix select over the candidate segments of one image (only when more than SORT_CAP keys were found):
+// returns a prefix `lo` with top_k <= #{key >= lo} <= SORT_CAP.  Kept OUT OF LINE: k_select runs once per launch with
+// cold instruction caches, so its common path must not jump across kilobytes of code it never executes.
+__device__ __noinline__ uint64_t select_radix_prefix(const uint64_t* __restrict__ seg0, const int* __restrict__ cnt, int tpi,
+                                                     int seg_cap, const uint8_t* __restrict__ vm, int top_k, int* s_hist,
+                                                     int* s_rdx) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int NW = SEL_THREADS / 32;
+    constexpr unsigned FULL = 0xffffffffu;
+    int& s_digit = s_rdx[0];
+    int& s_cum = s_rdx[1];
+    int& s_h = s_rdx[2];
+    uint64_t prefix = 0;
+    int need = top_k;                                   // rank (1-based, from the top) inside the prefix bucket
+    int above = 0;                                      // keys strictly above the prefix bucket
+    for (int shift = 56; shift >= 0; shift -= 8) {
+        for (int i = tid; i < 257; i += SEL_THREADS) s_hist[i] = 0;
+        __syncthreads();
+        for (int t = warp; t < tpi; t += NW) {
+            const int c = cnt[t];
+            const uint64_t* seg = seg0 + static_cast<size_t>(t) * seg_cap;
+            for (int e0 = 0; e0 < c; e0 += 32) {
+                const int e = e0 + lane;
+                int digit = 256;                        // dummy bin: past the end / outside the prefix
+                if (e < c) {
+                    const uint64_t k = seg[e];
+                    bool match = (shift == 56) || ((k >> (shift + 8)) == (prefix >> (shift + 8)));
+                    if (match && vm != nullptr) match = __ldg(vm + key_index(k)) != 0;
+                    if (match) digit = static_cast<int>((k >> shift) & 255u);
+                }
+                const unsigned peers = __match_any_sync(FULL, digit);
+                if (lane == __ffs(peers) - 1) atomicAdd(&s_hist[digit], __popc(peers));
+            }
+        }
+        __syncthreads();
+        if (warp == 0) {                                // find the digit holding the need-th largest key
+            int grp = 0;                                // lane l owns bins 255-8l .. 248-8l (descending)
+#pragma unroll
+            for (int q = 0; q < 8; ++q) grp += s_hist[255 - 8 * lane - q];
+            int incl = grp;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int up = __shfl_up_sync(FULL, incl, o);
+                if (lane >= o) incl += up;
+            }
+            const unsigned hit = __ballot_sync(FULL, incl >= need);
+            const int owner = __ffs(hit) - 1;           // exists: need <= keys in the bucket
+            if (lane == owner) {
+                int cum = incl - grp;
+                int d = 255 - 8 * lane;
+                for (int q = 0; q < 8; ++q, --d) {
+                    const int h = s_hist[d];
+                    if (cum + h >= need) break;
+                    cum += h;
+                }
+                s_digit = d;
+                s_cum = cum;
+                s_h = s_hist[d];
+            }
+        }
+        __syncthreads();
+        prefix |= static_cast<uint64_t>(s_digit) << shift;
+        above += s_cum;
+        need -= s_cum;
+        const bool done = (above + s_h <= SORT_CAP);
+        __syncthreads();
+        if (done) break;
+    }
+    return prefix;
+}
+
 __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __restrict__ cand,
                                                            const int* __restrict__ seg_cnt, int tpi, int seg_cap,
                                                            int top_k, int idx_shift, const SelExtra pf,
@@ -718,7 +789,7 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
     int* cur = base + NBK;                                             // NBK
     __shared__ int s_hist[257];
     __shared__ int s_red[32];
-    __shared__ int s_n, s_digit, s_cum, s_h, s_maxb;
+    __shared__ int s_n, s_maxb, s_meff, s_rdx[3];
     __shared__ unsigned s_hi, s_lo;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -732,20 +803,26 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
     pdl_launch_dependents();
     if (tid == 0) { s_n = 0; s_hi = 0u; s_lo = 0xffffffffu; s_maxb = 0; }
     for (int i = tid; i < NBK; i += SEL_THREADS) cur[i] = 0;
+
+    // Gather layout: LPS = 1, 2, 4 or 8 lanes share one segment (lane sub of a segment copies its items sub, sub + LPS,
+    // ...), so a warp iteration covers 32 / LPS segments: an item's position in the concatenation is its segment's
+    // exclusive offset (one warp scan of the counts) plus its index — no search.  LPS grows with the unit length (longer
+    // units hold more keys per segment) as long as one pass of the CTA still covers about all the segments.
+    int lps_log = 0;
+    while (lps_log < 3 && (SEG_CAP << lps_log) < seg_cap && (tpi << (lps_log + 1)) <= SEL_THREADS) ++lps_log;
+    const int lps = 1 << lps_log, spw = 32 >> lps_log;      // lanes per segment, segments per warp iteration
+    const int sub = lane & (lps - 1), sl = lane >> lps_log;
+    uint64_t lo = 0;                                        // gather keys >= lo (0: all of them)
     pdl_wait();                                              // the candidates of k_nms_* are complete and visible
     __syncthreads();
-
-    // segments per warp iteration: all 32 warps busy with as few dependent rounds as possible
-    const int gt = tpi >= 32 * NW ? 32 : (tpi + NW - 1) / NW;
-    uint64_t lo = 0;                                        // gather keys >= lo (0: all of them)
     for (int pass = 0; pass < 2; ++pass) {                  // second pass only if the first found n > SORT_CAP
-        // ---- gather: gt <= 32 segments per warp iteration; lane l reads segment l's count, the warp copies
-        // the concatenation of the segments with every lane busy (a 5-step search finds an item's segment)
         unsigned khi = 0u, klo = 0xffffffffu;                   // range of the gathered score words
-        for (int t0 = warp * gt; t0 < tpi; t0 += NW * gt) {
-            const int t = t0 + lane;
-            const int c = (lane < gt && t < tpi) ? cnt[t] : 0;
-            int incl = c;
+        int c_next = (warp * spw + sl < tpi) ? cnt[warp * spw + sl] : 0;
+        for (int t0 = warp * spw; t0 < tpi; t0 += NW * spw) {
+            const int t = t0 + sl;
+            const int c = c_next;                               // (the next iteration's counts are already on their way)
+            c_next = (t + NW * spw < tpi) ? cnt[t + NW * spw] : 0;
+            int incl = sub == 0 ? c : 0;
     #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
                 const int up = __shfl_up_sync(FULL, incl, o);
@@ -753,41 +830,43 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
             }
             const int total = __shfl_sync(FULL, incl, 31);
             if (total == 0) continue;                           // warp-uniform
+            const int excl = incl - c;                          // items of the warp's earlier segments
             int gbase = 0;
             if (lo == 0 && vm == nullptr) {                     // all keys are kept: reserve the slots at once
                 if (lane == 0) gbase = atomicAdd(&s_n, total);
                 gbase = __shfl_sync(FULL, gbase, 0);
                 if (gbase + total > SORT_CAP) continue;         // too many candidates (rare): counted, radix select below
             }
-            constexpr int GU = 4;                               // loads in flight per lane
-            for (int e0 = 0; e0 < total; e0 += 32 * GU) {
-                uint64_t kk[GU];
+            // One SM turns around roughly one scattered load request every 4 cycles, and with a few keys in each of
+            // hundreds of segments every request counts: a lane fetches its keys as 16-byte PAIRS (2q, 2q+1) — the
+            // segments are 32-byte aligned — and the LPS lanes of a segment read consecutive pairs (one sector per two lanes).
+            constexpr int GU = 4;                               // pair loads in flight per lane
+            const ulonglong2* seg = reinterpret_cast<const ulonglong2*>(seg0 + static_cast<size_t>(t < tpi ? t : 0) * seg_cap);
+            const int cmax = __reduce_max_sync(FULL, c);
+            for (int i0 = 0; i0 < cmax; i0 += 2 * lps * GU) {
+                uint64_t kk[2 * GU];
 #pragma unroll
-                for (int u = 0; u < GU; ++u) {                  // (warp-uniform trip count: shuffles inside)
-                    const int e = e0 + 32 * u + lane;
-                    int tl = 0;                                 // first lane whose inclusive count exceeds e
-#pragma unroll
-                    for (int step = 16; step > 0; step >>= 1) {
-                        const int v = __shfl_sync(FULL, incl, tl + step - 1);
-                        if (v <= e) tl += step;
-                    }
-                    const int excl = __shfl_sync(FULL, incl - c, tl);
-                    kk[u] = 0ull;
-                    if (e < total) kk[u] = seg0[static_cast<size_t>(t0 + tl) * seg_cap + (e - excl)];
+                for (int u = 0; u < GU; ++u) {
+                    const int i = i0 + 2 * (sub + (u << lps_log));  // first key of the pair
+                    DKD_ASSERT(i >= c || i + 1 < seg_cap);
+                    ulonglong2 q = make_ulonglong2(0ull, 0ull);
+                    if (i < c) q = __ldg(seg + (i >> 1));
+                    kk[2 * u] = q.x;
+                    kk[2 * u + 1] = i + 1 < c ? q.y : 0ull;
                 }
                 if (vm != nullptr) {                            // variant V5: a key on a masked pixel is no candidate
 #pragma unroll
-                    for (int u = 0; u < GU; ++u)
+                    for (int u = 0; u < 2 * GU; ++u)
                         if (kk[u] != 0ull && __ldg(vm + key_index(kk[u])) == 0) kk[u] = 0ull;
                 }
 #pragma unroll
-                for (int u = 0; u < GU; ++u) {
-                    const int e = e0 + 32 * u + lane;
+                for (int u = 0; u < 2 * GU; ++u) {
+                    const int i = i0 + 2 * (sub + ((u >> 1) << lps_log)) + (u & 1);
                     uint64_t k = kk[u];
                     if (lo == 0 && vm == nullptr) {
-                        if (e < total) { DKD_ASSERT(gbase + e >= 0 && gbase + e < SORT_CAP); keys[gbase + e] = k; }
+                        if (i < c) { DKD_ASSERT(gbase + excl + i >= 0 && gbase + excl + i < SORT_CAP); keys[gbase + excl + i] = k; }
                     } else {
-                        const bool take = (e < total) && k != 0ull && (k >= lo);
+                        const bool take = (i < c) && k != 0ull && (k >= lo);
                         const unsigned bal = __ballot_sync(FULL, take);
                         if (bal) {
                             int pb = 0;
@@ -812,65 +891,8 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
         __syncthreads();
         if (pass == 0 && tid == 0 && out_total != nullptr) out_total[b] = s_n;   // C_b: every candidate, before the cap
         if (s_n <= SORT_CAP) break;                         // block-uniform; always true in the second pass
-        {
-            uint64_t prefix = 0;
-            int need = top_k;                                   // rank (1-based, from the top) inside the prefix bucket
-            int above = 0;                                      // keys strictly above the prefix bucket
-            for (int shift = 56; shift >= 0; shift -= 8) {
-                for (int i = tid; i < 257; i += SEL_THREADS) s_hist[i] = 0;
-                __syncthreads();
-                for (int t = warp; t < tpi; t += NW) {
-                    const int c = cnt[t];
-                    const uint64_t* seg = seg0 + static_cast<size_t>(t) * seg_cap;
-                    for (int e0 = 0; e0 < c; e0 += 32) {
-                        const int e = e0 + lane;
-                        int digit = 256;                        // dummy bin: past the end / outside the prefix
-                        if (e < c) {
-                            const uint64_t k = seg[e];
-                            bool match = (shift == 56) || ((k >> (shift + 8)) == (prefix >> (shift + 8)));
-                            if (match && vm != nullptr) match = __ldg(vm + key_index(k)) != 0;
-                            if (match) digit = static_cast<int>((k >> shift) & 255u);
-                        }
-                        const unsigned peers = __match_any_sync(FULL, digit);
-                        if (lane == __ffs(peers) - 1) atomicAdd(&s_hist[digit], __popc(peers));
-                    }
-                }
-                __syncthreads();
-                if (warp == 0) {                                // find the digit holding the need-th largest key
-                    int grp = 0;                                // lane l owns bins 255-8l .. 248-8l (descending)
-    #pragma unroll
-                    for (int q = 0; q < 8; ++q) grp += s_hist[255 - 8 * lane - q];
-                    int incl = grp;
-    #pragma unroll
-                    for (int o = 1; o < 32; o <<= 1) {
-                        const int up = __shfl_up_sync(FULL, incl, o);
-                        if (lane >= o) incl += up;
-                    }
-                    const unsigned hit = __ballot_sync(FULL, incl >= need);
-                    const int owner = __ffs(hit) - 1;           // exists: need <= keys in the bucket
-                    if (lane == owner) {
-                        int cum = incl - grp;
-                        int d = 255 - 8 * lane;
-                        for (int q = 0; q < 8; ++q, --d) {
-                            const int h = s_hist[d];
-                            if (cum + h >= need) break;
-                            cum += h;
-                        }
-                        s_digit = d;
-                        s_cum = cum;
-                        s_h = s_hist[d];
-                    }
-                }
-                __syncthreads();
-                prefix |= static_cast<uint64_t>(s_digit) << shift;
-                above += s_cum;
-                need -= s_cum;
-                const bool done = (above + s_h <= SORT_CAP);
-                __syncthreads();
-                if (done) break;
-            }
-            lo = prefix;
-        }
+        lo = select_radix_prefix(seg0, cnt, tpi, seg_cap, vm, top_k, s_hist, s_rdx);   // (out of line: rare, and the common
+                                                            // path stays one contiguous run of instructions)
         if (tid == 0) { s_n = 0; s_hi = 0u; s_lo = 0xffffffffu; }
         __syncthreads();
     }
@@ -892,6 +914,7 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
         const unsigned kb = static_cast<unsigned>(k >> 32);
         return kb == hi ? key_index(k) >> idx_shift : NBT + static_cast<int>((hi - kb) >> shift);
     };
+    if (tid == 0) s_meff = m;
     for (int i = tid; i < m; i += SEL_THREADS) {
         DKD_ASSERT(bucket_of(keys[i]) >= 0 && bucket_of(keys[i]) < NBK);
         atomicAdd(&cur[bucket_of(keys[i])], 1);
@@ -899,12 +922,11 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
     __syncthreads();
     {   // exclusive scan of the NBK bucket counts (5 consecutive buckets per thread), largest bucket
         int c4[NBK / SEL_THREADS];
-        int sum = 0, mx = 0;
+        int sum = 0;
 #pragma unroll
         for (int q = 0; q < NBK / SEL_THREADS; ++q) {
             c4[q] = cur[tid * (NBK / SEL_THREADS) + q];
             sum += c4[q];
-            mx = c4[q] > mx ? c4[q] : mx;
         }
         int incl = sum;
 #pragma unroll
@@ -912,9 +934,7 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
             const int up = __shfl_up_sync(FULL, incl, o);
             if (lane >= o) incl += up;
         }
-        mx = __reduce_max_sync(FULL, mx);
         if (lane == 31) s_red[warp] = incl;
-        if (lane == 0) atomicMax(&s_maxb, mx);
         __syncthreads();
         int woff = s_red[lane];                             // 32 warp totals -> exclusive offsets
         int wincl = woff;
@@ -925,25 +945,37 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
         }
         woff = __shfl_sync(FULL, wincl - woff, warp);
         int run = woff + incl - sum;
+        // Only the buckets that start before rank K can hold a kept key: the keys of the others are neither scattered
+        // nor ranked (m_eff = end of the bucket that contains rank K-1), and only the kept buckets count for the size limit.
+        int mx = 0;
 #pragma unroll
         for (int q = 0; q < NBK / SEL_THREADS; ++q) {
             base[tid * (NBK / SEL_THREADS) + q] = run;
             cur[tid * (NBK / SEL_THREADS) + q] = 0;
+            if (run < K) {
+                mx = c4[q] > mx ? c4[q] : mx;
+                if (run + c4[q] >= K) s_meff = run + c4[q];  // (exactly one bucket when m >= K)
+            }
             run += c4[q];
         }
+        mx = __reduce_max_sync(FULL, mx);
+        if (lane == 0 && mx > 0) atomicMax(&s_maxb, mx);
         __syncthreads();
     }
+    const int m_eff = s_meff;                               // keys in the kept buckets (<= m)
+    DKD_ASSERT(m_eff >= K && m_eff <= m);
     if (s_maxb <= BUCKET_LIMIT) {                           // block-uniform
         for (int i = tid; i < m; i += SEL_THREADS) {        // scatter into bucket order
             const uint64_t k = keys[i];
             const int d = bucket_of(k);
             DKD_ASSERT(d >= 0 && d < NBK);
+            if (base[d] >= K) continue;                      // every key of this bucket ranks past K
             const int pos = base[d] + atomicAdd(&cur[d], 1);
-            DKD_ASSERT(pos >= 0 && pos < m && pos < SORT_CAP);
+            DKD_ASSERT(pos >= 0 && pos < m_eff && pos < SORT_CAP);
             sorted[pos] = k;
         }
         __syncthreads();
-        for (int i = tid; i < m; i += SEL_THREADS) {        // exact rank inside the own bucket
+        for (int i = tid; i < m_eff; i += SEL_THREADS) {    // exact rank inside the own bucket
             const uint64_t k = sorted[i];
             const int d = bucket_of(k);
             const int s0 = base[d], s1 = s0 + cur[d];
