@@ -114,6 +114,10 @@ struct dkd_ctx {
     cudaEvent_t prof_ev[MAX_KERNELS + 1];                   // measurement mode: event before/after every kernel
     int prof_n;                                             // kernels of the last profiled call (0: none)
     std::vector<GraphEntry> graphs;
+    Plan last_plan;                                         // plain-launch path: the most recent plan and what it was built for
+    ShapeKey last_plan_key;
+    ExtractArgs last_plan_args;
+    bool have_last_plan;
     cudaStream_t cap_stream;  // capture-only stream for building the cached graphs
     unsigned long long tick;
     unsigned long long n_instantiated, n_updated, n_replayed, n_stream;   // graph-cache statistics (dkd_graph_stats)
@@ -192,6 +196,7 @@ bool encode_map(dkd_ctx* ctx, CUtensorMap* tmap, const float* base, const Extrac
 template <int R>
 cudaError_t plan_nms(dkd_ctx* ctx, const ExtractArgs& a, const NmsPlan& p, KLaunch& k) {
     const bool prod = a.score2 != nullptr;
+    const bool pdl = ctx->use_pdl != 0;                      // (the kernel waits for its predecessor before touching memory)
     if (a.use_tma) {
         CUtensorMap tmap, tmap2;
         if (!encode_map(ctx, &tmap, a.score, a)) return cudaErrorInvalidValue;
@@ -202,7 +207,7 @@ cudaError_t plan_nms(dkd_ctx* ctx, const ExtractArgs& a, const NmsPlan& p, KLaun
         const size_t smem = prod ? 2 * NMS_SMEM_BYTES : NMS_SMEM_BYTES;
         const bool negt = !(p.thr_up > 0.0f);                // a -0.0 score may be a candidate: fold it onto +0
 #define DKD_PREP_TMA(NEGT, PROD)                                                                                         \
-    prep(k, k_nms_tma<R, NEGT, PROD>, dim3(grid), dim3(NMS_WARPS * 32), smem, false, tmap, tmap2, p, a.score, a.score2, \
+    prep(k, k_nms_tma<R, NEGT, PROD>, dim3(grid), dim3(NMS_WARPS * 32), smem, pdl, tmap, tmap2, p, a.score, a.score2, \
          ctx->cand, ctx->tile_cnt)
         if (prod) { if (negt) DKD_PREP_TMA(true, true); else DKD_PREP_TMA(false, true); }
         else { if (negt) DKD_PREP_TMA(true, false); else DKD_PREP_TMA(false, false); }
@@ -210,8 +215,8 @@ cudaError_t plan_nms(dkd_ctx* ctx, const ExtractArgs& a, const NmsPlan& p, KLaun
     } else {
         const int total = p.strips_x * p.chunks_y * a.B;
         const dim3 grid((total + PLAIN_WARPS - 1) / PLAIN_WARPS);
-        if (prod) prep(k, k_nms_plain<R, true>, grid, dim3(PLAIN_WARPS * 32), 0, false, a.score, a.score2, p, total, ctx->cand, ctx->tile_cnt);
-        else prep(k, k_nms_plain<R, false>, grid, dim3(PLAIN_WARPS * 32), 0, false, a.score, a.score2, p, total, ctx->cand, ctx->tile_cnt);
+        if (prod) prep(k, k_nms_plain<R, true>, grid, dim3(PLAIN_WARPS * 32), 0, pdl, a.score, a.score2, p, total, ctx->cand, ctx->tile_cnt);
+        else prep(k, k_nms_plain<R, false>, grid, dim3(PLAIN_WARPS * 32), 0, pdl, a.score, a.score2, p, total, ctx->cand, ctx->tile_cnt);
     }
     return cudaSuccess;
 }
@@ -251,7 +256,7 @@ void plan_rg_dt(const RGParams& p, int B, bool prod, bool pdl, KLaunch& k) {
     else plan_rg_g<DT, 32>(p, B, prod, pdl, k);
 }
 
-void plan_rg(const ExtractArgs& a, const int32_t* sel, bool pdl, KLaunch& k) {
+void plan_rg(const ExtractArgs& a, const int32_t* sel, bool pdl, int num_sms, KLaunch& k) {
     RGParams p;
     memset(&p, 0, sizeof(p));
     p.score = a.score; p.score2 = a.score2; p.H = a.H; p.W = a.W;
@@ -262,6 +267,7 @@ void plan_rg(const ExtractArgs& a, const int32_t* sel, bool pdl, KLaunch& k) {
     p.origin_x = a.origin_x; p.origin_y = a.origin_y;
     p.score_mode = a.score_mode;
     p.vec_window = (a.W % 4 == 0) && !misaligned(a.score, 16) && a.score2 == nullptr;
+    p.early_trigger = pdl && static_cast<long long>((a.top_k + RG_SLOTS - 1) / RG_SLOTS) * a.B <= 4LL * num_sms;
     const bool prod = a.score2 != nullptr;
     if (a.desc == nullptr) { plan_rg_g<-1, 8>(p, a.B, prod, pdl, k); return; }
     const size_t esz = a.desc_dtype == DKD_F16 ? 2 : 4;
@@ -289,7 +295,7 @@ cudaError_t build_plan(dkd_ctx* ctx, const ExtractArgs& a, Plan& pl) {
         ip.T = (IT_REG - 2 * ip.halo) & ~7;
         ip.tiles_x = (a.W + ip.T - 1) / ip.T; ip.tiles_y = (a.H + ip.T - 1) / ip.T;
         ip.thresh = a.thresh; ip.cand = ctx->cand; ip.seg_cnt = ctx->tile_cnt;
-        prep(pl.k[0], k_nms_iter, dim3(ip.tiles_x * ip.tiles_y, a.B), dim3(IT_THREADS), IT_SMEM_BYTES, false, ip);
+        prep(pl.k[0], k_nms_iter, dim3(ip.tiles_x * ip.tiles_y, a.B), dim3(IT_THREADS), IT_SMEM_BYTES, ctx->use_pdl != 0, ip);
         tpi = ip.tiles_x * ip.tiles_y;
         seg_cap = ip.T * ip.T;
     } else {
@@ -318,7 +324,7 @@ cudaError_t build_plan(dkd_ctx* ctx, const ExtractArgs& a, Plan& pl) {
     }
     prep(pl.k[1], k_select, dim3(a.B), dim3(SEL_THREADS), SEL_SMEM_BYTES, pdl, ctx->cand, ctx->tile_cnt, tpi,
          seg_cap, a.top_k, idx_shift, pf, sel, a.out_count, a.out_total);
-    plan_rg(a, sel, pdl, pl.k[2]);
+    plan_rg(a, sel, pdl, ctx->num_sms, pl.k[2]);
     pl.n = 3;
     return cudaSuccess;
 }
@@ -424,7 +430,7 @@ int build_graph(dkd_ctx* ctx, const Plan& pl, GraphEntry& ge) {
     cudaError_t e = cudaSuccess;
     ge.n_nodes = pl.n;
     for (int i = 0; i < pl.n; ++i) {
-        e = launch(pl.k[i], ctx->cap_stream, true);
+        e = launch(pl.k[i], ctx->cap_stream, i > 0);         // (the first node has no predecessor inside the graph)
         if (e != cudaSuccess) break;
         cudaStreamCaptureStatus cs;
         const cudaGraphNode_t* deps = nullptr;
@@ -488,8 +494,17 @@ int run(dkd_ctx* ctx, ExtractArgs a, cudaStream_t st) {
         return DKD_OK;
     }
     if (!ctx->use_graph || cap != cudaStreamCaptureStatusNone) {
-        CK(ctx, build_plan(ctx, a, pl));
-        CK(ctx, enqueue(ctx, pl, st));
+        // plain launches: the plan of the previous call is kept (a repeated call with the same arguments skips the
+        // tensor-map encoding and the rest of build_plan)
+        const ShapeKey key = shape_key(ctx, a);
+        if (!(ctx->have_last_plan && ctx->last_plan_key == key && same_values(ctx->last_plan_args, a))) {
+            ctx->have_last_plan = false;
+            CK(ctx, build_plan(ctx, a, ctx->last_plan));
+            ctx->last_plan_key = key;
+            ctx->last_plan_args = a;
+            ctx->have_last_plan = true;
+        }
+        CK(ctx, enqueue(ctx, ctx->last_plan, st));
         ++ctx->n_stream;
         return DKD_OK;
     }
@@ -653,6 +668,7 @@ int dkd_create(const dkd_create_params* p, dkd_ctx** out) {
     ctx->origin_x = ctx->origin_y = 0;
     ctx->err[0] = 0;
     ctx->tick = 0;
+    ctx->have_last_plan = false;
 #define CKC(call)                                                                                        \
     do {                                                                                                 \
         cudaError_t e_ = (call);                                                                         \

@@ -410,6 +410,10 @@ __global__ void __launch_bounds__(NMS_WARPS * 32, PROD ? 1 : NMS_CTAS) k_nms_tma
         fence_mbar_init();
     }
     __syncwarp();
+    // Launched with the programmatic attribute, this grid may have started while the previous kernel of the stream (the
+    // previous call's k_refine_gather, or whatever produced the score map) was still running: everything above is
+    // set-up; nothing is read from or written to global memory before the predecessor has completed.
+    pdl_wait();
 #pragma unroll
     for (int s = 0; s < NMS_STAGES; ++s) issue_box();
 
@@ -467,6 +471,7 @@ __global__ void __launch_bounds__(PLAIN_WARPS * 32) k_nms_plain(const float* __r
     const int t = blockIdx.x * PLAIN_WARPS + warp;          // unit == strip-tile (nms_plan: cpu = 1 on this path)
     pdl_launch_dependents();
     if (t >= total) return;
+    pdl_wait();                                              // (see k_nms_tma)
     const int tpi = p.strips_x * p.chunks_y;
     const int b = t / tpi, rem = t - b * tpi;
     const int cy = rem / p.strips_x, x0 = (rem - cy * p.strips_x) * STRIP_W, y0 = cy * TH;
@@ -539,6 +544,7 @@ __global__ void __launch_bounds__(IT_THREADS, 1) k_nms_iter(const __grid_constan
     const float* img2 = p.score2 ? p.score2 + b * img_px : nullptr;
     const int r = p.r;
     pdl_launch_dependents();
+    pdl_wait();                                              // (see k_nms_tma)
     for (int i = tid; i < NPX; i += IT_THREADS) {
         const int ry = i / IT_REG, rx = i - ry * IT_REG, gy = y0 + ry, gx = x0 + rx;
         float v = -INFINITY;
@@ -1144,6 +1150,7 @@ struct RGParams {
     int origin_x, origin_y;             // letterbox offset subtracted from the stored coordinates
     int score_mode;                     // DKD_SCORE_RAW: S at the integer peak; DKD_SCORE_BILINEAR: S at the refined point
     int vec_window;                     // W % 4 == 0 and a 16-byte aligned map: window rows as aligned 16-byte chunks
+    int early_trigger;                  // the grid fits the machine at once: let the stream's next kernel launch early
 };
 
 // score value at one pixel: S, or heat x reliability rounded once to fp32 (the product variant)
@@ -1259,6 +1266,10 @@ __global__ void __launch_bounds__(RG_THREADS, 4) k_refine_gather(const __grid_co
     const int b = blockIdx.y;
     const int slot0 = blockIdx.x * RG_SLOTS;                 // first slot (within the image) of this CTA
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // The next call's NMS kernel may be launched while this grid runs (it waits for this grid's completion before it
+    // touches memory) — but only when every CTA of this grid is resident at once: waiting CTAs of the successor must
+    // not take the place of CTAs of this grid that have not started yet.
+    if (p.early_trigger) pdl_launch_dependents();
     pdl_wait();                                              // the selection of k_select is complete and visible
 
     if (warp == 0) {
