@@ -821,7 +821,13 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
     uint64_t lo = 0;                                        // gather keys >= lo (0: all of them)
     pdl_wait();                                              // the candidates of k_nms_* are complete and visible
     __syncthreads();
+    // With a validity mask (V5) the keys are first STAGED in `sorted` by the fast copy and then filtered densely, every
+    // thread testing one key (one mask byte each, all in flight); only if more than SORT_CAP keys turn up is the first
+    // pass repeated with the per-lane filter, which counts without storing.
+    bool stage = vm != nullptr;
     for (int pass = 0; pass < 2; ++pass) {                  // second pass only if the first found n > SORT_CAP
+        const bool copy_all = lo == 0 && (vm == nullptr || stage);
+        uint64_t* const dst = stage ? sorted : keys;
         unsigned khi = 0u, klo = 0xffffffffu;                   // range of the gathered score words
         int c_next = (warp * spw + sl < tpi) ? cnt[warp * spw + sl] : 0;
         for (int t0 = warp * spw; t0 < tpi; t0 += NW * spw) {
@@ -838,7 +844,7 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
             if (total == 0) continue;                           // warp-uniform
             const int excl = incl - c;                          // items of the warp's earlier segments
             int gbase = 0;
-            if (lo == 0 && vm == nullptr) {                     // all keys are kept: reserve the slots at once
+            if (copy_all) {                                     // all keys are kept: reserve the slots at once
                 if (lane == 0) gbase = atomicAdd(&s_n, total);
                 gbase = __shfl_sync(FULL, gbase, 0);
                 if (gbase + total > SORT_CAP) continue;         // too many candidates (rare): counted, radix select below
@@ -860,7 +866,7 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
                     kk[2 * u] = q.x;
                     kk[2 * u + 1] = i + 1 < c ? q.y : 0ull;
                 }
-                if (vm != nullptr) {                            // variant V5: a key on a masked pixel is no candidate
+                if (vm != nullptr && !copy_all) {               // variant V5: a key on a masked pixel is no candidate
 #pragma unroll
                     for (int u = 0; u < 2 * GU; ++u)
                         if (kk[u] != 0ull && __ldg(vm + key_index(kk[u])) == 0) kk[u] = 0ull;
@@ -869,8 +875,9 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
                 for (int u = 0; u < 2 * GU; ++u) {
                     const int i = i0 + 2 * (sub + ((u >> 1) << lps_log)) + (u & 1);
                     uint64_t k = kk[u];
-                    if (lo == 0 && vm == nullptr) {
-                        if (i < c) { DKD_ASSERT(gbase + excl + i >= 0 && gbase + excl + i < SORT_CAP); keys[gbase + excl + i] = k; }
+                    if (copy_all) {
+                        if (i < c) { DKD_ASSERT(gbase + excl + i >= 0 && gbase + excl + i < SORT_CAP); dst[gbase + excl + i] = k; }
+                        if (stage) k = 0ull;                    // (the range is taken after the filter)
                     } else {
                         const bool take = (i < c) && k != 0ull && (k >= lo);
                         const unsigned bal = __ballot_sync(FULL, take);
@@ -895,6 +902,37 @@ __global__ void __launch_bounds__(SEL_THREADS, 1) k_select(const uint64_t* __res
         klo = __reduce_min_sync(FULL, klo);
         if (lane == 0 && khi >= klo) { atomicMax(&s_hi, khi); atomicMin(&s_lo, klo); }
         __syncthreads();
+        if (stage) {                                        // block-uniform
+            stage = false;
+            const int n0 = s_n;
+            __syncthreads();
+            if (tid == 0) s_n = 0;
+            __syncthreads();
+            if (n0 > SORT_CAP) { --pass; continue; }         // too many to stage: count with the per-lane filter instead
+            khi = 0u; klo = 0xffffffffu;
+            for (int i0 = 0; i0 < n0; i0 += SEL_THREADS) {   // (warp-uniform trip count: ballots inside)
+                const int i = i0 + tid;
+                const uint64_t k = i < n0 ? sorted[i] : 0ull;
+                const bool take = k != 0ull && __ldg(vm + key_index(k)) != 0;
+                const unsigned bal = __ballot_sync(FULL, take);
+                if (bal) {
+                    int pb = 0;
+                    if (lane == 0) pb = atomicAdd(&s_n, __popc(bal));
+                    pb = __shfl_sync(FULL, pb, 0);
+                    if (take) {
+                        DKD_ASSERT(pb + __popc(bal) <= SORT_CAP);
+                        keys[pb + __popc(bal & ((1u << lane) - 1u))] = k;
+                        const unsigned kb = static_cast<unsigned>(k >> 32);
+                        khi = kb > khi ? kb : khi;
+                        klo = kb < klo ? kb : klo;
+                    }
+                }
+            }
+            khi = __reduce_max_sync(FULL, khi);
+            klo = __reduce_min_sync(FULL, klo);
+            if (lane == 0 && khi >= klo) { atomicMax(&s_hi, khi); atomicMin(&s_lo, klo); }
+            __syncthreads();
+        }
         if (pass == 0 && tid == 0 && out_total != nullptr) out_total[b] = s_n;   // C_b: every candidate, before the cap
         if (s_n <= SORT_CAP) break;                         // block-uniform; always true in the second pass
         lo = select_radix_prefix(seg0, cnt, tpi, seg_cap, vm, top_k, s_hist, s_rdx);   // (out of line: rare, and the common

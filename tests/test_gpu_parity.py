@@ -329,6 +329,40 @@ def test_loader_graph_and_literal_variants_agree(ctx):
         assert torch.equal(getattr(base, n), getattr(lit, n)), n
 
 
+def test_back_to_back_stream_launches_overlap_safely(ctx):
+    """Plain launches with programmatic dependent launch: the NMS kernel of call i+1 is launched while the refine /
+    gather kernel of call i still runs (both use the context's candidate workspace).  200 calls alternating between
+    two different inputs, never synchronised in between, must give exactly the results of isolated calls; a producer
+    kernel of the caller enqueued right before a call (it writes the score map) must be seen completely."""
+    from paper_2607_01757_b200.binding import OPT_USE_GRAPH
+    ins = [small_inputs(2, 120, 380, seed=40 + j, nblobs=300 + 100 * j, D=128, dtype=torch.float16, stride=1) for j in range(2)]
+    sds = [i[0].cuda() for i in ins]
+    want = []
+    for j in range(2):
+        want.append(ctx.extract(sds[j], ins[j][1], 1, 2, 0.2, 256, 0.1))
+        torch.cuda.synchronize()
+    try:
+        ctx.set_option(OPT_USE_GRAPH, 0)
+        outs = [ctx.alloc_outputs(2, 256, ins[0][1], 128) for _ in range(200)]
+        for i in range(200):
+            ctx.extract(sds[i % 2], ins[i % 2][1], 1, 2, 0.2, 256, 0.1, out=outs[i])
+        torch.cuda.synchronize()
+        for i in range(200):
+            for n in ("kpts", "scores", "desc", "count", "index", "offsets"):
+                assert torch.equal(getattr(want[i % 2], n), getattr(outs[i], n)), (i, n)
+        # the score map is produced by a kernel of the caller right before the call
+        buf = torch.zeros_like(sds[0])
+        for i in range(20):
+            buf.copy_(sds[i % 2] * 1.0)                          # (an elementwise kernel on the same stream)
+            ctx.extract(buf, ins[i % 2][1], 1, 2, 0.2, 256, 0.1, out=outs[i])
+        torch.cuda.synchronize()
+        for i in range(20):
+            for n in ("kpts", "scores", "desc", "count", "index", "offsets"):
+                assert torch.equal(getattr(want[i % 2], n), getattr(outs[i], n)), ("producer", i, n)
+    finally:
+        ctx.set_option(OPT_USE_GRAPH, 1)
+
+
 def test_batch_equals_single_images_and_keypoints_only(ctx):
     score, desc = small_inputs(3, 90, 200, seed=2, nblobs=100, D=64, dtype=torch.float32, stride=1)
     sd = score.cuda()
