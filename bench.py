@@ -377,7 +377,7 @@ def run_ours(args):
         torch.cuda.empty_cache()
 
     # the same steps as plain stream launches (DKD_OPT_USE_GRAPH = 0: three PDL-linked launches per step)
-    stream_us = None
+    stream_us = stream_dev_us = graph_dev_us = None
     if args.leg not in ("c5", "pre", "match"):
         ctx.set_option(OPT_USE_GRAPH, 0)
         for i in range(Wm):
@@ -391,7 +391,26 @@ def run_ours(args):
         torch.cuda.synchronize()
         barrier()
         stream_us = max_over_ranks(ev0.elapsed_time(ev1) / K) * 1e3 / world
+        # the device's own time per step: the same launches queued behind a sleeping kernel, so that the host's launch
+        # rate (three launches per step from Python) does not limit them
+        Kq = min(K, 1000)
+        torch.cuda._sleep(int(30e-3 * 1.9e9))
+        ev0.record(stream)
+        for i in range(Kq):
+            calls[i % R]()
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        barrier()
+        stream_dev_us = max_over_ranks(ev0.elapsed_time(ev1) / Kq) * 1e3 / world
         ctx.set_option(OPT_USE_GRAPH, 1)
+        torch.cuda._sleep(int(30e-3 * 1.9e9))
+        ev0.record(stream)
+        for i in range(Kq):
+            calls[i % R]()
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        barrier()
+        graph_dev_us = max_over_ranks(ev0.elapsed_time(ev1) / Kq) * 1e3 / world
 
     # the same steps with output buffers the cached graph has not seen: every call hands the library another output set,
     # so each launch goes through the kernel-node update path of the shape-keyed graph cache (no capture, no instantiate)
@@ -727,8 +746,11 @@ def run_ours(args):
             "wall_ms_per_step": wall_ms_step,
             "latency_us": {"median": lat[len(lat) // 2], "min": lat[0], "p95": lat[int(len(lat) * 0.95)],
                            "what": "single shot: enqueue -> stream idle, host clock"},
-            "stream_launch": {"value": stream_us, "unit": UNIT,
-                              "what": "same steps with DKD_OPT_USE_GRAPH = 0: three PDL-linked launches per step instead of one graph launch"},
+            "stream_launch": {"value": stream_us, "unit": UNIT, "queued_on_device": stream_dev_us, "graph_queued_on_device": graph_dev_us,
+                              "what": "same steps with DKD_OPT_USE_GRAPH = 0: three PDL-linked launches per step instead of one graph launch "
+                                      "(the NMS kernel of a step is launched under the previous step's refine/gather); queued_on_device = the "
+                                      "same launches queued behind a sleeping kernel (the device's own time per step, no host launch-rate "
+                                      "limit), graph_queued_on_device = the default graph launches measured the same way"},
             "fresh_buffers": fresh,
             "kernel_us_c2": kt2,
             "clocks": sampler.summary(),
