@@ -150,6 +150,9 @@ __global__ void __launch_bounds__(MT_THREADS, 1) k_match_tc(const __grid_constan
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int rb = blockIdx.x, sp = blockIdx.y, pr = blockIdx.z;
+    // programmatic dependent launch: the next kernel of the call (the reverse direction, k_match_finalize) may be
+    // scheduled while this grid runs; k_match_finalize waits for its predecessor before it reads the partials
+    asm volatile("griddepcontrol.launch_dependents;");
     const int na = p.count_a ? min(max(p.count_a[pr], 0), p.Na) : p.Na;
     const int nb = p.count_b ? min(max(p.count_b[pr], 0), p.Nb) : p.Nb;
     const int tiles = (nb + MT_BN - 1) / MT_BN;
@@ -285,6 +288,9 @@ __global__ void __launch_bounds__(MT_THREADS, 1) k_match_tc(const __grid_constan
         tc_fence_after();
         tc_dealloc(tmem, MT_TMEM_COLS);
     }
+    // Launched with the programmatic attribute (the reverse direction of a mutual match) this grid read nothing its
+    // predecessor wrote; it only must not COMPLETE before it, so that k_match_finalize's wait covers both directions.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
 // merge of the column splits (in column order), ratio test (M3), mutual check (M4)
@@ -308,6 +314,7 @@ __device__ __forceinline__ MatchRec merge_splits(const MatchRec* part, int split
 }
 __global__ void __launch_bounds__(256) k_match_finalize(const __grid_constant__ FinalizeParams p) {
     const int i = blockIdx.x * 256 + threadIdx.x, pr = blockIdx.y;
+    asm volatile("griddepcontrol.wait;" ::: "memory");      // the partials of k_match_tc are complete and visible
     if (i >= p.Na) return;
     const int na = p.count_a ? min(max(p.count_a[pr], 0), p.Na) : p.Na;
     int m = -1;
@@ -566,7 +573,7 @@ int match_splits(int num_sms, int Na, int Nb, int P) {
 }
 
 cudaError_t launch_match_dir(dkd_ctx* ctx, const void* A, const int32_t* ca, int Na, const void* B, const int32_t* cb, int Nb, int D,
-                             int P, int splits, MatchRec* part, cudaStream_t st) {
+                             int P, int splits, MatchRec* part, cudaStream_t st, bool pdl) {
     CUtensorMap ta, tb;
     if (!encode_desc_map(&ta, A, Na, D, P) || !encode_desc_map(&tb, B, Nb, D, P)) return cudaErrorInvalidValue;
     MatchParams mp;
@@ -585,8 +592,9 @@ cudaError_t launch_match_dir(dkd_ctx* ctx, const void* A, const int32_t* ca, int
     }
     (void)ctx;
     const dim3 grid((Na + MT_BM - 1) / MT_BM, splits, P);
-    k_match_tc<<<grid, MT_THREADS, smem, st>>>(ta, tb, mp);
-    return cudaGetLastError();
+    KLaunch k;
+    prep(k, k_match_tc, grid, dim3(MT_THREADS), smem, pdl, ta, tb, mp);
+    return launch(k, st, true);
 }
 
 }  // namespace dkd
@@ -613,15 +621,20 @@ int dkd_match(dkd_ctx* ctx, const void* desc_a, const int32_t* count_a, int Na, 
     const size_t n_ab = static_cast<size_t>(P) * s_ab * Na, n_ba = static_cast<size_t>(P) * s_ba * Nb;
     MatchRec* part = static_cast<MatchRec*>(dkd_ctx_scratch(ctx, 0, (n_ab + n_ba) * sizeof(MatchRec)));
     if (!part) return DKD_ERR_CUDA;
-    cudaError_t e = launch_match_dir(ctx, desc_a, count_a, Na, desc_b, count_b, Nb, D, P, s_ab, part, st);
-    if (e == cudaSuccess && mutual) e = launch_match_dir(ctx, desc_b, count_b, Nb, desc_a, count_a, Na, D, P, s_ba, part + n_ab, st);
+    // the first kernel waits for whatever precedes it on the stream (it produced the descriptors); the reverse direction and
+    // the finalize kernel are programmatic dependents
+    cudaError_t e = launch_match_dir(ctx, desc_a, count_a, Na, desc_b, count_b, Nb, D, P, s_ab, part, st, false);
+    if (e == cudaSuccess && mutual) e = launch_match_dir(ctx, desc_b, count_b, Nb, desc_a, count_a, Na, D, P, s_ba, part + n_ab, st, true);
     if (e != cudaSuccess) return dkd_ctx_fail(ctx, DKD_ERR_CUDA, "dkd_match launch: ", cudaGetErrorString(e));
     FinalizeParams fp;
     memset(&fp, 0, sizeof(fp));
     fp.part = part; fp.rpart = mutual ? part + n_ab : nullptr; fp.count_a = count_a; fp.Na = Na; fp.Nb = Nb; fp.splits = s_ab;
     fp.rsplits = s_ba; fp.P = P; fp.ratio2 = ratio >= 1e9f ? -1.0f : ratio * ratio; fp.out_match = out_match; fp.out_sim = out_sim;
-    k_match_finalize<<<dim3((Na + 255) / 256, P), 256, 0, st>>>(fp);
-    e = cudaGetLastError();
+    {
+        KLaunch k;
+        prep(k, k_match_finalize, dim3((Na + 255) / 256, P), dim3(256), 0, true, fp);
+        e = launch(k, st, true);
+    }
     if (e != cudaSuccess) return dkd_ctx_fail(ctx, DKD_ERR_CUDA, "k_match_finalize launch: ", cudaGetErrorString(e));
     return DKD_OK;
 }
