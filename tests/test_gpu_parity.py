@@ -201,7 +201,7 @@ def test_random_sweep_and_worst_cases_under_the_debug_build():
     build.build(debug=True)
     env = dict(os.environ, DKD_LIBRARY="libdkd_debug.so")
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-    sel = "random_shapes or worst_case or many_candidates or units_of_several or small_multitile or ties_at_clamp"
+    sel = "random_shapes or worst_case or many_candidates or units_of_several or small_multitile or ties_at_clamp or back_to_back"
     r = subprocess.run([sys.executable, "-m", "pytest", "tests/test_gpu_parity.py", "tests/test_gpu_variants.py",
                         "tests/test_gpu_match.py", "-q", "-x", "-m", "gpu", "-k",
                         "(" + sel + " or reliability or validity or retrieval or match_small) and not debug_build"],

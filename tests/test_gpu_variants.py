@@ -85,6 +85,30 @@ def test_validity_mask(ctx, r, W):
     assert int(none.count.sum()) == 0 and int(none.total.sum()) == 0
 
 
+@pytest.mark.parametrize("unit", [0, 1, 4, 8])
+def test_validity_mask_with_more_candidates_than_the_sort_capacity(ctx, unit):
+    """A plateau map (tens of thousands of tied candidates) under a validity mask: the staged dense filter of k_select
+    overflows its 8192-key capacity, the first pass is repeated with the per-lane filter, the radix narrowing reads the
+    mask too — for one-tile and multi-tile NMS units (1, 2, 4, 8 lanes per candidate segment in the gather).  Also the
+    case where the UNMASKED candidates fit although the staged ones do not."""
+    from paper_2607_01757_b200.binding import OPT_NMS_UNIT
+    g = torch.Generator().manual_seed(11 + unit)
+    s = (torch.randint(0, 4, (2, 300, 400), generator=g).float() / 4.0)
+    s = torch.nn.functional.max_pool2d(s[None], 3, 1, 1)[0]                    # plateaus -> lots of tied maxima
+    dense = (torch.rand((2, 300, 400), generator=g) < 0.7).to(torch.uint8)    # > 8192 unmasked candidates
+    sparse = (torch.rand((2, 300, 400), generator=g) < 0.05).to(torch.uint8)  # staged > 8192, unmasked < 8192
+    try:
+        ctx.set_option(OPT_NMS_UNIT, unit)
+        for vm, top_k in ((dense, 500), (dense, 8192), (sparse, 3000)):
+            res = ctx.extract(s.cuda(), None, 1, 1, 0.2, top_k, 0.1, valid_mask=vm.cuda(), want_total=True)
+            ref = oracle.extract_var(s.numpy(), None, 1, 1, 0.2, top_k, 0.1, valid_mask=vm.numpy())
+            compare_var(res, ref)
+        staged = int(oracle.nms_mask(s[0].numpy(), 1, 0.2).sum())
+        assert staged > 8192 and ref.total.max() < 8192
+    finally:
+        ctx.set_option(OPT_NMS_UNIT, 0)
+
+
 @pytest.mark.parametrize("r", [1, 2, 3, 4])
 def test_score_at_refined_point(ctx, r):
     score, desc, _, _ = inputs(2, 96, 200, seed=30 + r, nblobs=200, D=0)
