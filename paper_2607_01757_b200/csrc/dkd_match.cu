@@ -100,6 +100,38 @@ __device__ __forceinline__ void tc_ld_32x32(uint32_t taddr, uint32_t (&v)[32]) {
         : "r"(taddr)
         : "memory");
 }
+// thread t of the warp writes row (lane base + t), columns c .. c+31 (the mirror of tc_ld_32x32)
+__device__ __forceinline__ void tc_st_32x32(uint32_t taddr, const uint32_t (&v)[32]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
+        "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};"
+        ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]),
+          "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]), "r"(v[16]), "r"(v[17]),
+          "r"(v[18]), "r"(v[19]), "r"(v[20]), "r"(v[21]), "r"(v[22]), "r"(v[23]), "r"(v[24]), "r"(v[25]), "r"(v[26]),
+          "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31])
+        : "memory");
+}
+// true in exactly one lane of a converged warp; the compiler then knows the guarded code runs in a single thread and emits
+// the uniform-register instructions (UTCHMMA, UTMALDG) without a per-lane election loop around each of them
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile("{\n.reg .pred P;\nelect.sync _|P, 0xffffffff;\nselp.u32 %0, 1, 0, P;\n}" : "=r"(pred));
+    return pred != 0;
+}
+__device__ __forceinline__ void tc_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+// D[tmem] (+)= A[tmem] * B[smem desc]^T: the A operand read from tensor memory (row m in lane m, fp16 pairs packed in
+// 32-bit columns), so that only B crosses the shared-memory port
+__device__ __forceinline__ void tc_mma_f16_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t desc_b, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n"
+        "}" ::"r"(tmem_d),
+        "r"(tmem_a), "l"(desc_b), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
 __device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 // ---- k_match_tc -------------------------------------------------------------------------------------------
@@ -116,7 +148,11 @@ __device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sy
 // Rows >= count_a and columns >= count_b (the zero padding of PAPER.md:139) are masked out.
 constexpr int MT_BM = 128, MT_BN = 128, MT_KBOX = 64;            // KBOX fp16 = 128 bytes = the swizzle span
 constexpr int MT_THREADS = 320;                                  // 10 warps
-constexpr int MT_TMEM_COLS = 256;                                // two accumulator buffers
+#ifndef DKD_MT_A_TMEM
+#define DKD_MT_A_TMEM 0                                          // 1: the A block lives in tensor memory (see k_match_tc)
+#endif
+constexpr int MT_ACC_COLS = 256;                                 // two accumulator buffers of 128 fp32 columns
+constexpr int MT_TMEM_COLS = DKD_MT_A_TMEM ? 512 : 256;          // + up to 128 columns of A (D / 2 packed fp16 pairs per row)
 constexpr int MT_MAX_KB = 4;                                     // D <= 256
 
 struct MatchRec {                      // partial result of one row over one column split
@@ -131,6 +167,7 @@ struct MatchParams {
     int Na, Nb, KB;                    // KB = D / 64
     int splits, stages;
     MatchRec* part;                    // [P, splits, Na]
+    const uint32_t* a_words;           // A as 32-bit words (two fp16 each): [P, Na, D / 2]
 };
 
 __device__ __forceinline__ uint64_t mt_desc(uint32_t smem_addr) {
@@ -164,10 +201,10 @@ __global__ void __launch_bounds__(MT_THREADS, 1) k_match_tc(const __grid_constan
     const uint32_t a_bytes = static_cast<uint32_t>(p.KB) * MT_BM * 128u;          // A block: KB x 16 KB
     const uint32_t b_bytes = static_cast<uint32_t>(p.KB) * MT_BN * 128u;          // one B tile
     unsigned char* smem_a = mt_smem + ((1024u - (m_smem_u32(mt_smem) & 1023u)) & 1023u);   // the swizzle atom is 1024 bytes
-    unsigned char* smem_b = smem_a + a_bytes;
+    unsigned char* smem_b = DKD_MT_A_TMEM ? smem_a : smem_a + a_bytes;
 
     if (threadIdx.x == 0) {
-        m_mbar_init(&bar_a, 1);
+        m_mbar_init(&bar_a, DKD_MT_A_TMEM ? 128 : 1);
         for (int s = 0; s < 4; ++s) { m_mbar_init(&bar_full[s], 1); m_mbar_init(&bar_empty[s], 1); }
         for (int a = 0; a < 2; ++a) { m_mbar_init(&bar_tfull[a], 1); m_mbar_init(&bar_tempty[a], 256); }
         m_fence_mbar_init();
@@ -183,8 +220,10 @@ __global__ void __launch_bounds__(MT_THREADS, 1) k_match_tc(const __grid_constan
             if (lane == 0) {                                     // ===== TMA producer =====
                 m_prefetch_tmap(&tmap_a);
                 m_prefetch_tmap(&tmap_b);
-                m_mbar_expect_tx(&bar_a, a_bytes);
-                for (int kb = 0; kb < p.KB; ++kb) m_tma_load_3d(smem_a + kb * (MT_BM * 128), &tmap_a, &bar_a, kb * MT_KBOX, row0, pr);
+                if (!DKD_MT_A_TMEM) {
+                    m_mbar_expect_tx(&bar_a, a_bytes);
+                    for (int kb = 0; kb < p.KB; ++kb) m_tma_load_3d(smem_a + kb * (MT_BM * 128), &tmap_a, &bar_a, kb * MT_KBOX, row0, pr);
+                }
                 for (int t = t0, it = 0; t < t1; ++t, ++it) {
                     const int s = it % p.stages;
                     if (it >= p.stages) m_mbar_wait(&bar_empty[s], ((it / p.stages) - 1) & 1);
@@ -194,7 +233,7 @@ __global__ void __launch_bounds__(MT_THREADS, 1) k_match_tc(const __grid_constan
                 }
             }
         } else if (warp == 1) {
-            if (lane == 0) {                                     // ===== MMA issuer =====
+            {                                                    // ===== MMA issuer: the warp stays converged, one elected lane issues =====
                 // instruction descriptor: D = F32 (bits 4-5 = 1), A = B = F16 (0), both K-major, N >> 3 at bit 17, M >> 4 at bit 24
                 const uint32_t idesc = (1u << 4) | (static_cast<uint32_t>(MT_BN >> 3) << 17) | (static_cast<uint32_t>(MT_BM >> 4) << 24);
                 m_mbar_wait(&bar_a, 0);
@@ -203,22 +242,56 @@ __global__ void __launch_bounds__(MT_THREADS, 1) k_match_tc(const __grid_constan
                     if (it >= 2) m_mbar_wait(&bar_tempty[acc], ((it >> 1) - 1) & 1);   // the epilogue has drained this buffer
                     m_mbar_wait(&bar_full[s], (it / p.stages) & 1);
                     tc_fence_after();
-                    const uint32_t a0 = m_smem_u32(smem_a), b0 = m_smem_u32(smem_b + s * b_bytes);
-                    for (int kb = 0; kb < p.KB; ++kb) {
+                    // One thread issues every tcgen05.mma, and a 128 x 128 x 16 MMA keeps the tensor pipe busy for only ~64
+                    // cycles: the descriptors must not cost a dependent chain each.  The 14-bit address field holds
+                    // (address >> 4) of a buffer below 256 KB, so the descriptor of a later K step is the stage's base
+                    // descriptor plus a constant — one independent add per MMA.
+                    const uint64_t a_base = mt_desc(m_smem_u32(smem_a)), b_base = mt_desc(m_smem_u32(smem_b + s * b_bytes));
+                    const uint32_t d_tmem = tmem + acc * MT_BN, a_tmem = tmem + MT_ACC_COLS;
+                    if (elect_one()) {
 #pragma unroll
-                        for (int k = 0; k < MT_KBOX / 16; ++k) {  // UMMA_K = 16 fp16 = 32 bytes inside the swizzle atom
-                            const uint64_t da = mt_desc(a0 + kb * (MT_BM * 128) + k * 32);
-                            const uint64_t db = mt_desc(b0 + kb * (MT_BN * 128) + k * 32);
-                            tc_mma_f16(tmem + acc * MT_BN, da, db, idesc, (kb | k) != 0);
+                    for (int kb = 0; kb < MT_MAX_KB; ++kb) {
+                        if (kb < p.KB) {
+#pragma unroll
+                            for (int k = 0; k < MT_KBOX / 16; ++k) {  // UMMA_K = 16 fp16 = 32 bytes inside the swizzle atom
+                                const uint64_t db = b_base + static_cast<uint64_t>((kb * (MT_BN * 128) + k * 32) >> 4);
+                                if (DKD_MT_A_TMEM) {              // 16 fp16 of K = 8 packed columns
+                                    tc_mma_f16_ts(d_tmem, a_tmem + kb * (MT_KBOX / 2) + k * 8, db, idesc, (kb | k) != 0);
+                                } else {
+                                    const uint64_t da = a_base + static_cast<uint64_t>((kb * (MT_BM * 128) + k * 32) >> 4);
+                                    tc_mma_f16(d_tmem, da, db, idesc, (kb | k) != 0);
+                                }
+                            }
                         }
                     }
                     tc_commit(&bar_empty[s]);                    // smem stage free once these MMAs have read it
                     tc_commit(&bar_tfull[acc]);                  // accumulator complete
+                    }
+                    __syncwarp();
                 }
             }
         } else {                                                 // ===== epilogue: one thread per row and column half =====
             const int q = warp & 3, h = (warp - 2) >> 2;
             const int row = row0 + 32 * q + lane;
+            if (DKD_MT_A_TMEM && h == 0) {
+                // The A block goes to TENSOR MEMORY once (row m in lane m, the row's fp16 pairs in D / 2 consecutive 32-bit
+                // columns behind the accumulators): every tcgen05.mma then reads only B through the shared-memory port,
+                // which is what bounds a 128 x 128 single-CTA tile.  Rows past the set read as zeros.
+                const uint32_t* arow = p.a_words + (static_cast<size_t>(pr) * p.Na + (row < p.Na ? row : 0)) * (p.KB * (MT_KBOX / 2));
+                for (int c = 0; c < p.KB * (MT_KBOX / 2); c += 32) {
+                    uint32_t w[32];
+#pragma unroll
+                    for (int j = 0; j < 32; j += 4) {
+                        uint4 t4 = make_uint4(0u, 0u, 0u, 0u);
+                        if (row < p.Na) t4 = __ldg(reinterpret_cast<const uint4*>(arow + c + j));
+                        w[j] = t4.x; w[j + 1] = t4.y; w[j + 2] = t4.z; w[j + 3] = t4.w;
+                    }
+                    tc_st_32x32(tmem + (static_cast<uint32_t>(32 * q) << 16) + MT_ACC_COLS + c, w);
+                }
+                tc_wait_st();
+                tc_fence_before();
+                m_mbar_arrive(&bar_a);                           // 128 arrivals: the whole block is in place
+            }
             float best = -INFINITY, second = -INFINITY;
             int arg = -1;
             for (int t = t0, it = 0; t < t1; ++t, ++it) {
@@ -579,7 +652,8 @@ cudaError_t launch_match_dir(dkd_ctx* ctx, const void* A, const int32_t* ca, int
     MatchParams mp;
     memset(&mp, 0, sizeof(mp));
     mp.count_a = ca; mp.count_b = cb; mp.Na = Na; mp.Nb = Nb; mp.KB = D / MT_KBOX; mp.splits = splits; mp.part = part;
-    const size_t a_bytes = static_cast<size_t>(mp.KB) * MT_BM * 128, b_bytes = static_cast<size_t>(mp.KB) * MT_BN * 128;
+    mp.a_words = static_cast<const uint32_t*>(A);
+    const size_t a_bytes = DKD_MT_A_TMEM ? 0 : static_cast<size_t>(mp.KB) * MT_BM * 128, b_bytes = static_cast<size_t>(mp.KB) * MT_BN * 128;
     int stages = static_cast<int>((200 * 1024 - a_bytes) / b_bytes);
     if (stages > 4) stages = 4;
     mp.stages = stages;
