@@ -131,6 +131,13 @@ __device__ __forceinline__ void st_keep_u64(uint64_t* p, uint64_t v, uint64_t po
 __device__ __forceinline__ void st_keep_s32(int* p, int v, uint64_t policy) {
     asm volatile("st.global.L2::cache_hint.b32 [%0], %1, %2;" ::"l"(p), "r"(v), "l"(policy) : "memory");
 }
+// true in exactly one lane of a converged warp (elect.sync): the compiler then knows the guarded code runs in a single
+// thread and emits the uniform-register instructions (UTMALDG) without a per-lane election loop around them
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile("{\n.reg .pred P;\nelect.sync _|P, 0xffffffff;\nselp.u32 %0, 1, 0, P;\n}" : "=r"(pred));
+    return pred != 0;
+}
 __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* tmap) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(tmap)) : "memory");
 }
@@ -387,7 +394,7 @@ __global__ void __launch_bounds__(NMS_WARPS * 32, PROD ? 1 : NMS_CTAS) k_nms_tma
     auto issue_box = [&]() {
         if (iit >= n_my) return;
         const int s = issued % NMS_STAGES;
-        if (lane == 0) {
+        if (elect_one()) {                                   // (the warp is converged here: one elected lane issues)
             mbar_arrive_expect_tx(&bar[s], STAGE_BYTES);
             tma_load_tile(my_smem + s * STAGE_BYTES, &tmap, &bar[s], iu.x0 - HALO_X, iu.y0 + R + TH * ic, iu.b, policy);
             if constexpr (PROD)
