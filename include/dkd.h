@@ -62,9 +62,13 @@ enum {
                                 score is 16-byte aligned; 0 = always the plain-load tile loader. */
     DKD_OPT_PROFILE   = 2,   /* [0] 1 = measurement mode: plain launches (no graph) with a CUDA event recorded
                                 on `stream` before and after every kernel; read with dkd_profile_read. */
-    DKD_OPT_USE_PDL   = 3,   /* [1] the select and refine/gather kernels are launched with programmatic
-                                stream serialization (they start while their predecessor drains and wait
-                                on-device for its results): hides the launch latency between the kernels. */
+    DKD_OPT_USE_PDL   = 3,   /* [1] the kernels are launched with programmatic stream serialization (they start
+                                while their predecessor drains and wait on-device, griddepcontrol.wait, before
+                                they touch global memory): hides the launch latency between the kernels.  The
+                                NMS kernel carries the attribute too, so with plain launches (DKD_OPT_USE_GRAPH
+                                = 0, or while the caller captures) it may be SCHEDULED while the previous kernel
+                                of `stream` still runs — it reads `score` only after that kernel has completed
+                                and flushed, whatever that kernel is; results never depend on this option. */
     DKD_OPT_ORIGIN_X  = 5,   /* [0] letterbox offset (ox, oy) of the score map inside the padded network input: it is */
     DKD_OPT_ORIGIN_Y  = 6,   /* [0] subtracted from every keypoint coordinate ("shifted back to native coordinates by
                                 subtracting the offset"); out_index / out_offset are unaffected. */
