@@ -146,13 +146,11 @@ __device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sy
 //            (best, arg best, second best) in registers — no cross-thread reduction; columns are visited in
 //            increasing order and the comparison is strict, so ties keep the smallest column (M2).
 // Rows >= count_a and columns >= count_b (the zero padding of PAPER.md:139) are masked out.
-constexpr int MT_BM = 128, MT_BN = 128, MT_KBOX = 64;            // KBOX fp16 = 128 bytes = the swizzle span
+constexpr int MT_BM = 128, MT_BN = 256, MT_KBOX = 64;            // KBOX fp16 = 128 bytes = the swizzle span
+constexpr int MT_BOX_ROWS = 128;                                 // rows of one TMA box (A block: one box per k-box; B unit: two)
 constexpr int MT_THREADS = 320;                                  // 10 warps
-#ifndef DKD_MT_A_TMEM
-#define DKD_MT_A_TMEM 0                                          // 1: the A block lives in tensor memory (see k_match_tc)
-#endif
-constexpr int MT_ACC_COLS = 256;                                 // two accumulator buffers of 128 fp32 columns
-constexpr int MT_TMEM_COLS = DKD_MT_A_TMEM ? 512 : 256;          // + up to 128 columns of A (D / 2 packed fp16 pairs per row)
+constexpr int MT_TMEM_COLS = 2 * MT_BN;                           // two accumulator buffers of 256 fp32 columns = all of TMEM
+constexpr int MT_MAX_STAGES = 8;                                 // ring units of the B stream
 constexpr int MT_MAX_KB = 4;                                     // D <= 256
 
 struct MatchRec {                      // partial result of one row over one column split
@@ -167,7 +165,6 @@ struct MatchParams {
     int Na, Nb, KB;                    // KB = D / 64
     int splits, stages;
     MatchRec* part;                    // [P, splits, Na]
-    const uint32_t* a_words;           // A as 32-bit words (two fp16 each): [P, Na, D / 2]
 };
 
 __device__ __forceinline__ uint64_t mt_desc(uint32_t smem_addr) {
@@ -181,7 +178,7 @@ __global__ void __launch_bounds__(MT_THREADS, 1) k_match_tc(const __grid_constan
                                                             const __grid_constant__ CUtensorMap tmap_b,
                                                             const __grid_constant__ MatchParams p) {
     extern __shared__ __align__(1024) unsigned char mt_smem[];
-    __shared__ __align__(8) uint64_t bar_a, bar_full[4], bar_empty[4], bar_tfull[2], bar_tempty[2];
+    __shared__ __align__(8) uint64_t bar_a, bar_full[MT_MAX_STAGES], bar_empty[MT_MAX_STAGES], bar_tfull[2], bar_tempty[2];
     __shared__ uint32_t s_tmem;
     __shared__ MatchRec s_half[MT_BM];                           // the upper column half's result of every row
 
@@ -199,13 +196,16 @@ __global__ void __launch_bounds__(MT_THREADS, 1) k_match_tc(const __grid_constan
     const bool active = row0 < na && t1 > t0;                    // (block-uniform)
 
     const uint32_t a_bytes = static_cast<uint32_t>(p.KB) * MT_BM * 128u;          // A block: KB x 16 KB
-    const uint32_t b_bytes = static_cast<uint32_t>(p.KB) * MT_BN * 128u;          // one B tile
+    // The B stream moves UNITS of one k-box: 256 rows x 128 bytes = 32 KB (two TMA boxes of 128 rows, one below the other,
+    // so that the 8-row groups of the whole unit are 1024 bytes apart: one N = 256 operand).  A tile of 256 columns of S is
+    // KB units; a unit's shared memory is released as soon as its four MMAs have read it.
+    const uint32_t b_bytes = static_cast<uint32_t>(MT_BN) * 128u;                 // one unit
     unsigned char* smem_a = mt_smem + ((1024u - (m_smem_u32(mt_smem) & 1023u)) & 1023u);   // the swizzle atom is 1024 bytes
-    unsigned char* smem_b = DKD_MT_A_TMEM ? smem_a : smem_a + a_bytes;
+    unsigned char* smem_b = smem_a + a_bytes;
 
     if (threadIdx.x == 0) {
-        m_mbar_init(&bar_a, DKD_MT_A_TMEM ? 128 : 1);
-        for (int s = 0; s < 4; ++s) { m_mbar_init(&bar_full[s], 1); m_mbar_init(&bar_empty[s], 1); }
+        m_mbar_init(&bar_a, 1);
+        for (int s = 0; s < MT_MAX_STAGES; ++s) { m_mbar_init(&bar_full[s], 1); m_mbar_init(&bar_empty[s], 1); }
         for (int a = 0; a < 2; ++a) { m_mbar_init(&bar_tfull[a], 1); m_mbar_init(&bar_tempty[a], 256); }
         m_fence_mbar_init();
     }
@@ -220,16 +220,16 @@ __global__ void __launch_bounds__(MT_THREADS, 1) k_match_tc(const __grid_constan
             if (lane == 0) {                                     // ===== TMA producer =====
                 m_prefetch_tmap(&tmap_a);
                 m_prefetch_tmap(&tmap_b);
-                if (!DKD_MT_A_TMEM) {
-                    m_mbar_expect_tx(&bar_a, a_bytes);
-                    for (int kb = 0; kb < p.KB; ++kb) m_tma_load_3d(smem_a + kb * (MT_BM * 128), &tmap_a, &bar_a, kb * MT_KBOX, row0, pr);
-                }
-                for (int t = t0, it = 0; t < t1; ++t, ++it) {
-                    const int s = it % p.stages;
-                    if (it >= p.stages) m_mbar_wait(&bar_empty[s], ((it / p.stages) - 1) & 1);
-                    m_mbar_expect_tx(&bar_full[s], b_bytes);
-                    for (int kb = 0; kb < p.KB; ++kb)
-                        m_tma_load_3d(smem_b + s * b_bytes + kb * (MT_BN * 128), &tmap_b, &bar_full[s], kb * MT_KBOX, t * MT_BN, pr);
+                m_mbar_expect_tx(&bar_a, a_bytes);
+                for (int kb = 0; kb < p.KB; ++kb) m_tma_load_3d(smem_a + kb * (MT_BM * 128), &tmap_a, &bar_a, kb * MT_KBOX, row0, pr);
+                for (int t = t0, iu = 0; t < t1; ++t) {
+                    for (int kb = 0; kb < p.KB; ++kb, ++iu) {
+                        const int s = iu % p.stages;
+                        if (iu >= p.stages) m_mbar_wait(&bar_empty[s], ((iu / p.stages) - 1) & 1);
+                        m_mbar_expect_tx(&bar_full[s], b_bytes);
+                        m_tma_load_3d(smem_b + s * b_bytes, &tmap_b, &bar_full[s], kb * MT_KBOX, t * MT_BN, pr);
+                        m_tma_load_3d(smem_b + s * b_bytes + MT_BOX_ROWS * 128, &tmap_b, &bar_full[s], kb * MT_KBOX, t * MT_BN + MT_BOX_ROWS, pr);
+                    }
                 }
             }
         } else if (warp == 1) {
@@ -237,61 +237,36 @@ __global__ void __launch_bounds__(MT_THREADS, 1) k_match_tc(const __grid_constan
                 // instruction descriptor: D = F32 (bits 4-5 = 1), A = B = F16 (0), both K-major, N >> 3 at bit 17, M >> 4 at bit 24
                 const uint32_t idesc = (1u << 4) | (static_cast<uint32_t>(MT_BN >> 3) << 17) | (static_cast<uint32_t>(MT_BM >> 4) << 24);
                 m_mbar_wait(&bar_a, 0);
-                for (int t = t0, it = 0; t < t1; ++t, ++it) {
-                    const int s = it % p.stages, acc = it & 1;
+                const uint64_t a_base = mt_desc(m_smem_u32(smem_a));
+                for (int t = t0, it = 0, iu = 0; t < t1; ++t, ++it) {
+                    const int acc = it & 1;
                     if (it >= 2) m_mbar_wait(&bar_tempty[acc], ((it >> 1) - 1) & 1);   // the epilogue has drained this buffer
-                    m_mbar_wait(&bar_full[s], (it / p.stages) & 1);
-                    tc_fence_after();
-                    // One thread issues every tcgen05.mma, and a 128 x 128 x 16 MMA keeps the tensor pipe busy for only ~64
-                    // cycles: the descriptors must not cost a dependent chain each.  The 14-bit address field holds
-                    // (address >> 4) of a buffer below 256 KB, so the descriptor of a later K step is the stage's base
-                    // descriptor plus a constant — one independent add per MMA.
-                    const uint64_t a_base = mt_desc(m_smem_u32(smem_a)), b_base = mt_desc(m_smem_u32(smem_b + s * b_bytes));
-                    const uint32_t d_tmem = tmem + acc * MT_BN, a_tmem = tmem + MT_ACC_COLS;
-                    if (elect_one()) {
+                    const uint32_t d_tmem = tmem + acc * MT_BN;
+                    for (int kb = 0; kb < p.KB; ++kb, ++iu) {
+                        const int s = iu % p.stages;
+                        m_mbar_wait(&bar_full[s], (iu / p.stages) & 1);
+                        tc_fence_after();
+                        // One thread issues every tcgen05.mma, and the tensor pipe is busy for only ~128 cycles per 128 x 256 x
+                        // 16 MMA: the descriptors must not cost a dependent chain each.  The 14-bit address field holds
+                        // (address >> 4) of a buffer below 256 KB, so the descriptor of a later K step is the base descriptor
+                        // plus a constant — one independent add per MMA.
+                        const uint64_t b_base = mt_desc(m_smem_u32(smem_b + s * b_bytes));
+                        const uint64_t a_kb = a_base + static_cast<uint64_t>((kb * (MT_BM * 128)) >> 4);
+                        if (elect_one()) {
 #pragma unroll
-                    for (int kb = 0; kb < MT_MAX_KB; ++kb) {
-                        if (kb < p.KB) {
-#pragma unroll
-                            for (int k = 0; k < MT_KBOX / 16; ++k) {  // UMMA_K = 16 fp16 = 32 bytes inside the swizzle atom
-                                const uint64_t db = b_base + static_cast<uint64_t>((kb * (MT_BN * 128) + k * 32) >> 4);
-                                if (DKD_MT_A_TMEM) {              // 16 fp16 of K = 8 packed columns
-                                    tc_mma_f16_ts(d_tmem, a_tmem + kb * (MT_KBOX / 2) + k * 8, db, idesc, (kb | k) != 0);
-                                } else {
-                                    const uint64_t da = a_base + static_cast<uint64_t>((kb * (MT_BM * 128) + k * 32) >> 4);
-                                    tc_mma_f16(d_tmem, da, db, idesc, (kb | k) != 0);
-                                }
-                            }
+                            for (int k = 0; k < MT_KBOX / 16; ++k)   // UMMA_K = 16 fp16 = 32 bytes inside the swizzle atom
+                                tc_mma_f16(d_tmem, a_kb + static_cast<uint64_t>((k * 32) >> 4), b_base + static_cast<uint64_t>((k * 32) >> 4),
+                                           idesc, (kb | k) != 0);
+                            tc_commit(&bar_empty[s]);            // the unit's shared memory is free once these MMAs have read it
+                            if (kb + 1 == p.KB) tc_commit(&bar_tfull[acc]);   // accumulator complete
                         }
+                        __syncwarp();
                     }
-                    tc_commit(&bar_empty[s]);                    // smem stage free once these MMAs have read it
-                    tc_commit(&bar_tfull[acc]);                  // accumulator complete
-                    }
-                    __syncwarp();
                 }
             }
         } else {                                                 // ===== epilogue: one thread per row and column half =====
             const int q = warp & 3, h = (warp - 2) >> 2;
             const int row = row0 + 32 * q + lane;
-            if (DKD_MT_A_TMEM && h == 0) {
-                // The A block goes to TENSOR MEMORY once (row m in lane m, the row's fp16 pairs in D / 2 consecutive 32-bit
-                // columns behind the accumulators): every tcgen05.mma then reads only B through the shared-memory port,
-                // which is what bounds a 128 x 128 single-CTA tile.  Rows past the set read as zeros.
-                const uint32_t* arow = p.a_words + (static_cast<size_t>(pr) * p.Na + (row < p.Na ? row : 0)) * (p.KB * (MT_KBOX / 2));
-                for (int c = 0; c < p.KB * (MT_KBOX / 2); c += 32) {
-                    uint32_t w[32];
-#pragma unroll
-                    for (int j = 0; j < 32; j += 4) {
-                        uint4 t4 = make_uint4(0u, 0u, 0u, 0u);
-                        if (row < p.Na) t4 = __ldg(reinterpret_cast<const uint4*>(arow + c + j));
-                        w[j] = t4.x; w[j + 1] = t4.y; w[j + 2] = t4.z; w[j + 3] = t4.w;
-                    }
-                    tc_st_32x32(tmem + (static_cast<uint32_t>(32 * q) << 16) + MT_ACC_COLS + c, w);
-                }
-                tc_wait_st();
-                tc_fence_before();
-                m_mbar_arrive(&bar_a);                           // 128 arrivals: the whole block is in place
-            }
             float best = -INFINITY, second = -INFINITY;
             int arg = -1;
             for (int t = t0, it = 0; t < t1; ++t, ++it) {
@@ -299,11 +274,11 @@ __global__ void __launch_bounds__(MT_THREADS, 1) k_match_tc(const __grid_constan
                 m_mbar_wait(&bar_tfull[acc], (it >> 1) & 1);
                 tc_fence_after();
 #pragma unroll
-                for (int c = 0; c < 64; c += 32) {
+                for (int c = 0; c < MT_BN / 2; c += 32) {
                     uint32_t v[32];
-                    tc_ld_32x32(tmem + (static_cast<uint32_t>(32 * q) << 16) + acc * MT_BN + 64 * h + c, v);
+                    tc_ld_32x32(tmem + (static_cast<uint32_t>(32 * q) << 16) + acc * MT_BN + (MT_BN / 2) * h + c, v);
                     tc_wait_ld();
-                    const int col0 = t * MT_BN + 64 * h + c;
+                    const int col0 = t * MT_BN + (MT_BN / 2) * h + c;
                     if (col0 + 32 <= nb) {
 #pragma unroll
                         for (int j = 0; j < 32; ++j) {
@@ -630,7 +605,7 @@ bool encode_desc_map(CUtensorMap* m, const void* base, int N, int D, int P) {
     if (!enc) return false;
     const cuuint64_t dims[3] = {(cuuint64_t)D, (cuuint64_t)N, (cuuint64_t)P};
     const cuuint64_t strides[2] = {(cuuint64_t)D * 2, (cuuint64_t)D * 2 * N};
-    const cuuint32_t box[3] = {(cuuint32_t)MT_KBOX, (cuuint32_t)MT_BN, 1};
+    const cuuint32_t box[3] = {(cuuint32_t)MT_KBOX, (cuuint32_t)MT_BOX_ROWS, 1};
     const cuuint32_t estr[3] = {1, 1, 1};
     return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
@@ -652,10 +627,9 @@ cudaError_t launch_match_dir(dkd_ctx* ctx, const void* A, const int32_t* ca, int
     MatchParams mp;
     memset(&mp, 0, sizeof(mp));
     mp.count_a = ca; mp.count_b = cb; mp.Na = Na; mp.Nb = Nb; mp.KB = D / MT_KBOX; mp.splits = splits; mp.part = part;
-    mp.a_words = static_cast<const uint32_t*>(A);
-    const size_t a_bytes = DKD_MT_A_TMEM ? 0 : static_cast<size_t>(mp.KB) * MT_BM * 128, b_bytes = static_cast<size_t>(mp.KB) * MT_BN * 128;
+    const size_t a_bytes = static_cast<size_t>(mp.KB) * MT_BM * 128, b_bytes = static_cast<size_t>(MT_BN) * 128;   // A block, one B unit
     int stages = static_cast<int>((200 * 1024 - a_bytes) / b_bytes);
-    if (stages > 4) stages = 4;
+    if (stages > MT_MAX_STAGES) stages = MT_MAX_STAGES;
     mp.stages = stages;
     const size_t smem = a_bytes + stages * b_bytes + 1024;
     static bool attr_set = false;
