@@ -146,10 +146,11 @@ __device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sy
 //            (best, arg best, second best) in registers — no cross-thread reduction; columns are visited in
 //            increasing order and the comparison is strict, so ties keep the smallest column (M2).
 // Rows >= count_a and columns >= count_b (the zero padding of PAPER.md:139) are masked out.
-constexpr int MT_BM = 128, MT_BN = 256, MT_KBOX = 64;            // KBOX fp16 = 128 bytes = the swizzle span
+constexpr int MT_BM = 128, MT_KBOX = 64;                         // KBOX fp16 = 128 bytes = the swizzle span
+// (the tile width BN = 256 or 128 columns of S is a template parameter: 256-wide MMAs when the problem fills the machine
+// with them — they use the tensor pipe better —, 128 for small sets, where more and smaller CTAs finish sooner)
 constexpr int MT_BOX_ROWS = 128;                                 // rows of one TMA box (A block: one box per k-box; B unit: two)
 constexpr int MT_THREADS = 320;                                  // 10 warps
-constexpr int MT_TMEM_COLS = 2 * MT_BN;                           // two accumulator buffers of 256 fp32 columns = all of TMEM
 constexpr int MT_MAX_STAGES = 8;                                 // ring units of the B stream
 constexpr int MT_MAX_KB = 4;                                     // D <= 256
 
@@ -174,6 +175,7 @@ __device__ __forceinline__ uint64_t mt_desc(uint32_t smem_addr) {
            (1ull << 46) | (2ull << 61);
 }
 
+template <int MT_BN>
 __global__ void __launch_bounds__(MT_THREADS, 1) k_match_tc(const __grid_constant__ CUtensorMap tmap_a,
                                                             const __grid_constant__ CUtensorMap tmap_b,
                                                             const __grid_constant__ MatchParams p) {
@@ -182,6 +184,7 @@ __global__ void __launch_bounds__(MT_THREADS, 1) k_match_tc(const __grid_constan
     __shared__ uint32_t s_tmem;
     __shared__ MatchRec s_half[MT_BM];                           // the upper column half's result of every row
 
+    constexpr int MT_TMEM_COLS = 2 * MT_BN;                      // two accumulator buffers (BN = 256: all of TMEM)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int rb = blockIdx.x, sp = blockIdx.y, pr = blockIdx.z;
     // programmatic dependent launch: the next kernel of the call (the reverse direction, k_match_finalize) may be
@@ -228,7 +231,8 @@ __global__ void __launch_bounds__(MT_THREADS, 1) k_match_tc(const __grid_constan
                         if (iu >= p.stages) m_mbar_wait(&bar_empty[s], ((iu / p.stages) - 1) & 1);
                         m_mbar_expect_tx(&bar_full[s], b_bytes);
                         m_tma_load_3d(smem_b + s * b_bytes, &tmap_b, &bar_full[s], kb * MT_KBOX, t * MT_BN, pr);
-                        m_tma_load_3d(smem_b + s * b_bytes + MT_BOX_ROWS * 128, &tmap_b, &bar_full[s], kb * MT_KBOX, t * MT_BN + MT_BOX_ROWS, pr);
+                        if (MT_BN > MT_BOX_ROWS)
+                            m_tma_load_3d(smem_b + s * b_bytes + MT_BOX_ROWS * 128, &tmap_b, &bar_full[s], kb * MT_KBOX, t * MT_BN + MT_BOX_ROWS, pr);
                     }
                 }
             }
@@ -611,8 +615,14 @@ bool encode_desc_map(CUtensorMap* m, const void* base, int N, int D, int P) {
                CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// tile width: 256 columns when row blocks x pairs x 256-wide tiles fill the machine, else 128
+int match_bn(int num_sms, int Na, int Nb, int P) {
+    const long long work = static_cast<long long>((Na + MT_BM - 1) / MT_BM) * P * ((Nb + 255) / 256);
+    return work >= num_sms ? 256 : 128;
+}
 int match_splits(int num_sms, int Na, int Nb, int P) {
-    const int rbs = (Na + MT_BM - 1) / MT_BM, tiles = (Nb + MT_BN - 1) / MT_BN;
+    const int bn = match_bn(num_sms, Na, Nb, P);
+    const int rbs = (Na + MT_BM - 1) / MT_BM, tiles = (Nb + bn - 1) / bn;
     int s = num_sms / (rbs * P > 0 ? rbs * P : 1);               // fill the machine once
     if (s < 1) s = 1;
     if (s > tiles) s = tiles;
@@ -627,21 +637,23 @@ cudaError_t launch_match_dir(dkd_ctx* ctx, const void* A, const int32_t* ca, int
     MatchParams mp;
     memset(&mp, 0, sizeof(mp));
     mp.count_a = ca; mp.count_b = cb; mp.Na = Na; mp.Nb = Nb; mp.KB = D / MT_KBOX; mp.splits = splits; mp.part = part;
-    const size_t a_bytes = static_cast<size_t>(mp.KB) * MT_BM * 128, b_bytes = static_cast<size_t>(MT_BN) * 128;   // A block, one B unit
+    const int bn = match_bn(dkd_ctx_num_sms(ctx), Na, Nb, P);
+    const size_t a_bytes = static_cast<size_t>(mp.KB) * MT_BM * 128, b_bytes = static_cast<size_t>(bn) * 128;   // A block, one B unit
     int stages = static_cast<int>((200 * 1024 - a_bytes) / b_bytes);
     if (stages > MT_MAX_STAGES) stages = MT_MAX_STAGES;
     mp.stages = stages;
     const size_t smem = a_bytes + stages * b_bytes + 1024;
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(k_match_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, 204 * 1024);   // (static smem takes ~3 KB of the 227)
+        cudaError_t e = cudaFuncSetAttribute(k_match_tc<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 204 * 1024);   // (static smem takes ~3 KB of the 227)
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_match_tc<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, 204 * 1024);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    (void)ctx;
     const dim3 grid((Na + MT_BM - 1) / MT_BM, splits, P);
     KLaunch k;
-    prep(k, k_match_tc, grid, dim3(MT_THREADS), smem, pdl, ta, tb, mp);
+    if (bn == 256) prep(k, k_match_tc<256>, grid, dim3(MT_THREADS), smem, pdl, ta, tb, mp);
+    else prep(k, k_match_tc<128>, grid, dim3(MT_THREADS), smem, pdl, ta, tb, mp);
     return launch(k, st, true);
 }
 
