@@ -100,18 +100,6 @@ __device__ __forceinline__ void tc_ld_32x32(uint32_t taddr, uint32_t (&v)[32]) {
         : "r"(taddr)
         : "memory");
 }
-// thread t of the warp writes row (lane base + t), columns c .. c+31 (the mirror of tc_ld_32x32)
-__device__ __forceinline__ void tc_st_32x32(uint32_t taddr, const uint32_t (&v)[32]) {
-    asm volatile(
-        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
-        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
-        "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};"
-        ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]),
-          "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]), "r"(v[16]), "r"(v[17]),
-          "r"(v[18]), "r"(v[19]), "r"(v[20]), "r"(v[21]), "r"(v[22]), "r"(v[23]), "r"(v[24]), "r"(v[25]), "r"(v[26]),
-          "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31])
-        : "memory");
-}
 // true in exactly one lane of a converged warp; the compiler then knows the guarded code runs in a single thread and emits
 // the uniform-register instructions (UTCHMMA, UTMALDG) without a per-lane election loop around each of them
 __device__ __forceinline__ bool elect_one() {
@@ -119,30 +107,17 @@ __device__ __forceinline__ bool elect_one() {
     asm volatile("{\n.reg .pred P;\nelect.sync _|P, 0xffffffff;\nselp.u32 %0, 1, 0, P;\n}" : "=r"(pred));
     return pred != 0;
 }
-__device__ __forceinline__ void tc_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
-// D[tmem] (+)= A[tmem] * B[smem desc]^T: the A operand read from tensor memory (row m in lane m, fp16 pairs packed in
-// 32-bit columns), so that only B crosses the shared-memory port
-__device__ __forceinline__ void tc_mma_f16_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t desc_b, uint32_t idesc, uint32_t accumulate) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "setp.ne.b32 p, %4, 0;\n"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n"
-        "}" ::"r"(tmem_d),
-        "r"(tmem_a), "l"(desc_b), "r"(idesc), "r"(accumulate)
-        : "memory");
-}
 __device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 // ---- k_match_tc -------------------------------------------------------------------------------------------
-// One CTA = one block of BM = 128 rows of A (one pair p) against the column tiles [t0, t1) of B.
-//   warp 0   TMA producer: the A block once (KB boxes of 64 k-elements x 128 rows, 128-byte swizzle), then one
-//            B tile (BN = 128 rows, all of K) per ring stage;
-//   warp 1   allocates TMEM and issues the MMAs: per B tile KB x 4 tcgen05.mma of 128 x 128 x 16 into one of two
-//            accumulator buffers (128 lanes x 128 fp32 columns each); tcgen05.commit frees the smem stage and
-//            publishes the accumulator;
-//   warps 2..9  epilogue: warp w reads TMEM lanes 32 (w % 4) .. +31 (the hardware's lane quadrant of the warp),
-//            columns 64 h .. 64 h + 63 with h = (w - 2) / 4: every thread owns ONE ROW of S and keeps its running
+// One CTA = one block of BM = 128 rows of A (one pair p) against the column tiles [t0, t1) of B, BN = 256 or 128 columns each.
+//   warp 0   TMA producer: the A block once (KB boxes of 64 k-elements x 128 rows, 128-byte swizzle), then the B stream in
+//            ring UNITS of one k-box (BN rows x 128 bytes: BN / 128 boxes one below the other = one N = BN operand);
+//   warp 1   allocates TMEM and, one elect.sync lane of the converged warp, issues the MMAs: per unit 4 tcgen05.mma of
+//            128 x BN x 16 into one of two accumulator buffers (128 lanes x BN fp32 columns each); tcgen05.commit frees the
+//            unit's shared memory, and after the tile's last unit publishes the accumulator;
+//   warps 2..9  epilogue: warp w reads TMEM lanes 32 (w % 4) .. +31 (the hardware's lane quadrant of the warp), the
+//            column half h = (w - 2) / 4 of the tile: every thread owns ONE ROW of S and keeps its running
 //            (best, arg best, second best) in registers — no cross-thread reduction; columns are visited in
 //            increasing order and the comparison is strict, so ties keep the smallest column (M2).
 // Rows >= count_a and columns >= count_b (the zero padding of PAPER.md:139) are masked out.
