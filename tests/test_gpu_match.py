@@ -86,6 +86,30 @@ def test_match_small_and_ragged(ctx, D, shape, mutual):
     assert (dec >= 0).sum() > 0.3 * min(Na, Nb)                   # the planted matches are found
 
 
+@pytest.mark.parametrize("D", [64, 192, 256])
+@pytest.mark.parametrize("mutual", [False, True])
+def test_match_wide_tiles_ragged(ctx, D, mutual):
+    """Sizes at which the kernel takes its 256-column tiles (row blocks x pairs x 256-wide tiles fill the machine) with
+    set sizes that are multiples of neither 128 nor 256 and ragged counts; ~160 rows per pair (tile edges + a random sample)
+    checked against the oracle over every column."""
+    Na, Nb = 1300, 2100
+    ca, cb = [Na - 17, Na], [Nb, Nb - 333]
+    A, B, cta, ctb = synth.match_sets(2, Na, Nb, D, seed=D + int(mutual), count_a=ca, count_b=cb)
+    Ad, Bd, cad, cbd = A.cuda(), B.cuda(), cta.cuda(), ctb.cuda()
+    nn, nsim = ctx.match(Ad, Bd, cad, cbd, ratio=1e9, mutual=False)
+    dec, _ = ctx.match(Ad, Bd, cad, cbd, ratio=0.8, mutual=mutual)
+    torch.cuda.synchronize()
+    amb = tot = 0
+    g = np.random.default_rng(D)
+    for p in range(2):
+        rows = np.unique(np.concatenate([g.choice(ca[p], 150, replace=False), [0, 127, 128, 255, 256, 1279, 1280, ca[p] - 1, Na - 1]]))
+        a, n = check_pair(A[p].numpy(), B[p].numpy(), ca[p], cb[p], 0.8, mutual, nn[p].cpu().numpy(), nsim[p].cpu().numpy(),
+                          dec[p].cpu().numpy(), rows=rows)
+        amb, tot = amb + a, tot + n
+    assert amb <= 0.03 * tot + 2
+    assert (dec >= 0).sum() > 0.3 * min(Na, Nb)
+
+
 def test_match_planted_exact_cases(ctx):
     D = 64
     E = torch.eye(D, dtype=torch.float16)

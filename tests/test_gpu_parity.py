@@ -204,7 +204,7 @@ def test_random_sweep_and_worst_cases_under_the_debug_build():
     sel = "random_shapes or worst_case or many_candidates or units_of_several or small_multitile or ties_at_clamp or back_to_back"
     r = subprocess.run([sys.executable, "-m", "pytest", "tests/test_gpu_parity.py", "tests/test_gpu_variants.py",
                         "tests/test_gpu_match.py", "-q", "-x", "-m", "gpu", "-k",
-                        "(" + sel + " or reliability or validity or retrieval or match_small) and not debug_build"],
+                        "(" + sel + " or reliability or validity or retrieval or match_small or wide_tiles) and not debug_build"],
                        cwd=root, env=env, capture_output=True, text=True, timeout=1500)
     assert r.returncode == 0, r.stdout[-3000:] + r.stderr[-2000:]
     assert "DKD_DEBUG" in subprocess.run([sys.executable, "-c", "import paper_2607_01757_b200 as d, ctypes; L = d.load_library(); "
