@@ -280,6 +280,47 @@ int dkd_match(dkd_ctx* ctx, const void* desc_a, const int32_t* count_a, int Na,
               float ratio, int mutual, int32_t* out_match, float* out_sim, void* stream);
 
 /*
+ * dkd_match_static — dkd_match for callers that are not allowed to allocate device memory.
+ *
+ * Who this is for: code that runs where cudaMalloc / cudaFree are off limits — a plug-in living inside a host
+ * application that hands out a fixed device-memory budget and forbids allocations of its own (an inference-server
+ * back-end, a ROS 2 component under a real-time executor: cudaMalloc takes a driver lock and may stall the whole
+ * device for milliseconds), a process whose memory pool has already claimed the entire GPU so that a further
+ * cudaMalloc simply fails, or a hard real-time loop in which any call of unbounded duration is banned.  Such a
+ * caller cannot use dkd_create (it allocates the workspace) and therefore none of the dkd_ctx entry points.  This one
+ * takes no context and calls neither cudaMalloc nor cudaFree nor any library routine that allocates: the one piece
+ * of scratch memory the matcher needs — the per-column-split partial results that k_match_tc hands to
+ * k_match_finalize — is a fixed-size array that is part of the library image itself.
+ *
+ * The limit: that array holds DKD_MATCH_STATIC_MAX_RECS records of 16 bytes = 1 MiB.  It is claimed on every GPU
+ * on which this library's code is loaded, whether or not this function is ever called there, and is given back only
+ * when the process exits.  A call needs  P * splits(Na,Nb) * Na  records, plus  P * splits(Nb,Na) * Nb  when
+ * mutual != 0, where splits (1..16) is how many CTAs share the columns of one row block so that the grid fills the
+ * GPU once.  Two pairs of 4096 x 4096 with the mutual check need 32768 records on a 148-SM part; a call that needs
+ * more than the array holds returns DKD_ERR_CAPACITY, launches nothing, and says both numbers in `err`.
+ *
+ * Arguments, results, tie rules and alignment requirements are exactly those of dkd_match (see above); the results
+ * are bit-identical to dkd_match on the same inputs.  Differences:
+ *   - no ctx: the call runs on the calling thread's CURRENT device; every pointer and `stream` must belong to it;
+ *   - err / err_len: optional caller-owned host buffer that receives the message of a failure (NUL-terminated,
+ *     truncated to err_len; empty on success); NULL / 0 = no message wanted;
+ *   - the first call on each device does a one-time set-up on that device (it looks up the device address of the
+ *     built-in array, reads the SM count, raises the matcher's shared-memory limit).  Make that first call during
+ *     start-up, on a stream that is not being captured; later calls on that device only launch kernels;
+ *   - every call on a device shares the one array, and the array keeps what the previous call left in it.  Nothing
+ *     in it needs to start at zero (each call overwrites every record it later reads), but two calls whose kernels
+ *     can be on the GPU at the same time — different streams, or the same stream from two threads without ordering —
+ *     overwrite each other's partials and return garbage.  Keep all calls on one device on one stream, or order
+ *     them with events.
+ * Asynchronous on `stream` (up to three kernel launches).
+ */
+#define DKD_MATCH_STATIC_MAX_RECS 65536
+int dkd_match_static(const void* desc_a, const int32_t* count_a, int Na,
+                     const void* desc_b, const int32_t* count_b, int Nb, int D, int dtype, int P,
+                     float ratio, int mutual, int32_t* out_match, float* out_sim, void* stream,
+                     char* err, int err_len);
+
+/*
  * dkd_retrieval_scan — brute-force loop-candidate retrieval ("cosine similarity between the current
  * descriptor g_t and a past descriptor g_k", Eq. 4; "a fixed window of the most recent keyframes is excluded";
  * "Candidates with sim > tau_sim are ranked by similarity"; "brute-force scan over the keyframe database, O(n)";

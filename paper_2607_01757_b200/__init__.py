@@ -6,8 +6,8 @@ PyTorch is used for device memory and streams.  There is no CPU fallback: import
 anywhere, but creating a context without the library or without a CUDA device raises.
 """
 from .binding import (DKD, DKDError, DKDResult, F16, F32, lib_path, load_library,  # noqa: F401
-                      EXPORTED_SYMBOLS)
+                      EXPORTED_SYMBOLS, MATCH_STATIC_MAX_RECS, match_static)
 from .sharding import shard_range, sharded_extract  # noqa: F401
 
 __all__ = ["DKD", "DKDError", "DKDResult", "F16", "F32", "lib_path", "load_library",
-           "EXPORTED_SYMBOLS", "shard_range", "sharded_extract"]
+           "EXPORTED_SYMBOLS", "MATCH_STATIC_MAX_RECS", "match_static", "shard_range", "sharded_extract"]

@@ -19,7 +19,7 @@ EXPORTED_SYMBOLS = (
     "dkd_create", "dkd_destroy", "dkd_last_error", "dkd_workspace_bytes", "dkd_set_option",
     "dkd_extract", "dkd_extract_ex", "dkd_extract_var", "dkd_extract_host", "dkd_launches_per_extract", "dkd_version",
     "dkd_profile_read", "dkd_kernel_name", "dkd_pre_padded_size", "dkd_preprocess", "dkd_graph_stats",
-    "dkd_match", "dkd_retrieval_scan", "dkd_stereo_validate", "dkd_cov_sqrt_info",
+    "dkd_match", "dkd_match_static", "dkd_retrieval_scan", "dkd_stereo_validate", "dkd_cov_sqrt_info",
 )
 
 
@@ -104,6 +104,8 @@ def load_library():
     L.dkd_extract_var.argtypes = common + [vp, vp, ctypes.POINTER(_VariantParams), vp]
     L.dkd_match.restype = i
     L.dkd_match.argtypes = [vp, vp, vp, i, vp, vp, i, i, i, i, f, i, vp, vp, vp]
+    L.dkd_match_static.restype = i
+    L.dkd_match_static.argtypes = [vp, vp, i, vp, vp, i, i, i, i, f, i, vp, vp, vp, ctypes.c_char_p, i]
     L.dkd_retrieval_scan.restype = i
     L.dkd_retrieval_scan.argtypes = [vp, vp, i, i, i, vp, i, f, i, vp, vp, vp, vp, vp]
     L.dkd_stereo_validate.restype = i
@@ -140,6 +142,45 @@ def _dt(t: Optional[torch.Tensor]) -> int:
 
 def _ptr(t: Optional[torch.Tensor]):
     return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+MATCH_STATIC_MAX_RECS = 65536
+
+
+def match_static(desc_a: torch.Tensor, desc_b: torch.Tensor, out_match: torch.Tensor,
+                 out_sim: Optional[torch.Tensor] = None, count_a: Optional[torch.Tensor] = None,
+                 count_b: Optional[torch.Tensor] = None, ratio: float = 0.8, mutual: bool = False, stream=None) -> None:
+    """dkd_match_static: the matcher for callers that may not allocate device memory (no context; the scratch is a
+    1 MiB array built into the library, shared by all calls on a device — keep them on one stream).  Nothing is
+    allocated here either: the caller passes the outputs.  desc_a [P,Na,D], desc_b [P,Nb,D] f16 cuda contiguous;
+    out_match [P,Na] i32, out_sim [P,Na,2] f32 or None; counts [P] i32 cuda or None.  Runs on desc_a's device, on
+    torch's current stream of that device unless `stream` is given.  Raises DKDError (code -3: the problem needs
+    more than MATCH_STATIC_MAX_RECS partial records)."""
+    L = load_library()
+    for t in (desc_a, desc_b):
+        if not (t.is_cuda and t.is_contiguous() and t.dim() == 3):
+            raise DKDError(-1, "descriptor sets must be contiguous CUDA [P,N,D] tensors")
+    P, Na, D = desc_a.shape
+    Nb = desc_b.shape[1]
+    if desc_b.shape[0] != P or desc_b.shape[2] != D or desc_a.dtype != desc_b.dtype or desc_b.device != desc_a.device:
+        raise DKDError(-1, "desc_a / desc_b disagree in P, D, dtype or device")
+    for c in (count_a, count_b):
+        if c is not None and not (c.device == desc_a.device and c.dtype == torch.int32 and c.is_contiguous() and c.numel() == P):
+            raise DKDError(-1, "counts must be contiguous CUDA int32 [P] tensors")
+    if not (out_match.device == desc_a.device and out_match.dtype == torch.int32 and out_match.is_contiguous()
+            and tuple(out_match.shape) == (P, Na)):
+        raise DKDError(-1, "out_match must be a contiguous CUDA int32 [P,Na] tensor")
+    if out_sim is not None and not (out_sim.device == desc_a.device and out_sim.dtype == torch.float32
+                                    and out_sim.is_contiguous() and tuple(out_sim.shape) == (P, Na, 2)):
+        raise DKDError(-1, "out_sim must be a contiguous CUDA float32 [P,Na,2] tensor")
+    err = ctypes.create_string_buffer(256)
+    with torch.cuda.device(desc_a.device):                       # the entry point runs on the current device
+        st = torch.cuda.current_stream(desc_a.device) if stream is None else stream
+        rc = L.dkd_match_static(_ptr(desc_a), _ptr(count_a), Na, _ptr(desc_b), _ptr(count_b), Nb, D, _dt(desc_a), P,
+                                float(ratio), int(bool(mutual)), _ptr(out_match), _ptr(out_sim),
+                                ctypes.c_void_p(st.cuda_stream), err, len(err))
+    if rc != 0:
+        raise DKDError(rc, err.value.decode(errors="replace"))
 
 
 class DKD:

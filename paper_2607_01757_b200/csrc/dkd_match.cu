@@ -14,7 +14,10 @@
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdint.h>
+#include <stdio.h>
 #include <string.h>
+
+#include <mutex>
 
 #include "dkd.h"
 #include "dkd_host.h"
@@ -632,6 +635,72 @@ cudaError_t launch_match_dir(dkd_ctx* ctx, const void* A, const int32_t* ca, int
     return launch(k, st, true);
 }
 
+// ---- dkd_match_static: the matcher with its partials in memory that is part of the loaded library ---------------------
+// The column-split partials of k_match_tc normally live in a context-owned buffer that dkd_create / dkd_match obtain
+// with cudaMalloc.  This array is the same buffer as a file-scope device variable: it comes into existence when the
+// library's module is loaded on a GPU and stays until the process exits (1 MiB on every GPU that loads the library).
+constexpr size_t MT_STATIC_RECS = DKD_MATCH_STATIC_MAX_RECS;
+static __device__ __align__(256) MatchRec g_match_static[MT_STATIC_RECS];
+
+// `g_match_static` named in HOST code is only the host-side handle of the variable, not an address the GPU can use;
+// the device address is asked for once per device (with that device current) and kept here with the SM count.
+constexpr int MT_STATIC_MAX_DEVICES = 64;
+struct MatchStaticDev {
+    MatchRec* part;                    // device address of g_match_static on this device
+    int num_sms;
+    bool ready;
+};
+static MatchStaticDev g_ms_dev[MT_STATIC_MAX_DEVICES];
+static std::mutex g_ms_mutex;
+
+// set-up of the current device `dev` (first call on it): symbol address, SM count, shared-memory limits of k_match_tc
+cudaError_t match_static_setup(int dev, MatchStaticDev* out) {
+    std::lock_guard<std::mutex> lk(g_ms_mutex);
+    MatchStaticDev& d = g_ms_dev[dev];
+    if (!d.ready) {
+        void* ptr = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&ptr, g_match_static);
+        if (e != cudaSuccess) return e;
+        int sms = 0;
+        e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(k_match_tc<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 204 * 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_match_tc<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, 204 * 1024);
+        if (e != cudaSuccess) return e;
+        d.part = static_cast<MatchRec*>(ptr);
+        d.num_sms = sms;
+        d.ready = true;
+    }
+    *out = d;
+    return cudaSuccess;
+}
+
+// one direction of the match (the geometry of launch_match_dir, with the SM count passed in and no attribute calls)
+cudaError_t launch_match_static_dir(int num_sms, const void* A, const int32_t* ca, int Na, const void* B, const int32_t* cb, int Nb,
+                                    int D, int P, int splits, MatchRec* part, cudaStream_t st, bool pdl) {
+    CUtensorMap ta, tb;
+    if (!encode_desc_map(&ta, A, Na, D, P) || !encode_desc_map(&tb, B, Nb, D, P)) return cudaErrorInvalidValue;
+    MatchParams mp;
+    memset(&mp, 0, sizeof(mp));
+    mp.count_a = ca; mp.count_b = cb; mp.Na = Na; mp.Nb = Nb; mp.KB = D / MT_KBOX; mp.splits = splits; mp.part = part;
+    const int bn = match_bn(num_sms, Na, Nb, P);
+    const size_t a_bytes = static_cast<size_t>(mp.KB) * MT_BM * 128, b_bytes = static_cast<size_t>(bn) * 128;
+    int stages = static_cast<int>((200 * 1024 - a_bytes) / b_bytes);
+    if (stages > MT_MAX_STAGES) stages = MT_MAX_STAGES;
+    mp.stages = stages;
+    const size_t smem = a_bytes + stages * b_bytes + 1024;
+    const dim3 grid((Na + MT_BM - 1) / MT_BM, splits, P);
+    KLaunch k;
+    if (bn == 256) prep(k, k_match_tc<256>, grid, dim3(MT_THREADS), smem, pdl, ta, tb, mp);
+    else prep(k, k_match_tc<128>, grid, dim3(MT_THREADS), smem, pdl, ta, tb, mp);
+    return launch(k, st, true);
+}
+
+int match_static_fail(char* err, int err_len, int code, const char* msg, const char* detail) {
+    if (err && err_len > 0) snprintf(err, static_cast<size_t>(err_len), "%s%s", msg, detail ? detail : "");
+    return code;
+}
+
 }  // namespace dkd
 
 using namespace dkd;
@@ -671,6 +740,54 @@ int dkd_match(dkd_ctx* ctx, const void* desc_a, const int32_t* count_a, int Na, 
         e = launch(k, st, true);
     }
     if (e != cudaSuccess) return dkd_ctx_fail(ctx, DKD_ERR_CUDA, "k_match_finalize launch: ", cudaGetErrorString(e));
+    return DKD_OK;
+}
+
+int dkd_match_static(const void* desc_a, const int32_t* count_a, int Na, const void* desc_b, const int32_t* count_b, int Nb,
+                     int D, int dtype, int P, float ratio, int mutual, int32_t* out_match, float* out_sim, void* stream,
+                     char* err, int err_len) {
+    if (err && err_len > 0) err[0] = '\0';
+    if (!desc_a || !desc_b || !out_match || Na < 1 || Nb < 1 || D < 1 || P < 1 || !(ratio > 0.0f))
+        return match_static_fail(err, err_len, DKD_ERR_INVALID_ARG, "dkd_match_static: NULL pointer, size < 1 or ratio <= 0", nullptr);
+    if (dtype != DKD_F16)
+        return match_static_fail(err, err_len, DKD_ERR_UNSUPPORTED, "dkd_match_static: descriptors must be DKD_F16", nullptr);
+    if (D % MT_KBOX != 0 || D > MT_KBOX * MT_MAX_KB)
+        return match_static_fail(err, err_len, DKD_ERR_UNSUPPORTED, "dkd_match_static: D must be 64, 128, 192 or 256", nullptr);
+    if (P > 65535) return match_static_fail(err, err_len, DKD_ERR_UNSUPPORTED, "dkd_match_static: P > 65535", nullptr);
+    if ((reinterpret_cast<uintptr_t>(desc_a) & 15) || (reinterpret_cast<uintptr_t>(desc_b) & 15))
+        return match_static_fail(err, err_len, DKD_ERR_UNSUPPORTED, "dkd_match_static: descriptor sets not 16-byte aligned", nullptr);
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return match_static_fail(err, err_len, DKD_ERR_CUDA, "dkd_match_static: cudaGetDevice: ", cudaGetErrorString(e));
+    if (dev < 0 || dev >= MT_STATIC_MAX_DEVICES)
+        return match_static_fail(err, err_len, DKD_ERR_UNSUPPORTED, "dkd_match_static: device ordinal above 63", nullptr);
+    MatchStaticDev d;
+    e = match_static_setup(dev, &d);
+    if (e != cudaSuccess) return match_static_fail(err, err_len, DKD_ERR_CUDA, "dkd_match_static: device set-up: ", cudaGetErrorString(e));
+    const int s_ab = match_splits(d.num_sms, Na, Nb, P), s_ba = mutual ? match_splits(d.num_sms, Nb, Na, P) : 0;
+    const size_t n_ab = static_cast<size_t>(P) * s_ab * Na, n_ba = static_cast<size_t>(P) * s_ba * Nb;
+    if (n_ab + n_ba > MT_STATIC_RECS) {
+        char buf[160];
+        snprintf(buf, sizeof(buf), "needs %zu partial records (P x column splits x rows, both directions if mutual), the built-in buffer holds %zu",
+                 n_ab + n_ba, MT_STATIC_RECS);
+        return match_static_fail(err, err_len, DKD_ERR_CAPACITY, "dkd_match_static: problem too large: ", buf);
+    }
+    // Nothing in the buffer has to be cleared: every record k_match_finalize reads (rows < Na of every split and pair,
+    // rows < Nb of the reverse direction) is written by k_match_tc earlier in this same call.
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    MatchRec* part = d.part;
+    e = launch_match_static_dir(d.num_sms, desc_a, count_a, Na, desc_b, count_b, Nb, D, P, s_ab, part, st, false);
+    if (e == cudaSuccess && mutual)
+        e = launch_match_static_dir(d.num_sms, desc_b, count_b, Nb, desc_a, count_a, Na, D, P, s_ba, part + n_ab, st, true);
+    if (e != cudaSuccess) return match_static_fail(err, err_len, DKD_ERR_CUDA, "dkd_match_static: k_match_tc launch: ", cudaGetErrorString(e));
+    FinalizeParams fp;
+    memset(&fp, 0, sizeof(fp));
+    fp.part = part; fp.rpart = mutual ? part + n_ab : nullptr; fp.count_a = count_a; fp.Na = Na; fp.Nb = Nb; fp.splits = s_ab;
+    fp.rsplits = s_ba; fp.P = P; fp.ratio2 = ratio >= 1e9f ? -1.0f : ratio * ratio; fp.out_match = out_match; fp.out_sim = out_sim;
+    KLaunch k;
+    prep(k, k_match_finalize, dim3((Na + 255) / 256, P), dim3(256), 0, true, fp);
+    e = launch(k, st, true);
+    if (e != cudaSuccess) return match_static_fail(err, err_len, DKD_ERR_CUDA, "dkd_match_static: k_match_finalize launch: ", cudaGetErrorString(e));
     return DKD_OK;
 }
 
