@@ -273,7 +273,10 @@ int dkd_preprocess(dkd_ctx* ctx, const uint8_t* src, int B, int H, int W, const 
  *   D        64, 128, 192 or 256; dtype must be DKD_F16 (else DKD_ERR_UNSUPPORTED)
  *   out_match device [P,Na] i32: j1 or -1 (no match / padding row);  out_sim device [P,Na,2] f32 (s1, s2) or NULL
  * Asynchronous on `stream`.  Uses a context-owned scratch buffer that is grown (cudaMalloc) when a call needs more than
- * any call before it: such a call must not be made while `stream` is being captured.
+ * any call before it: such a call must not be made while `stream` is being captured.  The buffer holds the partial results
+ * between the kernels of ONE call: a context must be used from one stream at a time (calls of dkd_match /
+ * dkd_retrieval_scan on the same context whose kernels could overlap on the GPU overwrite each other's partials; use
+ * one context per stream, or order the streams with events).
  */
 int dkd_match(dkd_ctx* ctx, const void* desc_a, const int32_t* count_a, int Na,
               const void* desc_b, const int32_t* count_b, int Nb, int D, int dtype, int P,

@@ -102,6 +102,7 @@ struct dkd_ctx {
     int* tile_cnt;           // [max_tiles] keys in each segment
     int32_t* sel_idx;        // [max_batch * max_top_k]
     size_t max_tiles;
+    size_t max_segs;         // ints in tile_cnt: max_tiles, or the tile count of the finest iterated-NMS tiling if larger
     size_t ws_bytes;
     // host-path staging (device), grown on demand
     void* st_score; size_t st_score_bytes;
@@ -368,7 +369,7 @@ int validate_shapes(dkd_ctx* ctx, const ExtractArgs& a) {
         if (halo > 40) return fail(ctx, DKD_ERR_UNSUPPORTED, "iterated NMS: (2 nms_iters + 1) r must be <= 40");
         const int T = (IT_REG - 2 * static_cast<int>(halo)) & ~7;
         const long long tiles = static_cast<long long>((a.W + T - 1) / T) * ((a.H + T - 1) / T) * a.B;
-        if (tiles * T * T > static_cast<long long>(ctx->max_tiles) * SEG_CAP)
+        if (tiles * T * T > static_cast<long long>(ctx->max_tiles) * SEG_CAP || tiles > static_cast<long long>(ctx->max_segs))
             return fail(ctx, DKD_ERR_CAPACITY, "iterated NMS: candidate workspace too small for these tiles (raise the dkd_create maxima)");
     }
     if (a.B > 65535) return fail(ctx, DKD_ERR_UNSUPPORTED, "B > 65535");
@@ -510,13 +511,21 @@ int run(dkd_ctx* ctx, ExtractArgs a, cudaStream_t st) {
     }
     ++ctx->tick;
     const ShapeKey key = shape_key(ctx, a);
-    for (auto& g : ctx->graphs) {
+    for (size_t gi = 0; gi < ctx->graphs.size(); ++gi) {
+        GraphEntry& g = ctx->graphs[gi];
         if (!(g.key == key)) continue;
         g.last_use = ctx->tick;
         if (!same_values(g.last, a)) {                      // other buffers / thresh / T: update the kernel nodes in place
             CK(ctx, build_plan(ctx, a, pl));
             if (g.n_nodes != pl.n || update_graph(g, pl) != cudaSuccess) {
-                (void)cudaGetLastError();                   // cannot update: plain PDL-linked launches, the graph stays as it is
+                // Cannot update.  The nodes are updated one by one, so the exec may now mix the new buffers with the old
+                // ones: drop the entry (rebuilt by the next call of this shape; an exec still in flight is freed when it
+                // completes) and serve this call with plain PDL-linked launches.
+                (void)cudaGetLastError();
+                cudaGraphExecDestroy(g.exec);
+                cudaGraphDestroy(g.graph);
+                ctx->graphs[gi] = ctx->graphs.back();
+                ctx->graphs.pop_back();
                 CK(ctx, enqueue(ctx, pl, st));
                 ++ctx->n_stream;
                 return DKD_OK;
@@ -693,10 +702,15 @@ int dkd_create(const dkd_create_params* p, dkd_ctx** out) {
     CKC(setup_nms<4>(ctx));
     CKC(cudaFuncSetAttribute(k_select, cudaFuncAttributeMaxDynamicSharedMemorySize, SEL_SMEM_BYTES));
     CKC(cudaFuncSetAttribute(k_nms_iter, cudaFuncAttributeMaxDynamicSharedMemorySize, IT_SMEM_BYTES));
+    CKC(dkd_match_setup_device());
     const size_t tx = (p->max_w + STRIP_W - 1) / STRIP_W, ty = (p->max_h + TH - 1) / TH;
     ctx->max_tiles = tx * (ty + MAX_CPU - 1) * p->max_batch;   // segments of whole units: up to MAX_CPU-1 spare strip-tiles per strip
     const size_t b_cand = align256(ctx->max_tiles * SEG_CAP * sizeof(uint64_t));
-    const size_t b_cnt = align256(ctx->max_tiles * sizeof(int));
+    // k_nms_iter writes one count per T x T tile; its smallest tile (halo 40) gives more tiles than there are NMS units
+    const size_t it_t_min = (IT_REG - 2 * 40) & ~7;
+    const size_t it_tiles = ((p->max_w + it_t_min - 1) / it_t_min) * ((p->max_h + it_t_min - 1) / it_t_min) * p->max_batch;
+    ctx->max_segs = ctx->max_tiles > it_tiles ? ctx->max_tiles : it_tiles;
+    const size_t b_cnt = align256(ctx->max_segs * sizeof(int));
     const size_t b_sel = align256(static_cast<size_t>(p->max_batch) * p->max_top_k * sizeof(int32_t));
     CKC(cudaStreamCreateWithFlags(&ctx->cap_stream, cudaStreamNonBlocking));
     for (int i = 0; i <= MAX_KERNELS; ++i) CKC(cudaEventCreate(&ctx->prof_ev[i]));

@@ -30,10 +30,19 @@ struct KLaunch {
     }
 };
 
+// bytes the argument values of a kernel take in KLaunch::blob (each at its natural alignment, in order)
+template <typename... T>
+constexpr size_t packed_arg_bytes() {
+    size_t o = 0;
+    ((o = ((o + alignof(T) - 1) & ~(alignof(T) - 1)) + sizeof(T)), ...);
+    return o;
+}
+
 template <typename... KArgs, typename... Args>
 inline void prep(KLaunch& k, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, bool pdl, Args... args) {
     static_assert(sizeof...(KArgs) == sizeof...(Args), "argument count");
     static_assert(sizeof...(KArgs) <= KLaunch::MAX_ARGS, "too many kernel arguments");
+    static_assert(packed_arg_bytes<KArgs...>() <= KLaunch::BLOB_BYTES, "kernel arguments do not fit KLaunch::blob");
     k.func = reinterpret_cast<const void*>(kern);
     k.grid = grid; k.block = block; k.smem = smem; k.pdl = pdl; k.nargs = 0;
     size_t o = 0;
@@ -45,7 +54,6 @@ inline void prep(KLaunch& k, void (*kern)(KArgs...), dim3 grid, dim3 block, size
         o += sizeof(T);
     };
     (put(static_cast<KArgs>(args)), ...);
-    if (o > KLaunch::BLOB_BYTES) k.func = nullptr;           // (cannot happen: checked per kernel below)
 }
 
 // allow_pdl = false strips the programmatic attribute (measurement mode)
@@ -87,6 +95,8 @@ int dkd_ctx_fail(dkd_ctx* ctx, int code, const char* msg, const char* detail);  
 // context-owned device scratch buffer `slot` (0: match partials, 1: retrieval scan) of at least `bytes` bytes, grown
 // with cudaMalloc when too small (not capture-safe then); NULL on failure (dkd_last_error set)
 void* dkd_ctx_scratch(dkd_ctx* ctx, int slot, size_t bytes);
+// shared-memory limits of k_match_tc / k_scan on the CURRENT device (dkd_match.cu); dkd_create calls it per context
+cudaError_t dkd_match_setup_device();
 // k_select on caller-provided candidate segments (one "image"): ranks the keys of `tpi` segments of `seg_cap` keys by
 // (score desc, index asc) into sel_idx[top_k] (-1 padded) and out_count[1]; n_items bounds the indices
 int dkd_internal_select(dkd_ctx* ctx, const uint64_t* cand, const int* seg_cnt, int tpi, int seg_cap, int top_k, int n_items,

@@ -608,26 +608,22 @@ int match_splits(int num_sms, int Na, int Nb, int P) {
     return s;
 }
 
-cudaError_t launch_match_dir(dkd_ctx* ctx, const void* A, const int32_t* ca, int Na, const void* B, const int32_t* cb, int Nb, int D,
+// One direction of the match.  The first direction of a call must be launched with pdl = false: k_match_tc reads the
+// counts and issues its TMA loads BEFORE its griddepcontrol.wait (which sits at the kernel's end), so only a launch that
+// read nothing its predecessor wrote — the reverse direction — may carry the programmatic attribute.
+cudaError_t launch_match_dir(int num_sms, const void* A, const int32_t* ca, int Na, const void* B, const int32_t* cb, int Nb, int D,
                              int P, int splits, MatchRec* part, cudaStream_t st, bool pdl) {
     CUtensorMap ta, tb;
     if (!encode_desc_map(&ta, A, Na, D, P) || !encode_desc_map(&tb, B, Nb, D, P)) return cudaErrorInvalidValue;
     MatchParams mp;
     memset(&mp, 0, sizeof(mp));
     mp.count_a = ca; mp.count_b = cb; mp.Na = Na; mp.Nb = Nb; mp.KB = D / MT_KBOX; mp.splits = splits; mp.part = part;
-    const int bn = match_bn(dkd_ctx_num_sms(ctx), Na, Nb, P);
+    const int bn = match_bn(num_sms, Na, Nb, P);
     const size_t a_bytes = static_cast<size_t>(mp.KB) * MT_BM * 128, b_bytes = static_cast<size_t>(bn) * 128;   // A block, one B unit
     int stages = static_cast<int>((200 * 1024 - a_bytes) / b_bytes);
     if (stages > MT_MAX_STAGES) stages = MT_MAX_STAGES;
     mp.stages = stages;
     const size_t smem = a_bytes + stages * b_bytes + 1024;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(k_match_tc<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 204 * 1024);   // (static smem takes ~3 KB of the 227)
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_match_tc<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, 204 * 1024);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
     const dim3 grid((Na + MT_BM - 1) / MT_BM, splits, P);
     KLaunch k;
     if (bn == 256) prep(k, k_match_tc<256>, grid, dim3(MT_THREADS), smem, pdl, ta, tb, mp);
@@ -664,8 +660,7 @@ cudaError_t match_static_setup(int dev, MatchStaticDev* out) {
         int sms = 0;
         e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(k_match_tc<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 204 * 1024);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_match_tc<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, 204 * 1024);
+        e = dkd_match_setup_device();
         if (e != cudaSuccess) return e;
         d.part = static_cast<MatchRec*>(ptr);
         d.num_sms = sms;
@@ -673,27 +668,6 @@ cudaError_t match_static_setup(int dev, MatchStaticDev* out) {
     }
     *out = d;
     return cudaSuccess;
-}
-
-// one direction of the match (the geometry of launch_match_dir, with the SM count passed in and no attribute calls)
-cudaError_t launch_match_static_dir(int num_sms, const void* A, const int32_t* ca, int Na, const void* B, const int32_t* cb, int Nb,
-                                    int D, int P, int splits, MatchRec* part, cudaStream_t st, bool pdl) {
-    CUtensorMap ta, tb;
-    if (!encode_desc_map(&ta, A, Na, D, P) || !encode_desc_map(&tb, B, Nb, D, P)) return cudaErrorInvalidValue;
-    MatchParams mp;
-    memset(&mp, 0, sizeof(mp));
-    mp.count_a = ca; mp.count_b = cb; mp.Na = Na; mp.Nb = Nb; mp.KB = D / MT_KBOX; mp.splits = splits; mp.part = part;
-    const int bn = match_bn(num_sms, Na, Nb, P);
-    const size_t a_bytes = static_cast<size_t>(mp.KB) * MT_BM * 128, b_bytes = static_cast<size_t>(bn) * 128;
-    int stages = static_cast<int>((200 * 1024 - a_bytes) / b_bytes);
-    if (stages > MT_MAX_STAGES) stages = MT_MAX_STAGES;
-    mp.stages = stages;
-    const size_t smem = a_bytes + stages * b_bytes + 1024;
-    const dim3 grid((Na + MT_BM - 1) / MT_BM, splits, P);
-    KLaunch k;
-    if (bn == 256) prep(k, k_match_tc<256>, grid, dim3(MT_THREADS), smem, pdl, ta, tb, mp);
-    else prep(k, k_match_tc<128>, grid, dim3(MT_THREADS), smem, pdl, ta, tb, mp);
-    return launch(k, st, true);
 }
 
 int match_static_fail(char* err, int err_len, int code, const char* msg, const char* detail) {
@@ -704,6 +678,16 @@ int match_static_fail(char* err, int err_len, int code, const char* msg, const c
 }  // namespace dkd
 
 using namespace dkd;
+
+// Dynamic shared-memory limits of the kernels of this file.  cudaFuncSetAttribute acts on the CURRENT device only, so
+// this runs once per context from dkd_create (with the context's device current), not once per process.
+cudaError_t dkd_match_setup_device() {
+    cudaError_t e = cudaFuncSetAttribute(k_match_tc<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 204 * 1024);   // (static smem takes ~3 KB of the 227)
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_match_tc<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, 204 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan<DKD_F16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan<DKD_F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+    return e;
+}
 
 extern "C" {
 
@@ -727,8 +711,8 @@ int dkd_match(dkd_ctx* ctx, const void* desc_a, const int32_t* count_a, int Na, 
     if (!part) return DKD_ERR_CUDA;
     // the first kernel waits for whatever precedes it on the stream (it produced the descriptors); the reverse direction and
     // the finalize kernel are programmatic dependents
-    cudaError_t e = launch_match_dir(ctx, desc_a, count_a, Na, desc_b, count_b, Nb, D, P, s_ab, part, st, false);
-    if (e == cudaSuccess && mutual) e = launch_match_dir(ctx, desc_b, count_b, Nb, desc_a, count_a, Na, D, P, s_ba, part + n_ab, st, true);
+    cudaError_t e = launch_match_dir(sms, desc_a, count_a, Na, desc_b, count_b, Nb, D, P, s_ab, part, st, false);
+    if (e == cudaSuccess && mutual) e = launch_match_dir(sms, desc_b, count_b, Nb, desc_a, count_a, Na, D, P, s_ba, part + n_ab, st, true);
     if (e != cudaSuccess) return dkd_ctx_fail(ctx, DKD_ERR_CUDA, "dkd_match launch: ", cudaGetErrorString(e));
     FinalizeParams fp;
     memset(&fp, 0, sizeof(fp));
@@ -776,9 +760,9 @@ int dkd_match_static(const void* desc_a, const int32_t* count_a, int Na, const v
     // rows < Nb of the reverse direction) is written by k_match_tc earlier in this same call.
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     MatchRec* part = d.part;
-    e = launch_match_static_dir(d.num_sms, desc_a, count_a, Na, desc_b, count_b, Nb, D, P, s_ab, part, st, false);
+    e = launch_match_dir(d.num_sms, desc_a, count_a, Na, desc_b, count_b, Nb, D, P, s_ab, part, st, false);
     if (e == cudaSuccess && mutual)
-        e = launch_match_static_dir(d.num_sms, desc_b, count_b, Nb, desc_a, count_a, Na, D, P, s_ba, part + n_ab, st, true);
+        e = launch_match_dir(d.num_sms, desc_b, count_b, Nb, desc_a, count_a, Na, D, P, s_ba, part + n_ab, st, true);
     if (e != cudaSuccess) return match_static_fail(err, err_len, DKD_ERR_CUDA, "dkd_match_static: k_match_tc launch: ", cudaGetErrorString(e));
     FinalizeParams fp;
     memset(&fp, 0, sizeof(fp));
@@ -823,13 +807,6 @@ int dkd_retrieval_scan(dkd_ctx* ctx, const void* db, int dtype, int n, int D, co
     sp.out_sim = out_sim ? out_sim : reinterpret_cast<float*>(ws + b_seg + b_cnt);
     sp.seg = reinterpret_cast<uint64_t*>(ws); sp.seg_cnt = reinterpret_cast<int*>(ws + b_seg); sp.seg_cap = seg_cap;
     const size_t smem_q = static_cast<size_t>(D) * 4;
-    static bool scan_attr = false;
-    if (!scan_attr) {
-        cudaError_t ea = cudaFuncSetAttribute(k_scan<DKD_F16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
-        if (ea == cudaSuccess) ea = cudaFuncSetAttribute(k_scan<DKD_F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
-        if (ea != cudaSuccess) return dkd_ctx_fail(ctx, DKD_ERR_CUDA, "k_scan attribute: ", cudaGetErrorString(ea));
-        scan_attr = true;
-    }
     if (dtype == DKD_F16) k_scan<DKD_F16><<<grid, SC_THREADS, smem_q, st>>>(sp);
     else k_scan<DKD_F32><<<grid, SC_THREADS, smem_q, st>>>(sp);
     cudaError_t e = cudaGetLastError();

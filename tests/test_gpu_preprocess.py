@@ -46,6 +46,28 @@ def test_preprocess_matches_oracle(ctx, cin, cout, dtype, HW, grid):
     assert torch.all(out.cpu()[:, :, mask] == -0.5)
 
 
+@pytest.mark.parametrize("cin,cout,dtype", [(1, 3, torch.float16), (3, 1, torch.float32)])
+def test_preprocess_1080p_bench_shape(cin, cout, dtype):
+    """1080 x 1920 -> 1088 x 1920 (grid 32): the shape bench.py times — the interior fast path with word loads plus the
+    padded rows — mono -> 3 channels f16 (the bench leg) and colour -> luminance f32."""
+    import paper_2607_01757_b200 as dkd
+    c = dkd.DKD(max_batch=2, max_h=1088, max_w=1920, max_top_k=64, max_dim=0)
+    try:
+        img = images(2, 1080, 1920, cin, seed=cin + 40)
+        out = c.preprocess(img.cuda(), cout, 32, bgr=False, mean=MEAN, inv_std=INV_STD, pad_value=-0.5, out_dtype=dtype)
+        torch.cuda.synchronize()
+        ref = oracle.preprocess(img.numpy(), cout, 32, bgr=False, mean=MEAN, inv_std=INV_STD, pad_value=-0.5)
+        assert tuple(out.shape) == ref.shape == (2, cout, 1088, 1920)
+        err = np.abs(out.cpu().double().numpy() - ref).max()
+        assert err <= (5e-6 if dtype == torch.float32 else 2.5e-3), err
+        Hp, Wp, oy, ox = c.padded_size(1080, 1920, 32)
+        mask = torch.ones((Hp, Wp), dtype=torch.bool)
+        mask[oy:oy + 1080, ox:ox + 1920] = False
+        assert torch.all(out.cpu()[:, :, mask] == -0.5)
+    finally:
+        c.close()
+
+
 def test_exact_copy_is_bit_exact(ctx):
     img = images(2, 100, 136, 1, seed=1)
     out = ctx.preprocess(img.cuda(), 1, 8, scale=1.0)

@@ -221,3 +221,42 @@ def test_iterated_nms_limits(ctx):
     with pytest.raises(dkd.DKDError) as e:
         ctx.extract(s, None, 1, 2, 0.2, 8, 0.1, nms_iters=-1)
     assert e.value.code == -1
+
+
+def test_iterated_nms_finest_tiling_at_the_context_maximum():
+    """r = 3, nms_iters = 6: halo 39, 24 x 24 tiles — more tiles (1080) than the context has single-pass NMS units, at the
+    very shape the context was created for: the per-tile counts must fit the workspace (they are sized for this tiling)."""
+    import paper_2607_01757_b200 as dkd
+    B, H, W = 2, 480, 640
+    c = dkd.DKD(B, H, W, 512, 0)
+    try:
+        score = synth.score_maps(B, H, W, 5, 0.1, 600)
+        res = c.extract(score.cuda(), None, 1, 3, 0.15, 512, 0.1, nms_iters=6, want_total=True)
+        ref = oracle.extract_var(score.numpy(), None, 1, 3, 0.15, 512, 0.1, nms_iters=6)
+        compare_var(res, ref)
+        assert ref.count.min() > 50
+        again = c.extract(score.cuda(), None, 1, 2, 0.15, 512, 0.1)           # the workspace after it is intact
+        compare_var(again, oracle.extract_var(score.numpy(), None, 1, 2, 0.15, 512, 0.1))
+    finally:
+        c.close()
+
+
+@pytest.mark.parametrize("unit", [0, 8])
+def test_reliability_at_1080p_in_the_batch64_launch_shape(ctx, unit):
+    """The heat x reliability NMS kernel at 1920 x 1080 with 8-tile units (the shape it is launched in at batch 64:
+    one CTA per SM, both TMA rings), on B = 4 frames the oracle finishes in seconds."""
+    from paper_2607_01757_b200.binding import OPT_NMS_UNIT
+    cfg = synth.CONFIGS["c5"]
+    B = 4
+    score = synth.score_maps(B, cfg.H, cfg.W, 31, 0.1, 4000)
+    desc = synth.desc_maps(B, cfg.H, cfg.W, 128, 31, torch.float16, "cuda")
+    rel = torch.rand(score.shape, generator=torch.Generator().manual_seed(6)) * 0.5 + 0.5
+    try:
+        ctx.set_option(OPT_NMS_UNIT, unit)
+        res = ctx.extract(score.cuda(), desc, 1, cfg.r, cfg.thresh, cfg.top_k, cfg.T, reliability=rel.cuda(), want_total=True)
+        torch.cuda.synchronize()
+    finally:
+        ctx.set_option(OPT_NMS_UNIT, 0)
+    ref = oracle.extract_var(score.numpy(), desc.cpu().numpy(), 1, cfg.r, cfg.thresh, cfg.top_k, cfg.T, reliability=rel.numpy())
+    compare_var(res, ref, torch.float16)
+    assert ref.count.min() > 500
