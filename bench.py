@@ -45,6 +45,7 @@ if ROOT not in sys.path:
 
 METRIC = "us_per_752x480_stereo_pair"
 UNIT = "us/pair"
+NOMINAL_HBM_GBS = 8000.0           # the data-sheet 8 TB/s (fraction reported against both peaks)
 FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback ("of fallback")
 
 
@@ -54,6 +55,7 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=2000)
     ap.add_argument("--warmup", type=int, default=50)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--blocks", type=int, default=50, help="back-to-back timed blocks of --steps steps; value = median block")
     ap.add_argument("--sets", type=int, default=64, help="distinct c2 input sets rotated through (cold inputs)")
     ap.add_argument("--no-batch64", action="store_true", help="skip the config-c5 (B=64 1080p) leg")
     ap.add_argument("--batch64-steps", type=int, default=30)
@@ -297,22 +299,39 @@ def run_ours(args):
     kept = sum(int(s[2].count.sum()) for s in sets) / R
     cb = credited_bytes(cfg.B, cfg.H, cfg.W, cfg.top_k, cfg.D, esz, kept)
 
+    def stats(xs):
+        xs = sorted(xs)
+        return {"min": xs[0], "median": xs[len(xs) // 2], "p95": xs[min(len(xs) - 1, int(len(xs) * 0.95))], "blocks": len(xs)}
+
     for i in range(Wm):
         calls[i % R]()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    # The timed region is NB back-to-back blocks of exactly K steps each, an event between blocks, barrier + synchronize
+    # on both sides of the series; `value` is the MEDIAN block (K = 20 is 0.35 ms of device time: a single block is
+    # dominated by pipeline fill and box noise, the median of 50 is not), min and p95 are reported beside it.
+    NB = args.blocks if args.leg not in ("c5", "pre", "match") else 1
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(NB + 1)]
     barrier()
     torch.cuda.synchronize()
     with sampler:
         t0 = time.perf_counter()
-        ev0.record(stream)
-        for i in range(K):
-            calls[i % R]()
-        ev1.record(stream)
+        evs[0].record(stream)
+        it = 0
+        for b in range(NB):
+            for _ in range(K):
+                calls[it % R]()
+                it += 1
+            evs[b + 1].record(stream)
         torch.cuda.synchronize()
         wall = time.perf_counter() - t0
     barrier()
-    ms_step = max_over_ranks(ev0.elapsed_time(ev1) / K)
-    wall_ms_step = max_over_ranks(wall * 1e3 / K)
+    block_ms = [evs[b].elapsed_time(evs[b + 1]) / K for b in range(NB)]
+    bst = stats(block_ms)
+    ms_step = max_over_ranks(bst["median"])
+    wall_ms_step = max_over_ranks(wall * 1e3 / (K * NB))
+    value_blocks = {"us_min": bst["min"] * 1e3 / world, "us_median": bst["median"] * 1e3 / world, "us_p95": bst["p95"] * 1e3 / world,
+                    "blocks": NB, "steps_per_block": K, "us_mean_all_blocks": evs[0].elapsed_time(evs[NB]) * 1e3 / (K * NB) / world,
+                    "what": "value = median over the blocks of (device time of K back-to-back steps) / K"}
 
     # single-shot latency (enqueue -> outputs complete), one pair at a time
     lat = []
@@ -364,14 +383,27 @@ def run_ours(args):
             for f in cl:
                 f()
             torch.cuda.synchronize()
-            ev0.record(stream)
-            for i in range(480):
-                cl[i % 16]()
-            ev1.record(stream)
-            torch.cuda.synchronize()
+
+            def blocks_us(fns, nb=20, per=48):
+                es = [torch.cuda.Event(enable_timing=True) for _ in range(nb + 1)]
+                for i in range(per):
+                    fns[i % len(fns)]()
+                es[0].record(stream)
+                for b_ in range(nb):
+                    for i in range(per):
+                        fns[(b_ * per + i) % len(fns)]()
+                    es[b_ + 1].record(stream)
+                torch.cuda.synchronize()
+                st_ = stats([es[b_].elapsed_time(es[b_ + 1]) * 1e3 / per for b_ in range(nb)])
+                return {"min": st_["min"], "median": st_["median"], "p95": st_["p95"], "blocks": nb, "calls_per_block": per}
+
+            cold = blocks_us(cl)
+            warm = blocks_us(cl[:1])
             kept_c = sum(int(k[2].count.sum()) for k in keep) / 16
-            other_cfgs[name] = {"us_per_call": ev0.elapsed_time(ev1) * 1e3 / 480, "kept_keypoints": kept_c,
-                                "workload": workload_name(cg)}
+            other_cfgs[name] = {"us_per_call": cold["median"], "cold": cold, "warm": warm, "kept_keypoints": kept_c,
+                                "workload": workload_name(cg),
+                                "what": "us per call, one graph launch per call; cold = rotating through 16 seeded input sets, "
+                                        "warm = one input set (L2-resident)"}
             del cl, keep
             cx.close()
         torch.cuda.empty_cache()
@@ -449,6 +481,21 @@ def run_ours(args):
         if i >= 5:
             for k, v in d.items():
                 kt2[k] = kt2.get(k, 0.0) + v * 1e3 / nprof
+    kt2_var = {}
+    if nprof:                                                    # the same pair through the variants V1 / V2 (per-kernel times)
+        sd_, desc_, out_, _ = sets[0]
+        for name, kw in (("nms_iters2", dict(nms_iters=2)), ("score_bilinear", dict(score_mode=1))):
+            acc = {}
+            for i in range(25):
+                ctx.extract(sd_, desc_, cfg.stride, cfg.r, cfg.thresh, cfg.top_k, cfg.T, out=out_, want_index=False,
+                            want_offsets=False, **kw)
+                d = ctx.profile_read()
+                if i >= 5:
+                    for k, v in d.items():
+                        acc[k] = acc.get(k, 0.0) + v * 1e3 / 20
+            kt2_var[name] = acc
+        calls[0]()                                               # restore set 0's outputs (the e2e leg compares against them)
+        torch.cuda.synchronize()
     ctx.set_option(OPT_PROFILE, 0)
 
     # ---- e2e: HOST buffers through dkd_extract_host, copies inside the timed region -----------------
@@ -471,18 +518,22 @@ def run_ours(args):
             ctx.extract_host(s, d, cfg.stride, cfg.r, cfg.thresh, cfg.top_k, cfg.T, out=o, desc_resident=resident)
         barrier()
         torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        for i in range(n):
-            s, d, o = host_sets[0 if resident else i % 2]
-            ctx.extract_host(s, d, cfg.stride, cfg.r, cfg.thresh, cfg.top_k, cfg.T, out=o, desc_resident=resident)
-        torch.cuda.synchronize()
-        dt = time.perf_counter() - t0
+        blk = []
+        for b_ in range(NBe):                                    # NBe blocks of n synchronised steps, host clock per block
+            t0 = time.perf_counter()
+            for i in range(n):
+                s, d, o = host_sets[0 if resident else i % 2]
+                ctx.extract_host(s, d, cfg.stride, cfg.r, cfg.thresh, cfg.top_k, cfg.T, out=o, desc_resident=resident)
+            torch.cuda.synchronize()
+            blk.append((time.perf_counter() - t0) * 1e6 / n)
         barrier()
-        return max_over_ranks(dt * 1e6 / n)
+        st_ = stats(blk)
+        return max_over_ranks(st_["median"]), st_
 
+    NBe = args.blocks if args.leg not in ("c5", "pre", "match") else 1
     with sampler:
-        e2e_us = e2e_pass(False, Ke)
-        e2e_res_us = e2e_pass(True, Ke)
+        e2e_us, e2e_st = e2e_pass(False, Ke)
+        e2e_res_us, e2e_res_st = e2e_pass(True, Ke)
     assert torch.equal(host_sets[0][2].count, sets[0][2].count.cpu())
 
     # ---- batch 64 (config c5): whole-path throughput + per-kernel roofline ---------------------------
@@ -552,10 +603,11 @@ def run_ours(args):
             traffic, traffic_src = ncu_traffic(dom)
             ach = algo.get(dom, 0) / (kt5[dom] * 1e-6) / 1e9
             roof = {"bound": "hbm", "kernel": dom, "workload": "c5 (B=64 1920x1080)", "achieved": ach, "peak": hbm_peak,
-                    "unit": "GB/s", "frac": ach / hbm_peak, "traffic": traffic, "traffic_source": traffic_src,
-                    "peak_source": peak_src,
+                    "unit": "GB/s", "frac": ach / hbm_peak, "frac_nominal": ach / NOMINAL_HBM_GBS, "traffic": traffic,
+                    "traffic_source": traffic_src, "peak_source": peak_src,
                     "algorithmic_bytes": algo.get(dom, 0), "kernel_us": kt5[dom],
-                    "whole_path": {"achieved": gbs, "frac": gbs / hbm_peak, "credited_bytes": cb5["total"]}}
+                    "whole_path": {"achieved": gbs, "frac": gbs / hbm_peak, "frac_nominal": gbs / NOMINAL_HBM_GBS,
+                                   "credited_bytes": cb5["total"]}}
             # the variants of SURVEY.md 8(f) f2 at c5: heat x reliability streamed as a second TMA stream (the NMS now
             # moves 8 B per pixel), and the validity mask (read only at candidates)
             var5 = None
@@ -566,7 +618,9 @@ def run_ours(args):
                 msk5 = (torch.rand(score5.shape, generator=g5, device=dev) < 0.9).to(torch.uint8)
                 ctx5.set_option(OPT_PROFILE, 1)
                 for name, kw, bpp in (("reliability", dict(reliability=rel5), 8), ("mask", dict(valid_mask=msk5), 4),
-                                      ("reliability+mask", dict(reliability=rel5, valid_mask=msk5), 8)):
+                                      ("reliability+mask", dict(reliability=rel5, valid_mask=msk5), 8),
+                                      ("nms_iters2", dict(nms_iters=2), 4),          # V1: suppress-and-recover NMS
+                                      ("score_bilinear", dict(score_mode=1), 4)):   # V2: score at the refined point
                     acc = {}
                     for i in range(8):
                         ctx5.extract(score5, desc5, c5.stride, c5.r, 0.1 if "reliability" in name else c5.thresh, c5.top_k, c5.T,
@@ -619,10 +673,51 @@ def run_ours(args):
             us = graph_time(lambda s_: ctxm.match(A, Bm, cnta, cntb, ratio=0.8, stream=s_), 10, 10)
             fl = 2.0 * Nn * Nn * Dd * 2
             match_leg["sizes"][f"N{Nn}_D{Dd}"] = {"us": us, "flops": fl, "tflops": fl / us / 1e6, "frac_of_tensor_peak": fl / us / 1e6 / tf_peak}
+            if (Nn, Dd) in ((1024, 128), (4096, 256)):           # the mutual check: a second k_match_tc with the operands swapped
+                usm = graph_time(lambda s_: ctxm.match(A, Bm, cnta, cntb, ratio=0.8, mutual=True, stream=s_), 10, 10)
+                match_leg["sizes"][f"N{Nn}_D{Dd}"]["us_mutual"] = usm
+                match_leg["sizes"][f"N{Nn}_D{Dd}"]["mutual_over_one_way"] = usm / us
         big = match_leg["sizes"]["N4096_D256"]
         match_leg["roofline"] = {"bound": "tensor", "kernel": "k_match_tc", "workload": "P=2 N=4096 D=256 fp16", "achieved": big["tflops"],
                                  "peak": tf_peak, "unit": "TFLOP/s", "frac": big["frac_of_tensor_peak"], "traffic": None,
                                  "peak_source": tf_src, "algorithmic_flops": big["flops"], "kernel_us": big["us"]}
+        # f4: the elementwise consumers, per call (launch-bound: one small kernel each)
+        nst = 1024
+        gk = torch.Generator(device=dev).manual_seed(3)
+        kl = torch.rand((nst, 2), generator=gk, device=dev) * 400 + 50
+        kr = kl - torch.tensor([20.0, 0.0], device=dev)
+        mt = torch.arange(nst, dtype=torch.int32, device=dev)
+        cam = dict(fx=458.0, fy=457.0, cx=367.0, cy=248.0, baseline=0.11, d_min=1.0, z_min=0.3, z_max=30.0)
+        Lf = torch.rand((nst, 3), generator=gk, device=dev) + 0.2
+        covp = dict(scale=1.25, floor_px=0.0, fx=460.0, fy=455.0, lam=0.3, lam_min=0.05, sigma0=1.5 / 460.0)
+        match_leg["stereo_validate_us"] = graph_time(lambda s_: ctxm.stereo_validate(kl, kr, mt, stream=s_, **cam), 20, 10)
+        match_leg["cov_sqrt_info_us"] = graph_time(lambda s_: ctxm.cov_sqrt_info(Lf, stream=s_, **covp), 20, 10)
+        match_leg["f4_what"] = "us per call on 1024 keypoints, GPU time from graph replays (20 calls per graph)"
+
+        # the composed front-end of one stereo frame, device-resident: dkd_extract on B = 4 views
+        # (L/R at t-1 and t) -> dkd_match P = 2 (temporal + stereo pair, ratio 0.8, mutual) on views of the extract outputs
+        # -> dkd_stereo_validate; the whole chain captured in ONE caller graph and replayed
+        frontend = {"what": "us per stereo frame: extract(B=4 752x480, 128-d f16) -> match(P=2, mutual) -> stereo_validate, one "
+                            "caller graph, GPU time from graph replays; cap = keypoint cap (PAPER.md:171: 256)"}
+        sq, dq = synth.stereo_sequence(cfg.H, cfg.W, cfg.D, seed=9, disparity=20, device=dev)
+        sq = sq.to(dev)
+        for cap in (256, 1024):
+            cf_ = dkd.DKD(4, cfg.H, cfg.W, cap, cfg.D, device=local)
+            of = cf_.alloc_outputs(4, cap, dq, cfg.D, want_index=False, want_offsets=False)
+
+            def chain(s_, cf_=cf_, of=of, cap=cap):
+                r_ = cf_.extract(sq, dq, 1, cfg.r, cfg.thresh, cap, cfg.T, out=of, stream=s_, want_index=False, want_offsets=False)
+                m_, _ = cf_.match(r_.desc[0:2], r_.desc[1:3], r_.count[0:2], r_.count[1:3], ratio=0.8, mutual=True,
+                                  want_sim=False, stream=s_)
+                return cf_.stereo_validate(r_.kpts[1], r_.kpts[2], m_[1], stream=s_, max_reproj=1.5, **cam)
+
+            us_f = graph_time(chain, 4, 25)
+            v_ = chain(None)[0]
+            torch.cuda.synchronize()
+            frontend[f"cap{cap}"] = {"us": us_f, "keypoints": [int(x) for x in of.count.tolist()], "stereo_valid": int(v_.sum())}
+            cf_.close()
+        match_leg["frontend_frame_us"] = frontend
+        del sq, dq
         # retrieval: AnyLoc-sized descriptors (32 x 384 = 12288); 20 000 keyframes = 492 MB > L2
         nk, Dg = 20000, 12288
         gq = torch.Generator(device=dev).manual_seed(11)
@@ -743,7 +838,7 @@ def run_ours(args):
                        "launch": "one cached CUDA-graph launch per step (3 kernels, programmatic dependent launch edges)", "parallelism": f"batch-sharded x{world}, no collective"},
             "frames_per_s": world * cfg.B / (ms_step * 1e-3), "keypoints_per_s": world * kept / (ms_step * 1e-3),
             "credited_bytes": cb, "credited_gbs": cb["total"] / (ms_step * 1e-3) / 1e9,
-            "wall_ms_per_step": wall_ms_step,
+            "wall_ms_per_step": wall_ms_step, "value_blocks": value_blocks,
             "latency_us": {"median": lat[len(lat) // 2], "min": lat[0], "p95": lat[int(len(lat) * 0.95)],
                            "what": "single shot: enqueue -> stream idle, host clock"},
             "stream_launch": {"value": stream_us, "unit": UNIT, "queued_on_device": stream_dev_us, "graph_queued_on_device": graph_dev_us,
@@ -752,17 +847,17 @@ def run_ours(args):
                                       "same launches queued behind a sleeping kernel (the device's own time per step, no host launch-rate "
                                       "limit), graph_queued_on_device = the default graph launches measured the same way"},
             "fresh_buffers": fresh,
-            "kernel_us_c2": kt2,
+            "kernel_us_c2": kt2, "kernel_us_c2_variants": kt2_var,
             "clocks": sampler.summary(),
             "e2e": {"value": e2e_us / world, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "steps": Ke, "what": "dkd_extract_host, pinned host buffers: score maps copied H2D, descriptor corner rows read "
+                    "steps": Ke, "blocks": e2e_st, "what": "median over blocks of `steps` calls; dkd_extract_host, pinned host buffers: score maps copied H2D, descriptor corner rows read "
                     "in place from the pinned map over PCIe (counted in h2d), every output stored by the kernels into the "
                     "pinned host tensors (counted in d2h); synchronised before return",
                     "descriptor_map_bytes_on_host": h2d_full - cfg.B * cfg.H * cfg.W * 4},
             "e2e_desc_resident": {"value": e2e_res_us / world, "unit": UNIT, "h2d_bytes_per_step": cfg.B * cfg.H * cfg.W * 4,
                                   "d2h_bytes_per_step": d2h,
                                   "what": "same, descriptor map left on the device by the previous call (network output)"},
-            "gpu_launches": K * 3,
+            "gpu_launches": K * 3 * NB,
             "batch64": b64, "roofline": roof, "cpu_baseline": cpu, "match": match_leg, "retrieval": retr_leg, "preprocess": pre, "cap_sweep": cap_sweep, "other_configs": other_cfgs,
             "context": "paper: whole pipeline 29-47 FPS mono / 18-33 FPS stereo on Jetson AGX Orin (PAPER.md:5) — other hardware, whole system",
         }

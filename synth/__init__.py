@@ -160,6 +160,29 @@ def make_inputs(cfg: Config, device="cpu", with_desc=True, pin_memory=False):
     return score, desc
 
 
+# ---- a stereo sequence for the composed chain extract -> match -> stereo validation ------
+def stereo_sequence(H, W, D, seed, disparity, motion=(5, -3), base=0.1, nblobs=900, dtype=torch.float16, device="cpu",
+                    margin=32):
+    """Four views of ONE synthetic world, as crops of a larger score map and descriptor map (stride 1), in the batch
+    order [L(t-1), L(t), R(t), R(t-1)]: the right camera sees every world point `disparity` pixels further left
+    (x_R = x_L - disparity: a fronto-parallel scene at depth fx * baseline / disparity), and between t-1 and t the image
+    content moves by motion = (dx, dy) pixels.  Integer shifts, so corresponding keypoints have identical windows and
+    identical bilinear samples: descriptors of true correspondences agree to rounding; points near the crop borders
+    have no partner.  Returns (score [4,H,W] f32 CPU, desc [4,H,W,D] `dtype` on `device`).  Stands in for consecutive
+    stereo frames of the paper's datasets (EuRoC-like 752 x 480), which are not available."""
+    dx, dy = int(motion[0]), int(motion[1])
+    d = int(disparity)
+    assert max(abs(dx), abs(dy)) <= margin and 0 <= d <= margin
+    Hb, Wb = H + 2 * margin, W + 2 * margin
+    world_s = score_maps(1, Hb, Wb, seed, base, nblobs)[0]
+    world_d = desc_maps(1, Hb, Wb, D, seed, dtype, device)[0]
+    # top-left corner of each view in the world: a point at world column c appears at c - x0 in the view
+    corners = [(margin - dy, margin - dx), (margin, margin), (margin, margin + d), (margin - dy, margin - dx + d)]
+    score = torch.stack([world_s[y0:y0 + H, x0:x0 + W] for y0, x0 in corners]).contiguous()
+    desc = torch.stack([world_d[y0:y0 + H, x0:x0 + W] for y0, x0 in corners]).contiguous()
+    return score, desc
+
+
 # ---- inputs for the consumers of the descriptor output (SURVEY.md 8(f) f3, f4) ---------------------------------
 def _unit_rows(g: torch.Generator, n: int, D: int) -> torch.Tensor:
     x = torch.randn((n, D), generator=g, dtype=torch.float64)
