@@ -296,7 +296,14 @@ cudaError_t build_plan(dkd_ctx* ctx, const ExtractArgs& a, Plan& pl) {
         ip.T = (IT_REG - 2 * ip.halo) & ~7;
         ip.tiles_x = (a.W + ip.T - 1) / ip.T; ip.tiles_y = (a.H + ip.T - 1) / ip.T;
         ip.thresh = a.thresh; ip.cand = ctx->cand; ip.seg_cnt = ctx->tile_cnt;
-        prep(pl.k[0], k_nms_iter, dim3(ip.tiles_x * ip.tiles_y, a.B), dim3(IT_THREADS), IT_SMEM_BYTES, ctx->use_pdl != 0, ip);
+        const dim3 ig(ip.tiles_x * ip.tiles_y, a.B), ib(IT_THREADS);
+        const bool ipdl = ctx->use_pdl != 0;
+        switch (a.r) {
+            case 1: prep(pl.k[0], k_nms_iter<1>, ig, ib, IT_SMEM_BYTES, ipdl, ip); break;
+            case 2: prep(pl.k[0], k_nms_iter<2>, ig, ib, IT_SMEM_BYTES, ipdl, ip); break;
+            case 3: prep(pl.k[0], k_nms_iter<3>, ig, ib, IT_SMEM_BYTES, ipdl, ip); break;
+            default: prep(pl.k[0], k_nms_iter<4>, ig, ib, IT_SMEM_BYTES, ipdl, ip); break;
+        }
         tpi = ip.tiles_x * ip.tiles_y;
         seg_cap = ip.T * ip.T;
     } else {
@@ -701,7 +708,10 @@ int dkd_create(const dkd_create_params* p, dkd_ctx** out) {
     CKC(setup_nms<3>(ctx));
     CKC(setup_nms<4>(ctx));
     CKC(cudaFuncSetAttribute(k_select, cudaFuncAttributeMaxDynamicSharedMemorySize, SEL_SMEM_BYTES));
-    CKC(cudaFuncSetAttribute(k_nms_iter, cudaFuncAttributeMaxDynamicSharedMemorySize, IT_SMEM_BYTES));
+    CKC(cudaFuncSetAttribute(k_nms_iter<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, IT_SMEM_BYTES));
+    CKC(cudaFuncSetAttribute(k_nms_iter<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, IT_SMEM_BYTES));
+    CKC(cudaFuncSetAttribute(k_nms_iter<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, IT_SMEM_BYTES));
+    CKC(cudaFuncSetAttribute(k_nms_iter<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, IT_SMEM_BYTES));
     CKC(dkd_match_setup_device());
     const size_t tx = (p->max_w + STRIP_W - 1) / STRIP_W, ty = (p->max_h + TH - 1) / TH;
     ctx->max_tiles = tx * (ty + MAX_CPU - 1) * p->max_batch;   // segments of whole units: up to MAX_CPU-1 spare strip-tiles per strip

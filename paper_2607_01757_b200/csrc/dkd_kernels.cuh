@@ -519,11 +519,17 @@ __global__ void __launch_bounds__(PLAIN_WARPS * 32) k_nms_plain(const float* __r
 // loads an IT_REG x IT_REG region (out-of-image pixels = -inf) into shared memory, runs every pooling stage on the
 // whole region as a separable row / column pass (values near the region's edge are wrong, but no output of the inner
 // T x T tile, T = IT_REG - 2 (2n+1) r, depends on them), applies border / threshold / validity mask to the tile and
-// appends its candidates to the tile's private segment (block scan, no atomics) for k_select.  A variant kernel: plain
-// loads, no TMA; the single-pass kernels above stay the hot path.
+// appends its candidates to the tile's private segment (block scan, no atomics) for k_select.
+// Every pass works on GROUPS of 4 horizontally adjacent pixels: one float4 (scores) or one 32-bit word of four 0/1 bytes
+// (masks) per shared-memory access.  A row pass reads the group and its two neighbours (r <= 4: the window never
+// reaches further) and slides the window over the 12 values in registers; a column pass reads the 2r+1 groups above /
+// below (rows clamped into the region: a repeated row does not change a maximum or an OR).  The radius is a template
+// parameter, so all window loops are unrolled.  32 warps per CTA hide the shared-memory latency between the passes.
 constexpr int IT_REG = 104;
-constexpr int IT_THREADS = 256;
+constexpr int IT_G = IT_REG / 4;                             // pixel groups per region row
+constexpr int IT_THREADS = 1024;
 constexpr int IT_SMEM_BYTES = IT_REG * IT_REG * (3 * 4 + 3);
+static_assert(IT_REG % 4 == 0 && MAX_R <= 4, "pixel groups of 4: a window may reach one group to either side");
 struct IterParams {
     const float* score;
     const float* score2;
@@ -533,15 +539,39 @@ struct IterParams {
     uint64_t* cand;
     int* seg_cnt;
 };
+__device__ __forceinline__ float4 it_max4(const float4& a, const float4& b) {
+    return make_float4(fmaxf(a.x, b.x), fmaxf(a.y, b.y), fmaxf(a.z, b.z), fmaxf(a.w, b.w));
+}
+// the four bytes that start D bytes after the start of word c in the byte sequence (l, c, rr); D in [-4, 4]
+template <int D>
+__device__ __forceinline__ uint32_t it_shift_bytes(uint32_t l, uint32_t c, uint32_t rr) {
+    if constexpr (D == 0) return c;
+    else if constexpr (D == -4) return l;
+    else if constexpr (D == 4) return rr;
+    else if constexpr (D < 0) return __funnelshift_r(l, c, 8 * (4 + D));
+    else return __funnelshift_r(c, rr, 8 * D);
+}
+template <int R, int D = -R>
+__device__ __forceinline__ uint32_t it_dilate_row(uint32_t l, uint32_t c, uint32_t rr) {
+    if constexpr (D > R) return 0u;
+    else return it_shift_bytes<D>(l, c, rr) | it_dilate_row<R, D + 1>(l, c, rr);
+}
+template <int R>
 __global__ void __launch_bounds__(IT_THREADS, 1) k_nms_iter(const __grid_constant__ IterParams p) {
     extern __shared__ __align__(16) unsigned char it_smem[];
-    constexpr int NPX = IT_REG * IT_REG;
+    constexpr int NPX = IT_REG * IT_REG, NG = NPX / 4;
     float* S = reinterpret_cast<float*>(it_smem);
     float* Sp = S + NPX;
     float* tmp = Sp + NPX;
     uint8_t* M = reinterpret_cast<uint8_t*>(tmp + NPX);
     uint8_t* tb = M + NPX;
     uint8_t* sup = tb + NPX;
+    const float4* S4 = reinterpret_cast<const float4*>(S);
+    float4* Sp4 = reinterpret_cast<float4*>(Sp);
+    float4* tmp4 = reinterpret_cast<float4*>(tmp);
+    uint32_t* M32 = reinterpret_cast<uint32_t*>(M);
+    uint32_t* tb32 = reinterpret_cast<uint32_t*>(tb);
+    uint32_t* sup32 = reinterpret_cast<uint32_t*>(sup);
     __shared__ int s_scan[IT_THREADS / 32];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tx = blockIdx.x % p.tiles_x, ty = blockIdx.x / p.tiles_x, b = blockIdx.y;
@@ -549,7 +579,8 @@ __global__ void __launch_bounds__(IT_THREADS, 1) k_nms_iter(const __grid_constan
     const size_t img_px = static_cast<size_t>(p.H) * p.W;
     const float* img = p.score + b * img_px;
     const float* img2 = p.score2 ? p.score2 + b * img_px : nullptr;
-    const int r = p.r;
+    const int r = R;
+    DKD_ASSERT(p.r == R);
     pdl_launch_dependents();
     pdl_wait();                                              // (see k_nms_tma)
     for (int i = tid; i < NPX; i += IT_THREADS) {
@@ -563,52 +594,69 @@ __global__ void __launch_bounds__(IT_THREADS, 1) k_nms_iter(const __grid_constan
         S[i] = v;
     }
     __syncthreads();
+    const float4 ninf4 = make_float4(-INFINITY, -INFINITY, -INFINITY, -INFINITY);
     // separable window maximum of `src` over the region: row pass into tmp, then the column pass is folded into its user
-    auto row_max = [&](const float* src) {
-        for (int i = tid; i < NPX; i += IT_THREADS) {
-            const int ry = i / IT_REG, rx = i - ry * IT_REG;
-            const int a = rx - r < 0 ? 0 : rx - r, e = rx + r >= IT_REG ? IT_REG - 1 : rx + r;
-            float m = src[ry * IT_REG + a];
-            for (int x = a + 1; x <= e; ++x) m = fmaxf(m, src[ry * IT_REG + x]);
-            tmp[i] = m;
+    auto row_max = [&](const float4* src4) {
+        for (int g = tid; g < NG; g += IT_THREADS) {
+            const int gx = g % IT_G;
+            const float4 c = src4[g];
+            const float4 l = gx > 0 ? src4[g - 1] : ninf4;
+            const float4 rr = gx < IT_G - 1 ? src4[g + 1] : ninf4;
+            const float w[12] = {l.x, l.y, l.z, l.w, c.x, c.y, c.z, c.w, rr.x, rr.y, rr.z, rr.w};
+            float o[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                float m = w[4 + j - R];
+#pragma unroll
+                for (int d = -R + 1; d <= R; ++d) m = fmaxf(m, w[4 + j + d]);
+                o[j] = m;
+            }
+            tmp4[g] = make_float4(o[0], o[1], o[2], o[3]);
         }
     };
-    auto col_max_at = [&](int ry, int rx) {
-        const int a = ry - r < 0 ? 0 : ry - r, e = ry + r >= IT_REG ? IT_REG - 1 : ry + r;
-        float m = tmp[a * IT_REG + rx];
-        for (int y = a + 1; y <= e; ++y) m = fmaxf(m, tmp[y * IT_REG + rx]);
+    auto col_max4 = [&](int ry, int gx) {
+        float4 m = tmp4[max(ry - R, 0) * IT_G + gx];
+#pragma unroll
+        for (int d = -R + 1; d <= R; ++d) m = it_max4(m, tmp4[min(max(ry + d, 0), IT_REG - 1) * IT_G + gx]);
         return m;
     };
-    row_max(S);
+    // bytes (0 / 1) of the pixels of `v` that are in the image and equal their window maximum `m`
+    auto maxima4 = [](const float4& v, const float4& m) {
+        return (v.x != -INFINITY && v.x == m.x ? 0x1u : 0u) | (v.y != -INFINITY && v.y == m.y ? 0x100u : 0u) |
+               (v.z != -INFINITY && v.z == m.z ? 0x10000u : 0u) | (v.w != -INFINITY && v.w == m.w ? 0x1000000u : 0u);
+    };
+    row_max(S4);
     __syncthreads();
-    for (int i = tid; i < NPX; i += IT_THREADS) {
-        const int ry = i / IT_REG, rx = i - ry * IT_REG;
-        M[i] = (S[i] != -INFINITY && S[i] == col_max_at(ry, rx)) ? 1 : 0;      // out-of-image pixels are never maxima
+    for (int g = tid; g < NG; g += IT_THREADS) {
+        const int ry = g / IT_G, gx = g - ry * IT_G;
+        M32[g] = maxima4(S4[g], col_max4(ry, gx));               // out-of-image pixels are never maxima
     }
     __syncthreads();
     for (int it = 0; it < p.iters; ++it) {
-        for (int i = tid; i < NPX; i += IT_THREADS) {            // supp = dilate(M): row pass
-            const int ry = i / IT_REG, rx = i - ry * IT_REG;
-            const int a = rx - r < 0 ? 0 : rx - r, e = rx + r >= IT_REG ? IT_REG - 1 : rx + r;
-            uint8_t m = 0;
-            for (int x = a; x <= e; ++x) m |= M[ry * IT_REG + x];
-            tb[i] = m;
+        for (int g = tid; g < NG; g += IT_THREADS) {             // supp = dilate(M): row pass
+            const int gx = g % IT_G;
+            tb32[g] = it_dilate_row<R>(gx > 0 ? M32[g - 1] : 0u, M32[g], gx < IT_G - 1 ? M32[g + 1] : 0u);
         }
         __syncthreads();
-        for (int i = tid; i < NPX; i += IT_THREADS) {            // column pass, and S' = supp ? 0 : S
-            const int ry = i / IT_REG, rx = i - ry * IT_REG;
-            const int a = ry - r < 0 ? 0 : ry - r, e = ry + r >= IT_REG ? IT_REG - 1 : ry + r;
-            uint8_t m = 0;
-            for (int y = a; y <= e; ++y) m |= tb[y * IT_REG + rx];
-            sup[i] = m;
-            Sp[i] = S[i] == -INFINITY ? -INFINITY : (m ? 0.0f : S[i]);
+        for (int g = tid; g < NG; g += IT_THREADS) {             // column pass, and S' = supp ? 0 : S
+            const int ry = g / IT_G, gx = g - ry * IT_G;
+            uint32_t m = 0;
+#pragma unroll
+            for (int d = -R; d <= R; ++d) m |= tb32[min(max(ry + d, 0), IT_REG - 1) * IT_G + gx];
+            sup32[g] = m;
+            const float4 v = S4[g];
+            Sp4[g] = make_float4(v.x == -INFINITY ? v.x : ((m & 0xFFu) ? 0.0f : v.x), v.y == -INFINITY ? v.y : ((m & 0xFF00u) ? 0.0f : v.y),
+                                 v.z == -INFINITY ? v.z : ((m & 0xFF0000u) ? 0.0f : v.z), v.w == -INFINITY ? v.w : ((m & 0xFF000000u) ? 0.0f : v.w));
         }
         __syncthreads();
-        row_max(Sp);
+        row_max(Sp4);
         __syncthreads();
-        for (int i = tid; i < NPX; i += IT_THREADS) {            // recover: maxima of S' outside the suppression mask
-            const int ry = i / IT_REG, rx = i - ry * IT_REG;
-            if (!sup[i] && Sp[i] != -INFINITY && Sp[i] == col_max_at(ry, rx)) M[i] = 1;
+        for (int g = tid; g < NG; g += IT_THREADS) {             // recover: maxima of S' outside the suppression mask
+            const int ry = g / IT_G, gx = g - ry * IT_G;
+            const uint32_t sm = sup32[g];
+            if (sm == 0x01010101u) continue;                     // every pixel of the group is suppressed
+            const uint32_t rec = maxima4(Sp4[g], col_max4(ry, gx)) & ~sm;
+            if (rec) M32[g] |= rec;
         }
         __syncthreads();
     }
