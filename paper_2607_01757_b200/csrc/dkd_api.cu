@@ -293,6 +293,8 @@ cudaError_t build_plan(dkd_ctx* ctx, const ExtractArgs& a, Plan& pl) {
         memset(&ip, 0, sizeof(ip));
         ip.score = a.score; ip.score2 = a.score2; ip.mask = a.mask; ip.H = a.H; ip.W = a.W; ip.r = a.r; ip.iters = a.nms_iters;
         ip.halo = (2 * a.nms_iters + 1) * a.r;
+        ip.halo_x = (ip.halo + 3) & ~3;                     // (fits: IT_REG - 2 halo - T >= halo_x - halo, IT_REG % 8 == 0)
+        ip.vec = (a.W % 4 == 0) && !misaligned(a.score, 16) && !misaligned(a.score2, 16);
         ip.T = (IT_REG - 2 * ip.halo) & ~7;
         ip.tiles_x = (a.W + ip.T - 1) / ip.T; ip.tiles_y = (a.H + ip.T - 1) / ip.T;
         ip.thresh = a.thresh; ip.cand = ctx->cand; ip.seg_cnt = ctx->tile_cnt;

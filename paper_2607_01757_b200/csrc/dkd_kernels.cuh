@@ -13,6 +13,7 @@
 #include <cuda.h>
 #include <cuda_fp16.h>
 #include <cuda_runtime.h>
+#include <type_traits>
 #include <stdint.h>
 
 #include "dkd.h"
@@ -525,16 +526,19 @@ __global__ void __launch_bounds__(PLAIN_WARPS * 32) k_nms_plain(const float* __r
 // reaches further) and slides the window over the 12 values in registers; a column pass reads the 2r+1 groups above /
 // below (rows clamped into the region: a repeated row does not change a maximum or an OR).  The radius is a template
 // parameter, so all window loops are unrolled.  32 warps per CTA hide the shared-memory latency between the passes.
-constexpr int IT_REG = 104;
+constexpr int IT_REG = 96;
 constexpr int IT_G = IT_REG / 4;                             // pixel groups per region row
-constexpr int IT_THREADS = 1024;
-constexpr int IT_SMEM_BYTES = IT_REG * IT_REG * (3 * 4 + 3);
-static_assert(IT_REG % 4 == 0 && MAX_R <= 4, "pixel groups of 4: a window may reach one group to either side");
+constexpr int IT_THREADS = 768;
+constexpr int IT_SMEM_BYTES = IT_REG * IT_REG * (2 * 4 + 3); // S, tmp (fp32); M, tb, sup (bytes): 99 KB -> two CTAs per SM,
+                                                             // one loads its region while the other runs its passes
+static_assert(IT_REG % 8 == 0 && MAX_R <= 4, "pixel groups of 4: a window may reach one group to either side");
+static_assert((IT_REG * IT_REG / 4) % IT_THREADS == 0, "every thread owns the same number of pixel groups");
 struct IterParams {
     const float* score;
     const float* score2;
     const uint8_t* mask;
-    int H, W, r, iters, T, halo, tiles_x, tiles_y;
+    int H, W, r, iters, T, halo, halo_x, tiles_x, tiles_y;   // halo_x = halo rounded up to 4: pixel groups are 4-aligned in the image
+    int vec;                                                 // W % 4 == 0 and 16-byte aligned maps: 16-byte global loads
     float thresh;
     uint64_t* cand;
     int* seg_cnt;
@@ -556,18 +560,21 @@ __device__ __forceinline__ uint32_t it_dilate_row(uint32_t l, uint32_t c, uint32
     if constexpr (D > R) return 0u;
     else return it_shift_bytes<D>(l, c, rr) | it_dilate_row<R, D + 1>(l, c, rr);
 }
+// S' = supp ? 0 : S of a pixel group (out-of-image pixels stay -inf); sm = the group's four suppression bytes
+__device__ __forceinline__ float4 it_suppressed(const float4& v, uint32_t sm) {
+    return make_float4(v.x == -INFINITY ? v.x : ((sm & 0xFFu) ? 0.0f : v.x), v.y == -INFINITY ? v.y : ((sm & 0xFF00u) ? 0.0f : v.y),
+                       v.z == -INFINITY ? v.z : ((sm & 0xFF0000u) ? 0.0f : v.z), v.w == -INFINITY ? v.w : ((sm & 0xFF000000u) ? 0.0f : v.w));
+}
 template <int R>
-__global__ void __launch_bounds__(IT_THREADS, 1) k_nms_iter(const __grid_constant__ IterParams p) {
+__global__ void __launch_bounds__(IT_THREADS, 2) k_nms_iter(const __grid_constant__ IterParams p) {
     extern __shared__ __align__(16) unsigned char it_smem[];
     constexpr int NPX = IT_REG * IT_REG, NG = NPX / 4;
     float* S = reinterpret_cast<float*>(it_smem);
-    float* Sp = S + NPX;
-    float* tmp = Sp + NPX;
+    float* tmp = S + NPX;
     uint8_t* M = reinterpret_cast<uint8_t*>(tmp + NPX);
     uint8_t* tb = M + NPX;
     uint8_t* sup = tb + NPX;
-    const float4* S4 = reinterpret_cast<const float4*>(S);
-    float4* Sp4 = reinterpret_cast<float4*>(Sp);
+    float4* S4 = reinterpret_cast<float4*>(S);
     float4* tmp4 = reinterpret_cast<float4*>(tmp);
     uint32_t* M32 = reinterpret_cast<uint32_t*>(M);
     uint32_t* tb32 = reinterpret_cast<uint32_t*>(tb);
@@ -575,33 +582,56 @@ __global__ void __launch_bounds__(IT_THREADS, 1) k_nms_iter(const __grid_constan
     __shared__ int s_scan[IT_THREADS / 32];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tx = blockIdx.x % p.tiles_x, ty = blockIdx.x / p.tiles_x, b = blockIdx.y;
-    const int x0 = tx * p.T - p.halo, y0 = ty * p.T - p.halo;     // image coordinates of the region's origin
+    const int x0 = tx * p.T - p.halo_x, y0 = ty * p.T - p.halo;   // image coordinates of the region's origin (x0 % 4 == 0)
     const size_t img_px = static_cast<size_t>(p.H) * p.W;
     const float* img = p.score + b * img_px;
     const float* img2 = p.score2 ? p.score2 + b * img_px : nullptr;
-    const int r = R;
-    DKD_ASSERT(p.r == R);
+    DKD_ASSERT(p.r == R && (x0 & 3) == 0);
     pdl_launch_dependents();
     pdl_wait();                                              // (see k_nms_tma)
-    for (int i = tid; i < NPX; i += IT_THREADS) {
-        const int ry = i / IT_REG, rx = i - ry * IT_REG, gy = y0 + ry, gx = x0 + rx;
-        float v = -INFINITY;
-        if (gy >= 0 && gy < p.H && gx >= 0 && gx < p.W) {
-            const size_t e = static_cast<size_t>(gy) * p.W + gx;
-            v = __ldg(img + e);
-            if (img2) v = __fmul_rn(v, __ldg(img2 + e));
+    const float4 ninf4 = make_float4(-INFINITY, -INFINITY, -INFINITY, -INFINITY);
+#pragma unroll
+    for (int g = tid; g < NG; g += IT_THREADS) {
+        const int ry = g / IT_G, gy = y0 + ry, gx = x0 + 4 * (g - ry * IT_G);
+        float4 v = ninf4;
+        if (gy >= 0 && gy < p.H && gx + 3 >= 0 && gx < p.W) {
+            const size_t e = static_cast<size_t>(gy) * p.W + gx;     // (not formed as a pointer unless in range)
+            if (p.vec) {                                     // W % 4 == 0 and gx % 4 == 0: the group is inside the row
+                v = __ldg(reinterpret_cast<const float4*>(img + e));
+                if (img2) {
+                    const float4 q = __ldg(reinterpret_cast<const float4*>(img2 + e));
+                    v = make_float4(__fmul_rn(v.x, q.x), __fmul_rn(v.y, q.y), __fmul_rn(v.z, q.z), __fmul_rn(v.w, q.w));
+                }
+            } else {
+                float t[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    t[j] = -INFINITY;
+                    if (gx + j >= 0 && gx + j < p.W) {
+                        t[j] = __ldg(img + e + j);
+                        if (img2) t[j] = __fmul_rn(t[j], __ldg(img2 + e + j));
+                    }
+                }
+                v = make_float4(t[0], t[1], t[2], t[3]);
+            }
         }
-        S[i] = v;
+        S4[g] = v;
     }
     __syncthreads();
-    const float4 ninf4 = make_float4(-INFINITY, -INFINITY, -INFINITY, -INFINITY);
-    // separable window maximum of `src` over the region: row pass into tmp, then the column pass is folded into its user
-    auto row_max = [&](const float4* src4) {
+    // separable window maximum over the region: the row pass of S (SUPP = false) or of S' = supp ? 0 : S, formed on the
+    // fly from S and the suppression bytes (SUPP = true), into tmp; the column pass is folded into its user
+    auto row_max = [&](auto supp_tag) {
+        constexpr bool SUPP = decltype(supp_tag)::value;
         for (int g = tid; g < NG; g += IT_THREADS) {
             const int gx = g % IT_G;
-            const float4 c = src4[g];
-            const float4 l = gx > 0 ? src4[g - 1] : ninf4;
-            const float4 rr = gx < IT_G - 1 ? src4[g + 1] : ninf4;
+            float4 c = S4[g];
+            float4 l = gx > 0 ? S4[g - 1] : ninf4;
+            float4 rr = gx < IT_G - 1 ? S4[g + 1] : ninf4;
+            if constexpr (SUPP) {
+                c = it_suppressed(c, sup32[g]);
+                if (gx > 0) l = it_suppressed(l, sup32[g - 1]);
+                if (gx < IT_G - 1) rr = it_suppressed(rr, sup32[g + 1]);
+            }
             const float w[12] = {l.x, l.y, l.z, l.w, c.x, c.y, c.z, c.w, rr.x, rr.y, rr.z, rr.w};
             float o[4];
 #pragma unroll
@@ -625,7 +655,7 @@ __global__ void __launch_bounds__(IT_THREADS, 1) k_nms_iter(const __grid_constan
         return (v.x != -INFINITY && v.x == m.x ? 0x1u : 0u) | (v.y != -INFINITY && v.y == m.y ? 0x100u : 0u) |
                (v.z != -INFINITY && v.z == m.z ? 0x10000u : 0u) | (v.w != -INFINITY && v.w == m.w ? 0x1000000u : 0u);
     };
-    row_max(S4);
+    row_max(std::false_type{});
     __syncthreads();
     for (int g = tid; g < NG; g += IT_THREADS) {
         const int ry = g / IT_G, gx = g - ry * IT_G;
@@ -638,49 +668,57 @@ __global__ void __launch_bounds__(IT_THREADS, 1) k_nms_iter(const __grid_constan
             tb32[g] = it_dilate_row<R>(gx > 0 ? M32[g - 1] : 0u, M32[g], gx < IT_G - 1 ? M32[g + 1] : 0u);
         }
         __syncthreads();
-        for (int g = tid; g < NG; g += IT_THREADS) {             // column pass, and S' = supp ? 0 : S
+        for (int g = tid; g < NG; g += IT_THREADS) {             // column pass
             const int ry = g / IT_G, gx = g - ry * IT_G;
             uint32_t m = 0;
 #pragma unroll
             for (int d = -R; d <= R; ++d) m |= tb32[min(max(ry + d, 0), IT_REG - 1) * IT_G + gx];
             sup32[g] = m;
-            const float4 v = S4[g];
-            Sp4[g] = make_float4(v.x == -INFINITY ? v.x : ((m & 0xFFu) ? 0.0f : v.x), v.y == -INFINITY ? v.y : ((m & 0xFF00u) ? 0.0f : v.y),
-                                 v.z == -INFINITY ? v.z : ((m & 0xFF0000u) ? 0.0f : v.z), v.w == -INFINITY ? v.w : ((m & 0xFF000000u) ? 0.0f : v.w));
         }
         __syncthreads();
-        row_max(Sp4);
+        row_max(std::true_type{});
         __syncthreads();
         for (int g = tid; g < NG; g += IT_THREADS) {             // recover: maxima of S' outside the suppression mask
             const int ry = g / IT_G, gx = g - ry * IT_G;
             const uint32_t sm = sup32[g];
             if (sm == 0x01010101u) continue;                     // every pixel of the group is suppressed
-            const uint32_t rec = maxima4(Sp4[g], col_max4(ry, gx)) & ~sm;
+            const uint32_t rec = maxima4(it_suppressed(S4[g], sm), col_max4(ry, gx)) & ~sm;
             if (rec) M32[g] |= rec;
         }
         __syncthreads();
     }
-    // the inner T x T tile: border exclusion, strict threshold, validity mask -> keys, compacted in pixel order
-    const int tile_px = p.T * p.T;
+    // the inner T x T tile: border exclusion, strict threshold, validity mask -> keys, compacted in pixel order.  The tile
+    // starts on a group boundary (halo_x % 4 == 0, T % 8 == 0): it is walked group by group, and a group whose four mask
+    // bytes are zero (almost all of them) costs one shared-memory load.
+    const int tile_px = p.T * p.T, gpr = p.T >> 2, tile_g = p.T * gpr;
     const uint8_t* vm = p.mask ? p.mask + b * img_px : nullptr;
-    auto is_cand = [&](int t, int& idx, float& v) {
-        const int ly = t / p.T, lx = t - ly * p.T;
-        const int gy = ty * p.T + ly, gx = tx * p.T + lx;
-        if (gy < r || gy >= p.H - r || gx < r || gx >= p.W - r) return false;
-        const int ri = (ly + p.halo) * IT_REG + lx + p.halo;
-        v = S[ri];
-        idx = gy * p.W + gx;
-        return M[ri] != 0 && v > p.thresh && (vm == nullptr || __ldg(vm + idx) != 0);
+    // candidates of tile group t (in pixel order): calls emit(v, idx) for each, returns their number
+    auto group_cands = [&](int t, auto&& emit) {
+        const int ly = t / gpr, lg = t - ly * gpr;
+        const int ri = (ly + p.halo) * IT_G + (p.halo_x >> 2) + lg;
+        const uint32_t mw = M32[ri];
+        if (mw == 0u) return 0;
+        const int gy = ty * p.T + ly;
+        if (gy < R || gy >= p.H - R) return 0;
+        const float4 v4 = S4[ri];
+        const float v[4] = {v4.x, v4.y, v4.z, v4.w};
+        int n = 0;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int gx = tx * p.T + 4 * lg + j;
+            if (!((mw >> (8 * j)) & 0xFFu) || gx < R || gx >= p.W - R || !(v[j] > p.thresh)) continue;
+            const int idx = gy * p.W + gx;
+            if (vm != nullptr && __ldg(vm + idx) == 0) continue;
+            emit(v[j], idx);
+            ++n;
+        }
+        return n;
     };
-    // each thread owns a contiguous run of the tile's pixels, so the segment is filled in pixel order
-    const int per = (tile_px + IT_THREADS - 1) / IT_THREADS;
-    const int t_lo = tid * per, t_hi = min(t_lo + per, tile_px);
+    // each thread owns a contiguous run of the tile's groups, so the segment is filled in pixel order
+    const int per = (tile_g + IT_THREADS - 1) / IT_THREADS;
+    const int t_lo = min(tid * per, tile_g), t_hi = min(t_lo + per, tile_g);
     int mine = 0;
-    for (int t = t_lo; t < t_hi; ++t) {
-        int idx;
-        float v;
-        mine += is_cand(t, idx, v) ? 1 : 0;
-    }
+    for (int t = t_lo; t < t_hi; ++t) mine += group_cands(t, [](float, int) {});
     int incl = mine;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -694,11 +732,9 @@ __global__ void __launch_bounds__(IT_THREADS, 1) k_nms_iter(const __grid_constan
     int pos = base + incl - mine;
     const int seg_id = (b * p.tiles_y + ty) * p.tiles_x + tx;
     uint64_t* seg = p.cand + static_cast<size_t>(seg_id) * tile_px;
-    for (int t = t_lo; t < t_hi; ++t) {
-        int idx;
-        float v;
-        if (is_cand(t, idx, v)) { DKD_ASSERT(pos < tile_px); seg[pos++] = make_key(v, idx); }
-    }
+    if (mine > 0)
+        for (int t = t_lo; t < t_hi; ++t)
+            group_cands(t, [&](float v, int idx) { DKD_ASSERT(pos < tile_px); seg[pos++] = make_key(v, idx); });
     if (tid == IT_THREADS - 1) p.seg_cnt[seg_id] = base + incl;
 }
 
