@@ -57,7 +57,7 @@
  *         textbook a c - b^2 cancels to a rounding residue for a singular prediction); a non-positive second pivot
  *         of the Cholesky recursion is a failure as well.
  *
- * Pins (tests/test_match_pins.py, tests/test_stereo_pins.py, -m "not gpu"): brute-force python loops on tiny
+ * Pins (tests/test_match_pins.py — matching, retrieval, stereo and covariance alike —, -m "not gpu"): brute-force python loops on tiny
  * sets; torch.topk on a float64 matmul; planted duplicates / orthogonal sets / exact ties; the Lowe test on hand
  * distances; closed-form triangulation of planted 3-D points; a 2x2 Cholesky worked by hand
  * (tests/golden/chol2x2.txt); Omega^T Omega Sigma_eff = I; the isotropic fallback.
