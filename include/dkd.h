@@ -85,6 +85,14 @@ typedef struct {
     int max_batch, max_h, max_w;
     int max_top_k;              /* <= DKD_MAX_TOP_K */
     int max_dim;                /* max D (0 = keypoints only) */
+    /* The fields below may all be 0 (a zero-initialised struct behaves as before they existed). */
+    int max_radius;             /* largest r a call may pass, 1..DKD_MAX_RADIUS; 0 = DKD_MAX_RADIUS.  A call with a larger r
+                                   returns DKD_ERR_CAPACITY. */
+    int max_match_n;            /* dkd_match: largest Na / Nb; > 0 sizes the matcher's scratch at create, so that no dkd_match
+                                   call within (max_match_n, max_match_pairs) ever allocates — also not the first one, which
+                                   may then be made inside a stream capture.  0 = grown on demand by the calls (cudaMalloc) */
+    int max_match_pairs;        /* dkd_match: largest P for the above; 0 = 2 (temporal + stereo pair) */
+    int max_scan_rows;          /* dkd_retrieval_scan: largest n; > 0 sizes its scratch at create likewise; 0 = on demand */
 } dkd_create_params;
 
 /* Allocates the workspace once on p->device (candidate keys sized for the worst case — every
@@ -273,7 +281,8 @@ int dkd_preprocess(dkd_ctx* ctx, const uint8_t* src, int B, int H, int W, const 
  *   D        64, 128, 192 or 256; dtype must be DKD_F16 (else DKD_ERR_UNSUPPORTED)
  *   out_match device [P,Na] i32: j1 or -1 (no match / padding row);  out_sim device [P,Na,2] f32 (s1, s2) or NULL
  * Asynchronous on `stream`.  Uses a context-owned scratch buffer that is grown (cudaMalloc) when a call needs more than
- * any call before it: such a call must not be made while `stream` is being captured.  The buffer holds the partial results
+ * any call before it: such a call must not be made while `stream` is being captured — unless the context was created with
+ * max_match_n / max_match_pairs (max_scan_rows for the scan) covering the call, which sizes it once at create.  The buffer holds the partial results
  * between the kernels of ONE call: a context must be used from one stream at a time (calls of dkd_match /
  * dkd_retrieval_scan on the same context whose kernels could overlap on the GPU overwrite each other's partials; use
  * one context per stream, or order the streams with events).

@@ -31,7 +31,9 @@ class DKDError(RuntimeError):
 
 class _CreateParams(ctypes.Structure):
     _fields_ = [("device", ctypes.c_int), ("max_batch", ctypes.c_int), ("max_h", ctypes.c_int),
-                ("max_w", ctypes.c_int), ("max_top_k", ctypes.c_int), ("max_dim", ctypes.c_int)]
+                ("max_w", ctypes.c_int), ("max_top_k", ctypes.c_int), ("max_dim", ctypes.c_int),
+                ("max_radius", ctypes.c_int), ("max_match_n", ctypes.c_int), ("max_match_pairs", ctypes.c_int),
+                ("max_scan_rows", ctypes.c_int)]
 
 
 class _PreParams(ctypes.Structure):
@@ -188,14 +190,18 @@ class DKD:
     mirrors dkd_extract_host."""
 
     def __init__(self, max_batch: int, max_h: int, max_w: int, max_top_k: int, max_dim: int = 0,
-                 device: int = 0):
+                 device: int = 0, max_radius: int = 0, max_match_n: int = 0, max_match_pairs: int = 0,
+                 max_scan_rows: int = 0):
+        """dkd_create.  The maxima after `device` may stay 0 (dkd.h): max_match_n / max_match_pairs / max_scan_rows size the
+        scratch of match / retrieval_scan at create, so that those calls never allocate (capture-safe from the first)."""
         self._h = None
         L = load_library()
         if not torch.cuda.is_available():
             raise DKDError(-4, "no CUDA device: libdkd has no CPU fallback")
         self._L = L
         self.device = torch.device("cuda", device)
-        p = _CreateParams(device, max_batch, max_h, max_w, max_top_k, max_dim)
+        p = _CreateParams(device, max_batch, max_h, max_w, max_top_k, max_dim, max_radius, max_match_n, max_match_pairs,
+                          max_scan_rows)
         h = ctypes.c_void_p()
         rc = L.dkd_create(ctypes.byref(p), ctypes.byref(h))
         if rc != 0:

@@ -373,6 +373,7 @@ int validate_shapes(dkd_ctx* ctx, const ExtractArgs& a) {
             return fail(ctx, DKD_ERR_UNSUPPORTED, "desc_dtype must be DKD_F32 or DKD_F16");
     }
     if (a.r > DKD_MAX_RADIUS) return fail(ctx, DKD_ERR_UNSUPPORTED, "r > DKD_MAX_RADIUS");
+    if (ctx->p.max_radius > 0 && a.r > ctx->p.max_radius) return fail(ctx, DKD_ERR_CAPACITY, "r above the dkd_create max_radius");
     if (a.nms_iters > 0) {
         const long long halo = (2LL * a.nms_iters + 1) * a.r;
         if (halo > 40) return fail(ctx, DKD_ERR_UNSUPPORTED, "iterated NMS: (2 nms_iters + 1) r must be <= 40");
@@ -673,6 +674,14 @@ int dkd_create(const dkd_create_params* p, dkd_ctx** out) {
         snprintf(g_create_error, sizeof(g_create_error), "max_top_k > DKD_MAX_TOP_K");
         return DKD_ERR_UNSUPPORTED;
     }
+    if (p->max_radius < 0 || p->max_match_n < 0 || p->max_match_pairs < 0 || p->max_scan_rows < 0) {
+        snprintf(g_create_error, sizeof(g_create_error), "invalid maxima (max_radius / max_match_n / max_match_pairs / max_scan_rows < 0)");
+        return DKD_ERR_INVALID_ARG;
+    }
+    if (p->max_radius > DKD_MAX_RADIUS) {
+        snprintf(g_create_error, sizeof(g_create_error), "max_radius > DKD_MAX_RADIUS");
+        return DKD_ERR_UNSUPPORTED;
+    }
     int prev_dev = -1;
     const bool have_prev = cudaGetDevice(&prev_dev) == cudaSuccess;   // the caller's current device is left unchanged
     (void)cudaGetLastError();
@@ -730,6 +739,24 @@ int dkd_create(const dkd_create_params* p, dkd_ctx** out) {
     CKC(cudaMalloc(&ctx->tile_cnt, b_cnt));
     CKC(cudaMalloc(&ctx->sel_idx, b_sel));
     ctx->ws_bytes = b_cand + b_cnt + b_sel;
+    // Scratch of the descriptor consumers, sized once for the declared maxima (upper bounds of what dkd_match /
+    // dkd_retrieval_scan ask dkd_ctx_scratch for), so that those calls never allocate:
+    //   match: both directions of P x splits x N partial records of 16 bytes, splits <= min(16, column tiles of 128);
+    //   scan:  one key per row plus at most 8 spare per warp of the grid (<= 16 warps per SM), the per-warp counts, and
+    //          the similarity of every row when the caller passes out_sim = NULL.
+    if (p->max_match_n > 0) {
+        const size_t n = p->max_match_n, P = p->max_match_pairs > 0 ? p->max_match_pairs : 2;
+        const size_t tiles = (n + 127) / 128, sp = tiles < 16 ? tiles : 16;
+        const size_t bytes = align256(2 * P * sp * n * 16);
+        CKC(cudaMalloc(&ctx->scratch[0], bytes));
+        ctx->scratch_bytes[0] = bytes;
+    }
+    if (p->max_scan_rows > 0) {
+        const size_t n = p->max_scan_rows, nw = 16 * static_cast<size_t>(ctx->num_sms);
+        const size_t bytes = align256((n + 8 * nw) * 8) + align256(nw * 4) + align256(n * 4);
+        CKC(cudaMalloc(&ctx->scratch[1], bytes));
+        ctx->scratch_bytes[1] = bytes;
+    }
 #undef CKC
     if (have_prev) cudaSetDevice(prev_dev);
     *out = ctx;
@@ -758,7 +785,7 @@ int dkd_destroy(dkd_ctx* ctx) {
 const char* dkd_last_error(const dkd_ctx* ctx) { return ctx ? ctx->err : g_create_error; }
 
 size_t dkd_workspace_bytes(const dkd_ctx* ctx) {
-    return ctx ? ctx->ws_bytes + ctx->st_score_bytes + ctx->st_desc_bytes + ctx->st_out_bytes : 0;
+    return ctx ? ctx->ws_bytes + ctx->st_score_bytes + ctx->st_desc_bytes + ctx->st_out_bytes + ctx->scratch_bytes[0] + ctx->scratch_bytes[1] : 0;
 }
 
 int dkd_set_option(dkd_ctx* ctx, int option, int value) {

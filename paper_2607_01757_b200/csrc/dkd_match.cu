@@ -686,6 +686,14 @@ cudaError_t dkd_match_setup_device() {
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_match_tc<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, 204 * 1024);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan<DKD_F16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan<DKD_F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+    // The remaining kernels of this file are loaded now as well (the runtime loads device functions lazily, on first use):
+    // a first dkd_match / dkd_retrieval_scan made inside a stream capture must not trigger a module load there.
+    cudaFuncAttributes fa;
+    if (e == cudaSuccess) e = cudaFuncGetAttributes(&fa, k_match_finalize);
+    if (e == cudaSuccess) e = cudaFuncGetAttributes(&fa, k_cand_sims);
+    if (e == cudaSuccess) e = cudaFuncGetAttributes(&fa, k_stereo);
+    if (e == cudaSuccess) e = cudaFuncGetAttributes(&fa, k_cov);
+    if (e == cudaSuccess && get_encode() == nullptr) e = cudaErrorNotSupported;   // (also resolves cuTensorMapEncodeTiled once)
     return e;
 }
 

@@ -174,6 +174,45 @@ def test_match_error_codes(ctx):
     assert e.value.code == -1
 
 
+def test_first_match_and_scan_calls_inside_a_capture():
+    """A context created with max_match_n / max_scan_rows owns its scratch from the start: the FIRST dkd_match and the
+    first dkd_retrieval_scan of its life are made while the stream is being captured (no allocation may happen there),
+    the graph is replayed, and the results equal those of an ordinary context."""
+    import paper_2607_01757_b200 as dkd
+    A, B, ca, cb = synth.match_sets(2, 700, 900, 128, seed=5, count_a=[650, 700], count_b=[900, 801])
+    Ad, Bd, cad, cbd = A.cuda(), B.cuda(), ca.cuda(), cb.cuda()
+    db, q = synth.keyframe_db(3000, 1024, seed=4, revisits=[10, 1500], dtype=torch.float16)
+    dbd, qd = db.cuda(), q.cuda()
+    c = dkd.DKD(2, 64, 128, 64, 0, max_match_n=900, max_match_pairs=2, max_scan_rows=3000, max_radius=2)
+    ref = dkd.DKD(2, 64, 128, 64, 0)
+    try:
+        ws0 = c.workspace_bytes
+        assert ws0 > ref.workspace_bytes
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            m, s = c.match(Ad, Bd, cad, cbd, ratio=0.8, mutual=True)
+            sim, cand, csim, cnt = c.retrieval_scan(dbd, qd, n_exclude=50, tau=0.6, max_cand=4, want_sim=False)
+        g.replay()
+        torch.cuda.synchronize()
+        assert c.workspace_bytes == ws0                         # nothing grew
+        m_r, s_r = ref.match(Ad, Bd, cad, cbd, ratio=0.8, mutual=True)
+        _, cand_r, csim_r, cnt_r = ref.retrieval_scan(dbd, qd, n_exclude=50, tau=0.6, max_cand=4, want_sim=False)
+        torch.cuda.synchronize()
+        assert torch.equal(m, m_r) and torch.equal(s, s_r) and int((m >= 0).sum()) > 300
+        assert torch.equal(cand, cand_r) and torch.equal(csim, csim_r) and int(cnt[0]) == int(cnt_r[0]) == 2
+        # max_radius is a capacity of the context
+        sc = torch.zeros((1, 32, 128), device="cuda")
+        with pytest.raises(dkd.DKDError) as e:
+            c.extract(sc, None, 1, 3, 0.2, 8, 0.1)
+        assert e.value.code == -3
+        c.extract(sc, None, 1, 2, 0.2, 8, 0.1)
+    finally:
+        c.close()
+        ref.close()
+    with pytest.raises(dkd.DKDError):
+        dkd.DKD(2, 64, 128, 64, 0, max_radius=5)
+
+
 # ---- retrieval scan -----------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("n,D,dtype", [(700, 12288, torch.float16), (333, 4096, torch.float32), (1, 12288, torch.float16),
                                        (51, 384, torch.float16), (4000, 12288, torch.float16),
