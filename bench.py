@@ -10,9 +10,11 @@ refinement -> descriptor gather) over one 752x480 stereo pair 
 (BASELINE.json configs[1], the configuration the metric "us per 752x480 stereo pair" is quoted on),
 through the C-ABI (`dkd_extract`, one cached CUDA-graph launch).  Per rank:
 
-  * value / ms_per_step : K steps on inputs resident in HBM, CUDA events on the launching stream,
-                          barrier + synchronize on both sides, max over ranks.  Cold inputs: the steps
-                          rotate through R distinct seeded input sets whose touched bytes exceed L2.
+  * value / ms_per_step : the MEDIAN over --blocks (50) back-to-back blocks of exactly K steps each on inputs
+                          resident in HBM, CUDA events on the launching stream (one between blocks), barrier +
+                          synchronize on both sides of the series, max over ranks; min / median / p95 in
+                          `value_blocks`.  Cold inputs: the steps rotate through R distinct seeded input sets
+                          whose touched bytes exceed L2.
   * e2e                 : the same K steps through `dkd_extract_host` with pinned HOST buffers, everything inside
                           the timed region: the score maps are copied host->device, the descriptor corner rows
                           are read in place from the pinned map over PCIe (counted as h2d bytes), and the kernels
@@ -22,8 +24,11 @@ through the C-ABI (`dkd_extract`, one cached CUDA-graph launch).  Per rank:
                           keypoints/s, credited GB/s, and the dominant kernel's duration measured with
                           CUDA events (library measurement mode) against MEASURED_PEAKS.json.
   * variants_c5         : c5 with the heat x reliability and validity-mask variants (NMS credited 8 B / 9 B per pixel).
-  * match / retrieval   : the consumers of the descriptors: tcgen05 matching (tensor roofline) and
-                          the keyframe-database cosine scan (HBM roofline).
+  * match / retrieval   : the consumers of the descriptors: tcgen05 matching (tensor roofline; also with
+                          the mutual check) and the keyframe-database cosine scan (HBM roofline); the f4 kernels per call;
+                          `match.frontend_frame_us`: the composed chain extract(B=4) -> match(P=2) -> stereo validation
+                          captured in one caller graph, at keypoint caps 256 and 1024.
+  * other_configs       : c1 / c3 / c4, cold and warm, min / median / p95 over blocks.
   * cpu_baseline        : the CPU oracle as it stands, timed on this box's host cores on c2 (rank 0); also with one
                           thread, and on a sample of c5.
 
