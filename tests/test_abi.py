@@ -78,3 +78,13 @@ def test_product_never_imports_the_oracle():
         if f.endswith((".py", ".c")):
             txt = open(os.path.join(ROOT, "oracle", f)).read()
             assert "import paper_2607_01757_b200" not in txt and "libdkd.so" not in txt
+
+
+def test_static_matcher_limit_is_the_same_in_header_binding_and_readme():
+    """DKD_MATCH_STATIC_MAX_RECS (the capacity of dkd_match_static's built-in scratch) is stated in three places."""
+    import paper_2607_01757_b200 as dkd
+    hdr = open(os.path.join(ROOT, "include", "dkd.h")).read()
+    m = re.search(r"#define\s+DKD_MATCH_STATIC_MAX_RECS\s+(\d+)", hdr)
+    assert m and int(m.group(1)) == dkd.MATCH_STATIC_MAX_RECS
+    assert int(m.group(1)) * 16 == 1 << 20                       # "1 MiB" in the header and the README
+    assert str(dkd.MATCH_STATIC_MAX_RECS) in open(os.path.join(ROOT, "README.md")).read()
